@@ -1,0 +1,106 @@
+/* boris_demag.h — C ABI of libborisdemag.so
+ *
+ * Demagnetizing field of one rectangular mesh of equal cuboid cells on one
+ * NVIDIA B200 (sm_100a):
+ *
+ *     H(r0) = - sum_r N(r - r0) M(r)              PAPER.md:L323 (Table 1), Eq. 4 (L73) with n = 1
+ *
+ * with N the Newell cell-averaged demagnetizing tensor (Ref. [50]),
+ * evaluated by the convolution theorem with zero padding to twice
+ * the mesh size in every non-flat dimension, organised as the
+ * paper's "pipelined convolution" (the innermost forward FFT, the
+ * point-by-point tensor multiplication and the innermost inverse FFT in a single
+ * kernel launch, for all three vector components at once).
+ *
+ * Conventions
+ *   - SI units: M, H in A/m; cell sides in metres; energy in joules; mu0 = 4 pi 1e-7.
+ *   - M and H are fp32, planar, [3][nz][ny][nx], x fastest: element (c, k, j, i) of
+ *     a component c in {x, y, z} at cell (i, j, k) is at ((c*nz + k)*ny + j)*nx + i.
+ *   - Supported sizes: nx, ny in {2, 4, ..., 1024} with nx >= 4; nz = 1 (2-D mode,
+ *     Nxz and Nyz dropped) or nz in {2, 4, ..., 512}.  Anything else: error -1.
+ *   - All fp32 arithmetic on the device; fp64 only at plan time and in the energy sum.
+ *   - A plan owns the kernel spectrum, twiddle tables and workspace on the device
+ *     that was current when it was created.  It may be used from one stream at a
+ *     time (the workspace is shared).  The caller owns M, H and E.
+ *   - Return codes: 0 ok; -1 invalid argument; -2 CUDA error; -3 out of memory.
+ *     boris_demag_last_error() returns a thread-local message for the last failure.
+ *   - There is no CPU fallback: without a CUDA device plan_create fails with -2.
+ */
+#ifndef BORIS_DEMAG_H
+#define BORIS_DEMAG_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct boris_demag_plan boris_demag_plan;   /* opaque; owns device memory */
+
+/* Build a plan (PAPER.md:L324 tensor, L275 kernel "in the transform space").
+ * nx, ny, nz: cells; hx, hy, hz: cell sides in metres (> 0).
+ * Synchronous; evaluates the tensor and its real, symmetry-reduced spectrum in
+ * fp64 on the device, stores it as fp32.  Returns NULL on failure (see last_error). */
+boris_demag_plan* boris_demag_plan_create(int nx, int ny, int nz, double hx, double hy, double hz);
+
+/* Free everything the plan owns.  NULL is allowed. */
+void boris_demag_plan_destroy(boris_demag_plan* plan);
+
+/* H = -N * M.  M, H: DEVICE pointers, fp32 [3][nz][ny][nx],
+ * 16-byte aligned, must not alias.  H is overwritten.  `stream` is a cudaStream_t
+ * passed as void* (NULL = default stream).  Enqueues kernels and returns at once;
+ * never allocates, never synchronises; bit-identical across calls. */
+int boris_demag_apply(boris_demag_plan* plan, const float* M, float* H, void* stream);
+
+/* E = -(mu0/2) hx hy hz sum_cells M.H  (PAPER.md:L293 relation between field and
+ * energy density, integrated; reading R13).  M, H: DEVICE pointers as in
+ * apply.  E_dev: DEVICE pointer to one double, written asynchronously on `stream`.
+ * Deterministic fixed-shape two-level reduction (warp shuffles, no atomics). */
+int boris_demag_energy(boris_demag_plan* plan, const float* M, const float* H, double* E_dev, void* stream);
+
+/* Same computation with HOST buffers: copies M host->device, applies, computes the
+ * energy, copies H (and E if E_host != NULL) device->host and synchronises `stream`.
+ * M_host, H_host: host pointers, fp32 [3][nz][ny][nx] (pinned memory makes the
+ * copies asynchronous; pageable works).  Uses device staging buffers owned by the
+ * plan (allocated on first use: the first call may return -3). */
+int boris_demag_apply_host(boris_demag_plan* plan, const float* M_host, float* H_host, double* E_host, void* stream);
+
+/* Thread-local description of the last error in this library ("" if none). */
+const char* boris_demag_last_error(void);
+
+/* Introspection for the measurement harness (north_star: "with the number of HBM
+ * passes stated").  Any out pointer may be NULL.
+ *   compulsory_bytes   = 12 N (M in) + 12 N (H out) + 4 ncomp (Px/2+1)(Py/2+1)(Pz/2+1),
+ *                        ncomp = 4 and Pz/2+1 -> 1 when nz = 1, else 6
+ *   designed_hbm_bytes = bytes the kernels of one apply are designed to move to/from HBM
+ *   workspace_bytes    = device memory owned by the plan
+ *   padded[3]          = (Px, Py, Pz)
+ *   kernel_launches    = kernels enqueued by one apply */
+int boris_demag_plan_info(const boris_demag_plan* plan, long long* compulsory_bytes,
+                          long long* designed_hbm_bytes, long long* workspace_bytes,
+                          int padded[3], int* kernel_launches);
+
+/* Copy the plan's kernel spectrum back to the host in natural, symmetry-reduced
+ * order: out[c][kz][ky][kx], c in (xx,yy,zz,xy[,xz,yz]), kz <= Pz/2 (1 plane if nz = 1),
+ * ky <= Py/2, kx <= Px/2, INCLUDING the folded factor -1/(2 Px Py Pz) (DESIGN.md
+ * reading R12).  out must hold ncomp*(Pz/2+1)*(Py/2+1)*(Px/2+1) floats.  Synchronous. */
+int boris_demag_plan_kernel_spectrum(const boris_demag_plan* plan, float* out_host);
+
+/* ---- host-only entry points (no GPU needed; used by the CPU tests) -------------- */
+
+/* The library's own real-space tensor (fp64 Newell formulas near, Gauss quadrature of
+ * the point-dipole tensor over the cell-separation distribution far),
+ * evaluated on the host with the same source code the device kernel compiles.
+ * out[6][nz][ny][nx]: N_c at displacement (i hx, j hy, k hz), c = xx,yy,zz,xy,xz,yz. */
+int boris_demag_tensor_host(int nx, int ny, int nz, double hx, double hy, double hz, double* out);
+
+/* The natural-order reduced kernel spectrum (as boris_demag_plan_kernel_spectrum, in
+ * fp64, same folded factor) computed on the host from boris_demag_tensor_host by the
+ * same cosine/sine-transform code the device kernels compile.  Small meshes only. */
+int boris_demag_spectrum_host(int nx, int ny, int nz, double hx, double hy, double hz, double* out);
+
+/* Library version string, e.g. "boris-demag-b200 0.1 (sm_100a)". */
+const char* boris_demag_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BORIS_DEMAG_H */

@@ -1,0 +1,181 @@
+"""ctypes binding of libborisdemag.so (include/boris_demag.h).  Argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels; torch is used for
+device memory and streams.  There is no CPU fallback: if the shared library is
+missing, or there is no CUDA device, the calls raise.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libborisdemag.so")
+
+_lib = None
+
+
+class DemagError(RuntimeError):
+    pass
+
+
+def lib():
+    """The loaded shared library (raises if it has not been built)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise DemagError(
+                f"{LIB_PATH} not found: build it with `python -m paper_2008_02478_b200.build` "
+                "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        c_int, c_dbl, c_vp = ctypes.c_int, ctypes.c_double, ctypes.c_void_p
+        L.boris_demag_plan_create.restype = c_vp
+        L.boris_demag_plan_create.argtypes = [c_int, c_int, c_int, c_dbl, c_dbl, c_dbl]
+        L.boris_demag_plan_destroy.restype = None
+        L.boris_demag_plan_destroy.argtypes = [c_vp]
+        L.boris_demag_apply.restype = c_int
+        L.boris_demag_apply.argtypes = [c_vp, c_vp, c_vp, c_vp]
+        L.boris_demag_energy.restype = c_int
+        L.boris_demag_energy.argtypes = [c_vp, c_vp, c_vp, c_vp, c_vp]
+        L.boris_demag_apply_host.restype = c_int
+        L.boris_demag_apply_host.argtypes = [c_vp, c_vp, c_vp, c_vp, c_vp]
+        L.boris_demag_last_error.restype = ctypes.c_char_p
+        L.boris_demag_last_error.argtypes = []
+        L.boris_demag_plan_info.restype = c_int
+        L.boris_demag_plan_info.argtypes = [c_vp, ctypes.POINTER(ctypes.c_longlong), ctypes.POINTER(ctypes.c_longlong),
+                                            ctypes.POINTER(ctypes.c_longlong), ctypes.POINTER(c_int), ctypes.POINTER(c_int)]
+        L.boris_demag_plan_kernel_spectrum.restype = c_int
+        L.boris_demag_plan_kernel_spectrum.argtypes = [c_vp, c_vp]
+        L.boris_demag_tensor_host.restype = c_int
+        L.boris_demag_tensor_host.argtypes = [c_int, c_int, c_int, c_dbl, c_dbl, c_dbl, c_vp]
+        L.boris_demag_spectrum_host.restype = c_int
+        L.boris_demag_spectrum_host.argtypes = [c_int, c_int, c_int, c_dbl, c_dbl, c_dbl, c_vp]
+        L.boris_demag_version.restype = ctypes.c_char_p
+        L.boris_demag_version.argtypes = []
+        _lib = L
+    return _lib
+
+
+def last_error():
+    return lib().boris_demag_last_error().decode()
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise DemagError(f"{what} failed ({rc}): {last_error()}")
+
+
+def version():
+    return lib().boris_demag_version().decode()
+
+
+def tensor_host(nx, ny, nz, hx, hy, hz):
+    """boris_demag_tensor_host: the library's real-space tensor, fp64 [6][nz][ny][nx] (host only)."""
+    out = np.empty((6, nz, ny, nx), np.float64)
+    _check(lib().boris_demag_tensor_host(nx, ny, nz, hx, hy, hz, out.ctypes.data), "boris_demag_tensor_host")
+    return out
+
+
+def spectrum_host(nx, ny, nz, hx, hy, hz):
+    """boris_demag_spectrum_host: natural reduced spectrum, fp64 [ncomp][nzr][nyr][nxr] (host only)."""
+    ncomp = 6 if nz > 1 else 4
+    out = np.empty((ncomp, nz + 1 if nz > 1 else 1, ny + 1, nx + 1), np.float64)
+    _check(lib().boris_demag_spectrum_host(nx, ny, nz, hx, hy, hz, out.ctypes.data), "boris_demag_spectrum_host")
+    return out
+
+
+class DemagPlan:
+    """boris_demag_plan_create / apply / energy on the current CUDA device.
+
+    M, H are torch CUDA float32 tensors of shape [3, nz, ny, nx] (contiguous).
+    """
+
+    def __init__(self, nx, ny, nz, hx, hy, hz):
+        self._h = None
+        self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
+        self.h = (float(hx), float(hy), float(hz))
+        h = lib().boris_demag_plan_create(self.nx, self.ny, self.nz, *self.h)
+        if not h:
+            raise DemagError(f"boris_demag_plan_create failed: {last_error()}")
+        self._h = h
+
+    @property
+    def shape(self):
+        return (3, self.nz, self.ny, self.nx)
+
+    def close(self):
+        if self._h:
+            lib().boris_demag_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _ptr(self, t, name):
+        import torch
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()
+                and tuple(t.shape) == self.shape):
+            raise DemagError(f"{name} must be a contiguous CUDA float32 tensor of shape {self.shape}")
+        return t.data_ptr()
+
+    @staticmethod
+    def _stream(stream):
+        import torch
+        s = torch.cuda.current_stream() if stream is None else stream
+        return s.cuda_stream
+
+    def apply(self, M, H, stream=None):
+        """H <- -N * M on `stream` (default: torch's current stream).  Asynchronous."""
+        _check(lib().boris_demag_apply(self._h, self._ptr(M, "M"), self._ptr(H, "H"), self._stream(stream)),
+               "boris_demag_apply")
+        return H
+
+    def energy(self, M, H, E=None, stream=None):
+        """E (CUDA float64 tensor of 1 element) <- -(mu0/2) dV sum M.H.  Asynchronous."""
+        import torch
+        if E is None:
+            E = torch.empty(1, dtype=torch.float64, device=M.device)
+        _check(lib().boris_demag_energy(self._h, self._ptr(M, "M"), self._ptr(H, "H"), E.data_ptr(),
+                                        self._stream(stream)), "boris_demag_energy")
+        return E
+
+    def apply_host(self, M_host, H_host, want_energy=True, stream=None):
+        """Host-buffer entry point: numpy/torch CPU float32 arrays [3][nz][ny][nx]; returns E (float) or None."""
+        mp, hp = _host_ptr(M_host, self.shape), _host_ptr(H_host, self.shape)
+        e = ctypes.c_double(0.0)
+        _check(lib().boris_demag_apply_host(self._h, mp, hp, ctypes.addressof(e) if want_energy else None,
+                                            self._stream(stream)), "boris_demag_apply_host")
+        return e.value if want_energy else None
+
+    def info(self):
+        comp, des, ws = ctypes.c_longlong(), ctypes.c_longlong(), ctypes.c_longlong()
+        padded = (ctypes.c_int * 3)()
+        nl = ctypes.c_int()
+        _check(lib().boris_demag_plan_info(self._h, ctypes.byref(comp), ctypes.byref(des), ctypes.byref(ws), padded,
+                                           ctypes.byref(nl)), "boris_demag_plan_info")
+        return {"compulsory_bytes": comp.value, "designed_hbm_bytes": des.value, "workspace_bytes": ws.value,
+                "padded": tuple(padded), "kernel_launches": nl.value}
+
+    def kernel_spectrum(self):
+        """Natural reduced fp32 spectrum [ncomp][nzr][nyr][nxr] read back from the device."""
+        ncomp = 6 if self.nz > 1 else 4
+        out = np.empty((ncomp, self.nz + 1 if self.nz > 1 else 1, self.ny + 1, self.nx + 1), np.float32)
+        _check(lib().boris_demag_plan_kernel_spectrum(self._h, out.ctypes.data), "boris_demag_plan_kernel_spectrum")
+        return out
+
+
+def _host_ptr(a, shape):
+    try:
+        import torch
+        if isinstance(a, torch.Tensor):
+            if a.is_cuda or a.dtype != torch.float32 or not a.is_contiguous() or tuple(a.shape) != tuple(shape):
+                raise DemagError(f"host tensor must be contiguous CPU float32 of shape {shape}")
+            return a.data_ptr()
+    except ImportError:
+        pass
+    if not (isinstance(a, np.ndarray) and a.dtype == np.float32 and a.flags.c_contiguous and a.shape == tuple(shape)):
+        raise DemagError(f"host array must be C-contiguous float32 of shape {shape}")
+    return a.ctypes.data

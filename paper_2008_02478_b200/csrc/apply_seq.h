@@ -1,0 +1,124 @@
+// apply_seq.h — launch configuration and the launch sequence of one demag evaluation,
+// written against a Launcher policy so that boris_demag.cu (CUDA launches) and the
+// host emulation of the CPU tests (tests/emu) step through the same code.
+#pragma once
+#include <cmath>
+#include <vector>
+
+#include "kernels.h"
+#include "khat_layout.h"
+
+namespace bd {
+
+struct LaunchCfg {
+    int rb;        // rows per block of XFwd / XInv
+    int nb_y2d;    // kx slots per block of Y2D
+    int nb_y;      // rows per block of YFwd / YInv
+    int cs;        // kx slots per chunk of the 3-D path
+    int ty;        // y positions per block of ZFused
+};
+
+inline LaunchCfg make_launch_cfg(int nx, int ny, int nz) {
+    LaunchCfg c;
+    const int Py = 2 * ny, Pz = nz > 1 ? 2 * nz : 1;
+    c.rb = nx <= 512 ? 16 : 8;
+    while (c.rb > ny) c.rb >>= 1;
+    c.nb_y2d = Py >= 256 ? 1 : 256 / Py;
+    c.nb_y = Py >= 1024 ? 2 : 2048 / Py;
+    c.ty = Pz <= 128 ? 16 : (Pz <= 256 ? 8 : (Pz <= 512 ? 4 : 2));
+    while (c.ty > Py) c.ty >>= 1;
+    if (nz == 1) c.ty = 1;
+    // kx slots per chunk: the scratch T (~32 MB) stays in the 126 MB L2 between YFwd,
+    // ZFused and YInv, so the y-padded spectrum never reaches HBM
+    const long slot_bytes = 3L * nz * Py * (long)sizeof(float2);
+    long cs = (32L << 20) / slot_bytes;
+    c.cs = (int)(cs < 1 ? 1 : (cs > nx + 1 ? nx + 1 : cs));
+    return c;
+}
+
+// h[k] = exp(-2 pi i k / denom), k < count, rounded once from fp64; exact at quarter turns
+inline void fill_twiddles(float2* h, int count, int denom) {
+    const double pi = 3.14159265358979323846264338327950288;
+    for (int k = 0; k < count; ++k) {
+        if ((4L * k) % denom == 0) {
+            const int quarter = (int)((4L * k) / denom % 4);
+            const float cx[4] = {1.f, 0.f, -1.f, 0.f}, sy[4] = {0.f, -1.f, 0.f, 1.f};
+            h[k].x = cx[quarter]; h[k].y = sy[quarter];
+        } else {
+            const double a = -2.0 * pi * (double)k / (double)denom;
+            h[k].x = (float)std::cos(a);
+            h[k].y = (float)std::sin(a);
+        }
+    }
+}
+
+struct PlanView {
+    int nx, ny, nz;
+    LaunchCfg cfg;
+    const float* Kst;
+    const float2 *tw_x, *tw_xpost, *tw_y, *tw_z;
+    float2 *W, *T;
+};
+
+template <int L> struct IC { static constexpr int value = L; };
+template <class F>
+int dispatch_len(int L, F&& f) {
+    switch (L) {
+        case 4: return f(IC<4>{});
+        case 8: return f(IC<8>{});
+        case 16: return f(IC<16>{});
+        case 32: return f(IC<32>{});
+        case 64: return f(IC<64>{});
+        case 128: return f(IC<128>{});
+        case 256: return f(IC<256>{});
+        case 512: return f(IC<512>{});
+        case 1024: return f(IC<1024>{});
+        case 2048: return f(IC<2048>{});
+        default: return -1;
+    }
+}
+
+struct Grid { unsigned x, y; };
+
+inline int apply_launch_count(int nx, int nz, const LaunchCfg& c) {
+    const int NS = nx + 1;
+    return nz == 1 ? 3 : 2 + 3 * ((NS + c.cs - 1) / c.cs);
+}
+
+// Launcher::run<K>(Grid, const K::Args&) -> 0 on success.
+template <class Launcher>
+int enqueue_apply(Launcher& run, const PlanView& p, const float* M, float* H) {
+    const int nx = p.nx, ny = p.ny, nz = p.nz, NS = nx + 1, Py = 2 * ny, Pz = 2 * nz;
+    const LaunchCfg& c = p.cfg;
+    XArgs xa{M, H, p.W, p.tw_x, p.tw_xpost, ny, nz, c.rb};
+    const Grid gx{(unsigned)(3L * nz * ny / c.rb), 1};
+    int rc = dispatch_len(nx, [&](auto ic) { return run.template run<XFwd<decltype(ic)::value>>(gx, xa); });
+    if (rc) return rc;
+    if (nz == 1) {
+        FusedArgs fa{p.W, p.Kst, p.tw_y, NS, c.nb_y2d, 0, 0, 0, 1};
+        const Grid g{(unsigned)((NS + c.nb_y2d - 1) / c.nb_y2d), 1};
+        rc = dispatch_len(Py, [&](auto ic) { return run.template run<Y2D<decltype(ic)::value>>(g, fa); });
+        if (rc) return rc;
+    } else {
+        const long w_cstride = (long)NS * nz * ny;
+        for (int s0 = 0; s0 < NS; s0 += c.cs) {
+            const int cs = (NS - s0 < c.cs) ? NS - s0 : c.cs;
+            const int rows = cs * nz;
+            const long t_cstride = (long)cs * nz * Py;
+            YArgs yf{p.W + (long)s0 * nz * ny, p.T, ny, Py, w_cstride, t_cstride, rows, c.nb_y, p.tw_y};
+            const Grid gy{(unsigned)((rows + c.nb_y - 1) / c.nb_y), 3};
+            rc = dispatch_len(Py, [&](auto ic) { return run.template run<YPass<decltype(ic)::value, false>>(gy, yf); });
+            if (rc) return rc;
+            FusedArgs fa{p.T, p.Kst, p.tw_z, 0, 0, Py, cs, s0, c.ty};
+            const Grid gz{(unsigned)(Py / c.ty), (unsigned)cs};
+            rc = dispatch_len(Pz, [&](auto ic) { return run.template run<ZFused<decltype(ic)::value>>(gz, fa); });
+            if (rc) return rc;
+            YArgs yi{p.T, p.W + (long)s0 * nz * ny, Py, ny, t_cstride, w_cstride, rows, c.nb_y, p.tw_y};
+            rc = dispatch_len(Py, [&](auto ic) { return run.template run<YPass<decltype(ic)::value, true>>(gy, yi); });
+            if (rc) return rc;
+        }
+    }
+    return dispatch_len(nx, [&](auto ic) { return run.template run<XInv<decltype(ic)::value>>(gx, xa); });
+}
+
+}  // namespace bd

@@ -1,0 +1,460 @@
+// boris_demag.cu — C ABI (include/boris_demag.h), plan construction and kernel launches.
+//
+// Build: nvcc -std=c++17 -O3 -lineinfo -gencode arch=compute_100a,code=sm_100a
+//             -shared -Xcompiler -fPIC -o libborisdemag.so boris_demag.cu
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/boris_demag.h"
+#include "apply_seq.h"
+#include "kernels.h"
+#include "khat_layout.h"
+#include "plan_math.h"
+
+namespace {
+
+using namespace bd;
+
+thread_local std::string g_err;
+
+int fail(int code, const std::string& msg) { g_err = msg; return code; }
+int cuda_fail(cudaError_t e, const char* what) {
+    const int code = (e == cudaErrorMemoryAllocation) ? -3 : -2;
+    return fail(code, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define BD_CUDA(call)                                             \
+    do {                                                          \
+        cudaError_t e_ = (call);                                  \
+        if (e_ != cudaSuccess) return cuda_fail(e_, #call);       \
+    } while (0)
+
+bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+
+// ------------------------------------------------------------------ kernel wrapper
+template <class K, int PH>
+__device__ __forceinline__ void run_phases(const typename K::Args& a, float2* sm) {
+    K::template phase<PH>(threadIdx.x, blockIdx.x, blockIdx.y, a, sm);
+    if constexpr (PH + 1 < K::NPHASES) {
+        __syncthreads();
+        run_phases<K, PH + 1>(a, sm);
+    }
+}
+
+template <class K>
+__global__ void __launch_bounds__(K::NT) phase_kernel(const __grid_constant__ typename K::Args a) {
+    extern __shared__ __align__(16) float2 bd_smem[];
+    run_phases<K, 0>(a, bd_smem);
+}
+
+// CUDA launcher policy of bd::enqueue_apply (apply_seq.h)
+struct CudaLauncher {
+    cudaStream_t st;
+    cudaError_t err = cudaSuccess;
+    template <class K>
+    int run(bd::Grid g, const typename K::Args& a) {
+        const size_t smem = (size_t)K::smem_elems(a) * sizeof(float2);
+        static size_t opted = 48 * 1024;           // per kernel instantiation
+        if (smem > opted) {
+            err = cudaFuncSetAttribute(phase_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (err != cudaSuccess) return -2;
+            opted = smem;
+        }
+        phase_kernel<K><<<dim3(g.x, g.y), K::NT, smem, st>>>(a);
+        err = cudaGetLastError();
+        return err == cudaSuccess ? 0 : -2;
+    }
+};
+
+// ------------------------------------------------------------------ plan-time kernels (fp64)
+__global__ void k_tensor(double* N, int ncomp, int nx, int ny, int nz, double hx, double hy, double hz) {
+    const long total = (long)nx * ny * nz;
+    for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total; idx += (long)gridDim.x * blockDim.x) {
+        const int i = (int)(idx % nx), j = (int)((idx / nx) % ny), k = (int)(idx / ((long)nx * ny));
+        double out[6];
+        tensor_point(i, j, k, hx, hy, hz, out);
+        for (int c = 0; c < ncomp; ++c) N[c * total + idx] = out[c];
+    }
+}
+
+// out[c][a2][a1][k] along dimension `dim` of an array in[c][d2][d1][d0]; the transformed
+// dimension has n samples in and n+1 (or 1 if n == 1) frequencies out.
+__global__ void k_real_transform(const double* in, double* out, int ncomp, int d0, int d1, int d2, int dim,
+                                 const double2* cs) {
+    const int n = dim == 0 ? d0 : (dim == 1 ? d1 : d2);
+    const int nk = n > 1 ? n + 1 : 1;
+    const int o0 = dim == 0 ? nk : d0, o1 = dim == 1 ? nk : d1, o2 = dim == 2 ? nk : d2;
+    const long total = (long)ncomp * o2 * o1 * o0;
+    const long stride = dim == 0 ? 1 : (dim == 1 ? d0 : (long)d0 * d1);
+    for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total; idx += (long)gridDim.x * blockDim.x) {
+        const int a0 = (int)(idx % o0), a1 = (int)((idx / o0) % o1), a2 = (int)((idx / ((long)o0 * o1)) % o2);
+        const int c = (int)(idx / ((long)o0 * o1 * o2));
+        const int k = dim == 0 ? a0 : (dim == 1 ? a1 : a2);
+        const long base = (((long)c * d2 + (dim == 2 ? 0 : a2)) * d1 + (dim == 1 ? 0 : a1)) * d0 + (dim == 0 ? 0 : a0);
+        out[idx] = real_transform(in + base, stride, n, k, comp_is_odd(c, dim), cs);
+    }
+}
+
+__global__ void k_scale_sign(double* K, KLayout kl, double scale) {
+    const long per = (long)kl.nzr() * kl.nyr() * kl.nxr(), total = kl.ncomp * per;
+    for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total; idx += (long)gridDim.x * blockDim.x) {
+        const int c = (int)(idx / per);
+        K[idx] *= (c >= 3 ? -scale : scale);      // (-i)^2 of the two odd coordinates
+    }
+}
+
+__global__ void k_fill_storage(float* Kst, KLayout kl, const double* Kred) {
+    const long total = kl.storage_elems();
+    for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total; idx += (long)gridDim.x * blockDim.x)
+        Kst[idx] = (float)storage_value(kl, idx, Kred);
+}
+
+__global__ void k_gather_natural(const float* Kst, KLayout kl, float* out) {
+    const long total = kl.reduced_elems();
+    for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total; idx += (long)gridDim.x * blockDim.x) {
+        long r = idx;
+        const int kx = (int)(r % kl.nxr()); r /= kl.nxr();
+        const int ky = (int)(r % kl.nyr()); r /= kl.nyr();
+        const int kz = (int)(r % kl.nzr()); const int c = (int)(r / kl.nzr());
+        float sign;
+        const long s = storage_index_of(kl, c, kz, ky, kx, sign);
+        out[idx] = sign * Kst[s];
+    }
+}
+
+// ------------------------------------------------------------------ energy (S8)
+constexpr int kEnergyBlocks = 592, kEnergyThreads = 256;
+
+__device__ __forceinline__ double warp_sum(double v) {
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ double block_sum(double v, double* sh) {
+    v = warp_sum(v);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (lane == 0) sh[wid] = v;
+    __syncthreads();
+    const int nw = blockDim.x >> 5;
+    v = (threadIdx.x < nw) ? sh[threadIdx.x] : 0.0;
+    if (wid == 0) v = warp_sum(v);
+    return v;
+}
+
+__global__ void __launch_bounds__(kEnergyThreads) k_energy_partial(const float4* __restrict__ M, const float4* __restrict__ H,
+                                                                    long n4, double* partial) {
+    __shared__ double sh[32];
+    double acc = 0.0;
+    for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < n4; i += (long)gridDim.x * blockDim.x) {
+        const float4 m = __ldg(&M[i]), h = __ldg(&H[i]);
+        acc += (double)m.x * h.x + (double)m.y * h.y + (double)m.z * h.z + (double)m.w * h.w;
+    }
+    acc = block_sum(acc, sh);
+    if (threadIdx.x == 0) partial[blockIdx.x] = acc;
+}
+__global__ void __launch_bounds__(1024) k_energy_final(const double* partial, int n, double factor, double* E) {
+    __shared__ double sh[32];
+    double acc = 0.0;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) acc += partial[i];
+    acc = block_sum(acc, sh);
+    if (threadIdx.x == 0) *E = factor * acc;
+}
+
+int grid_for(long total, int threads) {
+    long g = (total + threads - 1) / threads;
+    return (int)(g < 1 ? 1 : (g > 148L * 64 ? 148L * 64 : g));
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------ plan
+struct boris_demag_plan {
+    int nx, ny, nz;
+    double hx, hy, hz;
+    bd::KLayout kl;
+    int device;
+    // device memory
+    float* Kst = nullptr;            // kernel spectrum, fused-pass order
+    float2* tw_x = nullptr;          // exp(-2 pi i k / LX)
+    float2* tw_xpost = nullptr;      // exp(-2 pi i k / Px), k <= LX/2
+    float2* tw_y = nullptr;          // exp(-2 pi i k / Py)
+    float2* tw_z = nullptr;          // exp(-2 pi i k / Pz)
+    float2* W = nullptr;             // [3][NS][nz][ny]
+    float2* T = nullptr;             // [3][cs][nz][Py]   (nz > 1)
+    double* partial = nullptr;       // energy partial sums
+    float* stage_M = nullptr;        // apply_host staging
+    float* stage_H = nullptr;
+    double* stage_E = nullptr;
+    bd::LaunchCfg cfg;               // launch configuration (apply_seq.h)
+    long bytes = 0;
+};
+
+namespace {
+
+template <class T>
+int dev_alloc(boris_demag_plan* p, T** ptr, size_t count) {
+    const size_t bytes = count * sizeof(T);
+    cudaError_t e = cudaMalloc((void**)ptr, bytes ? bytes : sizeof(T));
+    if (e != cudaSuccess) { *ptr = nullptr; return cuda_fail(e, "cudaMalloc"); }
+    p->bytes += (long)bytes;
+    return 0;
+}
+
+int upload_twiddles(boris_demag_plan* p, float2** dst, int count, int denom) {
+    std::vector<float2> h((size_t)count);
+    bd::fill_twiddles(h.data(), count, denom);
+    if (int rc = dev_alloc(p, dst, (size_t)count)) return rc;
+    BD_CUDA(cudaMemcpy(*dst, h.data(), (size_t)count * sizeof(float2), cudaMemcpyHostToDevice));
+    return 0;
+}
+
+int upload_cs_table(double2** dst, int P) {
+    std::vector<double2> h((size_t)P);
+    for (int m = 0; m < P; ++m) {
+        const double a = 2.0 * bd::kPi * (double)m / (double)P;
+        h[m].x = std::cos(a); h[m].y = std::sin(a);
+        if ((4 * m) % P == 0) {
+            const int quarter = (4 * m) / P % 4;
+            const double cx[4] = {1, 0, -1, 0}, sy[4] = {0, 1, 0, -1};
+            h[m].x = cx[quarter]; h[m].y = sy[quarter];
+        }
+    }
+    BD_CUDA(cudaMalloc((void**)dst, (size_t)P * sizeof(double2)));
+    BD_CUDA(cudaMemcpy(*dst, h.data(), (size_t)P * sizeof(double2), cudaMemcpyHostToDevice));
+    return 0;
+}
+
+// Build the kernel spectrum on the device (fp64), store it as fp32 in fused-pass order.
+int build_spectrum(boris_demag_plan* p) {
+    const bd::KLayout& kl = p->kl;
+    const int nx = p->nx, ny = p->ny, nz = p->nz, nc = kl.ncomp;
+    const long cells = (long)nx * ny * nz;
+    double *dN = nullptr, *dA = nullptr, *dB = nullptr, *dC = nullptr;
+    double2 *csx = nullptr, *csy = nullptr, *csz = nullptr;
+    int rc = 0;
+    auto cleanup = [&]() {
+        cudaFree(dN); cudaFree(dA); cudaFree(dB); cudaFree(dC); cudaFree(csx); cudaFree(csy); cudaFree(csz);
+    };
+#define BD_TRY(call)                                                              \
+    do {                                                                          \
+        cudaError_t e_ = (call);                                                  \
+        if (e_ != cudaSuccess) { rc = cuda_fail(e_, #call); cleanup(); return rc; } \
+    } while (0)
+    const long nA = (long)nc * nz * ny * kl.nxr(), nB = (long)nc * nz * kl.nyr() * kl.nxr(), nC = kl.reduced_elems();
+    BD_TRY(cudaMalloc((void**)&dN, (size_t)nc * cells * sizeof(double)));
+    BD_TRY(cudaMalloc((void**)&dA, (size_t)nA * sizeof(double)));
+    k_tensor<<<grid_for(cells, 128), 128>>>(dN, nc, nx, ny, nz, p->hx, p->hy, p->hz);
+    BD_TRY(cudaGetLastError());
+    if ((rc = upload_cs_table(&csx, kl.Px))) { cleanup(); return rc; }
+    if ((rc = upload_cs_table(&csy, kl.Py))) { cleanup(); return rc; }
+    if ((rc = upload_cs_table(&csz, kl.Pz > 1 ? kl.Pz : 2))) { cleanup(); return rc; }
+    k_real_transform<<<grid_for(nA, 128), 128>>>(dN, dA, nc, nx, ny, nz, 0, csx);
+    BD_TRY(cudaGetLastError());
+    BD_TRY(cudaDeviceSynchronize());
+    cudaFree(dN); dN = nullptr;
+    BD_TRY(cudaMalloc((void**)&dB, (size_t)nB * sizeof(double)));
+    k_real_transform<<<grid_for(nB, 128), 128>>>(dA, dB, nc, kl.nxr(), ny, nz, 1, csy);
+    BD_TRY(cudaGetLastError());
+    BD_TRY(cudaDeviceSynchronize());
+    cudaFree(dA); dA = nullptr;
+    BD_TRY(cudaMalloc((void**)&dC, (size_t)nC * sizeof(double)));
+    k_real_transform<<<grid_for(nC, 128), 128>>>(dB, dC, nc, kl.nxr(), kl.nyr(), nz, 2, csz);
+    BD_TRY(cudaGetLastError());
+    // fold -1/(2 Px Py Pz): minus sign of H = -N*M, FFT normalisation, and the factor 2
+    // each of XFwd's post-pass and XInv's pre-pass leaves out (reading R12)
+    const double scale = -1.0 / (2.0 * (double)kl.Px * (double)kl.Py * (double)kl.Pz);
+    k_scale_sign<<<grid_for(nC, 256), 256>>>(dC, kl, scale);
+    BD_TRY(cudaGetLastError());
+    if ((rc = dev_alloc(p, &p->Kst, (size_t)kl.storage_elems()))) { cleanup(); return rc; }
+    k_fill_storage<<<grid_for(kl.storage_elems(), 256), 256>>>(p->Kst, kl, dC);
+    BD_TRY(cudaGetLastError());
+    BD_TRY(cudaDeviceSynchronize());
+#undef BD_TRY
+    cleanup();
+    return 0;
+}
+
+int check_sizes(int nx, int ny, int nz, double hx, double hy, double hz) {
+    if (!(hx > 0.0) || !(hy > 0.0) || !(hz > 0.0) || !std::isfinite(hx) || !std::isfinite(hy) || !std::isfinite(hz))
+        return fail(-1, "cell sides must be positive and finite");
+    if (!is_pow2(nx) || nx < 4 || nx > 1024) return fail(-1, "nx must be a power of two in [4, 1024]");
+    if (!is_pow2(ny) || ny < 2 || ny > 1024) return fail(-1, "ny must be a power of two in [2, 1024]");
+    if (!(nz == 1 || (is_pow2(nz) && nz >= 2 && nz <= 512))) return fail(-1, "nz must be 1 or a power of two in [2, 512]");
+    return 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* boris_demag_version(void) { return "boris-demag-b200 0.1 (sm_100a)"; }
+const char* boris_demag_last_error(void) { return g_err.c_str(); }
+
+void boris_demag_plan_destroy(boris_demag_plan* p) {
+    if (!p) return;
+    cudaFree(p->Kst); cudaFree(p->tw_x); cudaFree(p->tw_xpost); cudaFree(p->tw_y); cudaFree(p->tw_z);
+    cudaFree(p->W); cudaFree(p->T); cudaFree(p->partial);
+    cudaFree(p->stage_M); cudaFree(p->stage_H); cudaFree(p->stage_E);
+    delete p;
+}
+
+boris_demag_plan* boris_demag_plan_create(int nx, int ny, int nz, double hx, double hy, double hz) {
+    g_err.clear();
+    if (check_sizes(nx, ny, nz, hx, hy, hz)) return nullptr;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { cuda_fail(e, "cudaGetDevice (no CUDA device: this library has no CPU fallback)"); return nullptr; }
+    boris_demag_plan* p = new (std::nothrow) boris_demag_plan();
+    if (!p) { fail(-3, "out of host memory"); return nullptr; }
+    p->nx = nx; p->ny = ny; p->nz = nz; p->hx = hx; p->hy = hy; p->hz = hz; p->device = dev;
+    const int Py = 2 * ny, Pz = nz > 1 ? 2 * nz : 1;
+    p->cfg = bd::make_launch_cfg(nx, ny, nz);
+    p->kl = bd::make_klayout(nx, ny, nz, p->cfg.ty);
+    const bd::KLayout& kl = p->kl;
+
+    int rc = build_spectrum(p);
+    if (!rc) rc = upload_twiddles(p, &p->tw_x, nx, nx);
+    if (!rc) rc = upload_twiddles(p, &p->tw_xpost, nx / 2 + 1, 2 * nx);
+    if (!rc) rc = upload_twiddles(p, &p->tw_y, Py, Py);
+    if (!rc && nz > 1) rc = upload_twiddles(p, &p->tw_z, Pz, Pz);
+    if (!rc) rc = dev_alloc(p, &p->W, (size_t)3 * kl.nxr() * nz * ny);
+    if (!rc && nz > 1) rc = dev_alloc(p, &p->T, (size_t)3 * p->cfg.cs * nz * Py);
+    if (!rc) rc = dev_alloc(p, &p->partial, (size_t)kEnergyBlocks);
+    if (rc) { std::string keep = g_err; boris_demag_plan_destroy(p); g_err = keep; return nullptr; }
+    return p;
+}
+
+int boris_demag_apply(boris_demag_plan* p, const float* M, float* H, void* stream) {
+    if (!p || !M || !H) return fail(-1, "null argument");
+    if (M == H) return fail(-1, "M and H must not alias");
+    if (((uintptr_t)M | (uintptr_t)H) & 15) return fail(-1, "M and H must be 16-byte aligned");
+    CudaLauncher run{(cudaStream_t)stream};
+    const bd::PlanView pv{p->nx, p->ny, p->nz, p->cfg, p->Kst, p->tw_x, p->tw_xpost, p->tw_y, p->tw_z, p->W, p->T};
+    const int rc = bd::enqueue_apply(run, pv, M, H);
+    if (rc == -2) return cuda_fail(run.err, "kernel launch");
+    if (rc) return fail(rc, "unsupported size");
+    return 0;
+}
+
+int boris_demag_energy(boris_demag_plan* p, const float* M, const float* H, double* E_dev, void* stream) {
+    if (!p || !M || !H || !E_dev) return fail(-1, "null argument");
+    if (((uintptr_t)M | (uintptr_t)H) & 15) return fail(-1, "M and H must be 16-byte aligned");
+    cudaStream_t st = (cudaStream_t)stream;
+    const long n4 = 3L * p->nx * p->ny * p->nz / 4;
+    const double factor = -0.5 * (4e-7 * bd::kPi) * p->hx * p->hy * p->hz;
+    k_energy_partial<<<kEnergyBlocks, kEnergyThreads, 0, st>>>((const float4*)M, (const float4*)H, n4, p->partial);
+    BD_CUDA(cudaGetLastError());
+    k_energy_final<<<1, 1024, 0, st>>>(p->partial, kEnergyBlocks, factor, E_dev);
+    BD_CUDA(cudaGetLastError());
+    return 0;
+}
+
+int boris_demag_apply_host(boris_demag_plan* p, const float* M_host, float* H_host, double* E_host, void* stream) {
+    if (!p || !M_host || !H_host) return fail(-1, "null argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t n = (size_t)3 * p->nx * p->ny * p->nz;
+    if (!p->stage_M) {
+        if (int rc = dev_alloc(p, &p->stage_M, n)) return rc;
+        if (int rc = dev_alloc(p, &p->stage_H, n)) return rc;
+        if (int rc = dev_alloc(p, &p->stage_E, 1)) return rc;
+    }
+    BD_CUDA(cudaMemcpyAsync(p->stage_M, M_host, n * sizeof(float), cudaMemcpyHostToDevice, st));
+    if (int rc = boris_demag_apply(p, p->stage_M, p->stage_H, stream)) return rc;
+    if (E_host) {
+        if (int rc = boris_demag_energy(p, p->stage_M, p->stage_H, p->stage_E, stream)) return rc;
+        BD_CUDA(cudaMemcpyAsync(E_host, p->stage_E, sizeof(double), cudaMemcpyDeviceToHost, st));
+    }
+    BD_CUDA(cudaMemcpyAsync(H_host, p->stage_H, n * sizeof(float), cudaMemcpyDeviceToHost, st));
+    BD_CUDA(cudaStreamSynchronize(st));
+    return 0;
+}
+
+int boris_demag_plan_info(const boris_demag_plan* p, long long* compulsory_bytes, long long* designed_hbm_bytes,
+                          long long* workspace_bytes, int padded[3], int* kernel_launches) {
+    if (!p) return fail(-1, "null plan");
+    const bd::KLayout& kl = p->kl;
+    const long long N = (long long)p->nx * p->ny * p->nz;
+    const long long kred = 4LL * kl.ncomp * kl.nxr() * kl.nyr() * kl.nzr();
+    const long long wbytes = 3LL * kl.nxr() * p->nz * p->ny * (long long)sizeof(float2);
+    if (compulsory_bytes) *compulsory_bytes = 24 * N + kred;
+    // M in, W out | W in, stored spectrum in, W out | W in, H out.  The scratch T of the
+    // 3-D path is sized to stay in L2 and is not counted.
+    if (designed_hbm_bytes) *designed_hbm_bytes = 24 * N + 4 * wbytes + 4LL * kl.storage_elems();
+    if (workspace_bytes) *workspace_bytes = p->bytes;
+    if (padded) { padded[0] = kl.Px; padded[1] = kl.Py; padded[2] = kl.Pz; }
+    if (kernel_launches) *kernel_launches = bd::apply_launch_count(p->nx, p->nz, p->cfg);
+    return 0;
+}
+
+int boris_demag_plan_kernel_spectrum(const boris_demag_plan* p, float* out_host) {
+    if (!p || !out_host) return fail(-1, "null argument");
+    const long n = p->kl.reduced_elems();
+    float* d = nullptr;
+    BD_CUDA(cudaMalloc((void**)&d, (size_t)n * sizeof(float)));
+    k_gather_natural<<<grid_for(n, 256), 256>>>(p->Kst, p->kl, d);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaMemcpy(out_host, d, (size_t)n * sizeof(float), cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    if (e != cudaSuccess) return cuda_fail(e, "kernel spectrum read-back");
+    return 0;
+}
+
+// ---- host-only entry points ----------------------------------------------------------
+int boris_demag_tensor_host(int nx, int ny, int nz, double hx, double hy, double hz, double* out) {
+    if (!out || nx < 1 || ny < 1 || nz < 1 || !(hx > 0) || !(hy > 0) || !(hz > 0)) return fail(-1, "invalid argument");
+    const long cells = (long)nx * ny * nz;
+    for (long idx = 0; idx < cells; ++idx) {
+        const int i = (int)(idx % nx), j = (int)((idx / nx) % ny), k = (int)(idx / ((long)nx * ny));
+        double v[6];
+        bd::tensor_point(i, j, k, hx, hy, hz, v);
+        for (int c = 0; c < 6; ++c) out[c * cells + idx] = v[c];
+    }
+    return 0;
+}
+
+int boris_demag_spectrum_host(int nx, int ny, int nz, double hx, double hy, double hz, double* out) {
+    if (!out || nx < 1 || ny < 1 || nz < 1 || !(hx > 0) || !(hy > 0) || !(hz > 0)) return fail(-1, "invalid argument");
+    const int nc = nz > 1 ? 6 : 4;
+    const int nxr = nx + 1, nyr = ny + 1, nzr = nz > 1 ? nz + 1 : 1;
+    const long cells = (long)nx * ny * nz;
+    std::vector<double> N6((size_t)6 * cells);
+    boris_demag_tensor_host(nx, ny, nz, hx, hy, hz, N6.data());
+    auto table = [](int P) {
+        std::vector<double2> t((size_t)P);
+        for (int m = 0; m < P; ++m) {
+            const double a = 2.0 * bd::kPi * m / P;
+            t[m].x = std::cos(a); t[m].y = std::sin(a);
+        }
+        return t;
+    };
+    const auto csx = table(2 * nx), csy = table(2 * ny), csz = table(nz > 1 ? 2 * nz : 2);
+    std::vector<double> A((size_t)nc * nz * ny * nxr), B((size_t)nc * nz * nyr * nxr);
+    for (int c = 0; c < nc; ++c)
+        for (int k = 0; k < nz; ++k)
+            for (int j = 0; j < ny; ++j)
+                for (int kx = 0; kx < nxr; ++kx)
+                    A[(((size_t)c * nz + k) * ny + j) * nxr + kx] =
+                        bd::real_transform(&N6[(((size_t)c * nz + k) * ny + j) * nx], 1, nx, kx, bd::comp_is_odd(c, 0), csx.data());
+    for (int c = 0; c < nc; ++c)
+        for (int k = 0; k < nz; ++k)
+            for (int ky = 0; ky < nyr; ++ky)
+                for (int kx = 0; kx < nxr; ++kx)
+                    B[(((size_t)c * nz + k) * nyr + ky) * nxr + kx] =
+                        bd::real_transform(&A[(((size_t)c * nz + k) * ny) * nxr + kx], nxr, ny, ky, bd::comp_is_odd(c, 1), csy.data());
+    const double scale = -1.0 / (2.0 * (2.0 * nx) * (2.0 * ny) * (nz > 1 ? 2.0 * nz : 1.0));
+    for (int c = 0; c < nc; ++c)
+        for (int kz = 0; kz < nzr; ++kz)
+            for (int ky = 0; ky < nyr; ++ky)
+                for (int kx = 0; kx < nxr; ++kx)
+                    out[(((size_t)c * nzr + kz) * nyr + ky) * nxr + kx] =
+                        (c >= 3 ? -scale : scale) *
+                        bd::real_transform(&B[(((size_t)c * nz) * nyr + ky) * nxr + kx], (long)nyr * nxr, nz, kz, bd::comp_is_odd(c, 2), csz.data());
+    return 0;
+}
+
+}  // extern "C"

@@ -1,0 +1,28 @@
+// hd.h — host/device portability shims.
+//
+// Every arithmetic routine of the library is written as a BD_HD inline function
+// so that the same source compiles (a) with nvcc into the sm_100a kernels and
+// (b) with g++ into the host-side emulation used by the CPU tests
+// (tests/emu/emulate.cpp), which steps the kernels' phases thread by thread.
+// The emulation is test infrastructure: libborisdemag.so never runs it.
+#pragma once
+
+#if defined(__CUDACC__)
+#define BD_HD __host__ __device__ __forceinline__
+#define BD_D __device__ __forceinline__
+#else
+#define BD_HD inline
+#define BD_D inline
+#endif
+
+#if defined(__CUDA_ARCH__)
+#define BD_LDG(p) __ldg(p)
+#define BD_UNROLL _Pragma("unroll")
+#else
+#define BD_LDG(p) (*(p))
+#define BD_UNROLL
+#endif
+
+#include <vector_types.h>   // float2, float4, double2 (plain structs on the host)
+
+BD_HD float2 bd_f2(float x, float y) { float2 r; r.x = x; r.y = y; return r; }

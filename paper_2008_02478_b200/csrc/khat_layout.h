@@ -1,0 +1,99 @@
+// khat_layout.h — where the fused multiply finds the kernel spectrum.
+//
+// Natural, symmetry-reduced spectrum (pin P12):
+//     Kred[c][kz <= Pz/2][ky <= Py/2][kx <= Px/2]      (fp64 at plan time)
+// with the value at a mirrored frequency Py - ky (Pz - kz) equal to the stored one
+// times -1 for the components odd in y (z).  kx needs no mirror (real -> complex in x).
+//
+// Device storage (fp32), in the order the fused kernels meet it (fft_core.h khat_*):
+//   nz == 1 (Y2D, fused dimension y):
+//       K[slot = kx][c (4)][q (RL)][row]                       row = canonical y item
+//   nz  > 1 (ZFused, fused dimension z; y is a plain tile coordinate and keeps all Py
+//            positions of the in-place y FFT, in its digit-reversed order):
+//       K[slot = kx][ytile][c (6)][q (RL)][row][t]             py = ytile*ty + t
+// The entry (q, row) of the fused dimension holds frequency k = f'(row) + F*q; if
+// k > L/2 it is read from the natural array at L - k with the odd-component sign.
+#pragma once
+#include "fft_core.h"
+#include "plan_math.h"
+
+namespace bd {
+
+struct KLayout {
+    int nx, ny, nz;        // cells
+    int Px, Py, Pz;        // padded (Pz = 1 when nz = 1)
+    int ncomp;             // 4 (nz = 1) or 6
+    int Lf;                // fused FFT length: Py (nz = 1) or Pz
+    int RL, nrows;         // last radix and canonical rows of the fused dimension
+    int ty, ntiles;        // y tile of ZFused (ty = ntiles = 1... for nz = 1: ty = 1, ntiles = 1)
+    BD_HD int nxr() const { return nx + 1; }
+    BD_HD int nyr() const { return ny + 1; }
+    BD_HD int nzr() const { return nz > 1 ? nz + 1 : 1; }
+    BD_HD long reduced_elems() const { return (long)ncomp * nzr() * nyr() * nxr(); }
+    BD_HD long storage_elems() const {
+        return nz == 1 ? (long)nxr() * 4 * RL * nrows : (long)nxr() * ntiles * 6 * RL * nrows * ty;
+    }
+    BD_HD long reduced_index(int c, int kz, int ky, int kx) const {
+        return (((long)c * nzr() + kz) * nyr() + ky) * nxr() + kx;
+    }
+};
+
+BD_HD KLayout make_klayout(int nx, int ny, int nz, int ty) {
+    KLayout k;
+    k.nx = nx; k.ny = ny; k.nz = nz;
+    k.Px = 2 * nx; k.Py = 2 * ny; k.Pz = nz > 1 ? 2 * nz : 1;
+    k.ncomp = nz > 1 ? 6 : 4;
+    k.Lf = nz > 1 ? k.Pz : k.Py;
+    k.RL = dec_rlast(k.Lf);
+    k.nrows = khat_rows(k.Lf);
+    k.ty = nz > 1 ? ty : 1;
+    k.ntiles = nz > 1 ? k.Py / ty : 1;
+    return k;
+}
+
+// fold a full frequency k of a length-L dimension to the stored half: returns the
+// reduced index and flips `sign` for components odd in that dimension
+BD_HD int fold_freq(int L, int k, bool odd, double& sign) {
+    if (2 * k > L) { if (odd) sign = -sign; return L - k; }
+    return k;
+}
+
+// value of storage element idx, read from the natural reduced array
+BD_HD double storage_value(const KLayout& kl, long idx, const double* Kred) {
+    double sign = 1.0;
+    if (kl.nz == 1) {
+        const int row = (int)(idx % kl.nrows); idx /= kl.nrows;
+        const int q = (int)(idx % kl.RL); idx /= kl.RL;
+        const int c = (int)(idx % 4); const int slot = (int)(idx / 4);
+        const int k = khat_f_of_row(kl.Py, row) + dec_items(kl.Py) * q;
+        const int kyr = fold_freq(kl.Py, k, comp_is_odd(c, 1), sign);
+        return sign * Kred[kl.reduced_index(c, 0, kyr, slot)];
+    }
+    const int t = (int)(idx % kl.ty); idx /= kl.ty;
+    const int row = (int)(idx % kl.nrows); idx /= kl.nrows;
+    const int q = (int)(idx % kl.RL); idx /= kl.RL;
+    const int c = (int)(idx % 6); idx /= 6;
+    const int tile = (int)(idx % kl.ntiles); const int slot = (int)(idx / kl.ntiles);
+    const int ky = freq_of_pos(kl.Py, tile * kl.ty + t);
+    const int kyr = fold_freq(kl.Py, ky, comp_is_odd(c, 1), sign);
+    const int kz = khat_f_of_row(kl.Pz, row) + dec_items(kl.Pz) * q;
+    const int kzr = fold_freq(kl.Pz, kz, comp_is_odd(c, 2), sign);
+    return sign * Kred[kl.reduced_index(c, kzr, kyr, slot)];
+}
+
+// storage index and sign that hold the natural reduced entry (c, kz, ky, kx)
+BD_HD long storage_index_of(const KLayout& kl, int c, int kz, int ky, int kx, float& sign) {
+    sign = 1.f;
+    const int L = kl.Lf, F = dec_items(L), kf = kl.nz == 1 ? ky : kz;
+    int f = kf % F, q = kf / F;
+    if (2 * f > F) {            // stored under its mirror item, q reversed
+        f = F - f; q = kl.RL - 1 - q;
+        if (comp_is_odd(c, kl.nz == 1 ? 1 : 2)) sign = -1.f;
+    }
+    const int row = khat_row_of_f(L, f);
+    if (kl.nz == 1) return (((long)kx * 4 + c) * kl.RL + q) * kl.nrows + row;
+    const int py = pos_of_freq(kl.Py, ky), tile = py / kl.ty, t = py % kl.ty;
+    return (((((long)kx * kl.ntiles + tile) * 6 + c) * kl.RL + q) * kl.nrows + row) * kl.ty + t;
+}
+
+}  // namespace bd

@@ -1,0 +1,116 @@
+// emulate.cpp — host emulation of the CUDA kernels (TEST INFRASTRUCTURE, CPU tests only).
+//
+// Compiles paper_2008_02478_b200/csrc/{kernels,apply_seq,khat_layout}.h with g++ and
+// steps every kernel block by block, phase by phase, thread by thread — the same
+// phase functions, launch sequence and kernel-spectrum layout the sm_100a build uses.
+// It lets the index logic (digit-reversed orders, mirror rows, transposes, chunking)
+// be checked against the oracle on a machine without a GPU.  libborisdemag.so does not
+// contain or call any of this.
+#include <cmath>
+#include <cstring>
+#include <limits>
+#include <vector>
+
+#include "../../paper_2008_02478_b200/csrc/apply_seq.h"
+
+namespace {
+
+template <class K, int PH>
+void run_phases(int bx, int by, const typename K::Args& a, float2* sm) {
+    for (int tid = 0; tid < K::NT; ++tid) K::template phase<PH>(tid, bx, by, a, sm);
+    if constexpr (PH + 1 < K::NPHASES) run_phases<K, PH + 1>(bx, by, a, sm);
+}
+
+struct HostLauncher {
+    long launches = 0;
+    template <class K>
+    int run(bd::Grid g, const typename K::Args& a) {
+        const long n = K::smem_elems(a);
+        std::vector<float2> sm((size_t)n + 1);
+        const float nan = std::numeric_limits<float>::quiet_NaN();
+        for (unsigned by = 0; by < g.y; ++by)
+            for (unsigned bx = 0; bx < g.x; ++bx) {
+                for (auto& v : sm) { v.x = nan; v.y = nan; }     // shared memory starts undefined
+                run_phases<K, 0>((int)bx, (int)by, a, sm.data());
+            }
+        ++launches;
+        return 0;
+    }
+};
+
+}  // namespace
+
+extern "C" {
+
+// Kred: natural reduced spectrum [ncomp][nzr][nyr][nxr] in fp64 including the folded
+// factor (as boris_demag_spectrum_host returns it).  M, H: fp32 [3][nz][ny][nx].
+// cs_override > 0 forces the number of kx slots per chunk (to exercise chunking).
+int emu_apply(int nx, int ny, int nz, const double* Kred, const float* M, float* H, int cs_override) {
+    using namespace bd;
+    LaunchCfg cfg = make_launch_cfg(nx, ny, nz);
+    if (cs_override > 0) cfg.cs = cs_override;
+    const KLayout kl = make_klayout(nx, ny, nz, cfg.ty);
+    const int Py = 2 * ny, Pz = nz > 1 ? 2 * nz : 1, NS = nx + 1;
+    std::vector<float> Kst((size_t)kl.storage_elems());
+    for (long i = 0; i < kl.storage_elems(); ++i) Kst[(size_t)i] = (float)storage_value(kl, i, Kred);
+    std::vector<float2> twx((size_t)nx), twxp((size_t)nx / 2 + 1), twy((size_t)Py), twz((size_t)(Pz > 1 ? Pz : 1));
+    fill_twiddles(twx.data(), nx, nx);
+    fill_twiddles(twxp.data(), nx / 2 + 1, 2 * nx);
+    fill_twiddles(twy.data(), Py, Py);
+    if (nz > 1) fill_twiddles(twz.data(), Pz, Pz);
+    const float nan = std::numeric_limits<float>::quiet_NaN();
+    float2 poison; poison.x = nan; poison.y = nan;
+    std::vector<float2> W((size_t)3 * NS * nz * ny, poison), T(nz > 1 ? (size_t)3 * cfg.cs * nz * Py : 1, poison);
+    PlanView pv{nx, ny, nz, cfg, Kst.data(), twx.data(), twxp.data(), twy.data(), twz.data(), W.data(), T.data()};
+    HostLauncher run;
+    const int rc = enqueue_apply(run, pv, M, H);
+    if (rc) return rc;
+    return (int)run.launches == apply_launch_count(nx, nz, cfg) ? 0 : -100;
+}
+
+// gather the natural reduced spectrum back out of the storage layout (round trip check)
+int emu_storage_roundtrip(int nx, int ny, int nz, const double* Kred, double* out) {
+    using namespace bd;
+    const LaunchCfg cfg = make_launch_cfg(nx, ny, nz);
+    const KLayout kl = make_klayout(nx, ny, nz, cfg.ty);
+    std::vector<double> Kst((size_t)kl.storage_elems());
+    for (long i = 0; i < kl.storage_elems(); ++i) Kst[(size_t)i] = storage_value(kl, i, Kred);
+    for (int c = 0; c < kl.ncomp; ++c)
+        for (int kz = 0; kz < kl.nzr(); ++kz)
+            for (int ky = 0; ky < kl.nyr(); ++ky)
+                for (int kx = 0; kx < kl.nxr(); ++kx) {
+                    float sign;
+                    const long s = storage_index_of(kl, c, kz, ky, kx, sign);
+                    if (s < 0 || s >= kl.storage_elems()) return -1;
+                    out[kl.reduced_index(c, kz, ky, kx)] = sign * Kst[(size_t)s];
+                }
+    return 0;
+}
+
+int emu_pos_of_freq(int L, int k) { return bd::pos_of_freq(L, k); }
+int emu_freq_of_pos(int L, int p) { return bd::freq_of_pos(L, p); }
+int emu_khat_rows(int L) { return bd::khat_rows(L); }
+int emu_khat_row_of_f(int L, int f) { return bd::khat_row_of_f(L, f); }
+int emu_khat_f_of_row(int L, int r) { return bd::khat_f_of_row(L, r); }
+int emu_dec(int L, int what) { return what < 0 ? bd::dec_np(L) : bd::dec_r(L, what); }
+
+// One forward + inverse pass chain on a single pencil, no multiply: x[0..L/2) -> X (digit
+// reversed, length L) -> back to x[0..L/2) scaled by L.  Used to test the butterflies alone.
+int emu_fft_roundtrip(int L, const float* in_ri, float* spec_ri, float* out_ri) {
+    using namespace bd;
+    std::vector<float2> tw((size_t)L), a((size_t)L), b((size_t)L);
+    fill_twiddles(tw.data(), L, L);
+    for (int i = 0; i < L / 2; ++i) { a[i].x = in_ri[2 * i]; a[i].y = in_ri[2 * i + 1]; }
+    YArgs f{a.data(), b.data(), L, L, 0, 0, 1, 1, tw.data()};
+    YArgs g{b.data(), a.data(), L, L, 0, 0, 1, 1, tw.data()};
+    HostLauncher run;
+    int rc = dispatch_len(L, [&](auto ic) { return run.template run<YPass<decltype(ic)::value, false>>(Grid{1, 1}, f); });
+    if (rc) return rc;
+    for (int i = 0; i < L; ++i) { spec_ri[2 * i] = b[i].x; spec_ri[2 * i + 1] = b[i].y; }
+    rc = dispatch_len(L, [&](auto ic) { return run.template run<YPass<decltype(ic)::value, true>>(Grid{1, 1}, g); });
+    if (rc) return rc;
+    for (int i = 0; i < L / 2; ++i) { out_ri[2 * i] = a[i].x; out_ri[2 * i + 1] = a[i].y; }
+    return 0;
+}
+
+}  // extern "C"
