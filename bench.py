@@ -1,0 +1,390 @@
+"""bench.py — demag evaluations/s of boris_demag_apply (+ energy) on synthetic meshes.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C5] [--impl ours|reference]
+
+A step = one pass of the whole hot path: boris_demag_apply
+followed by boris_demag_energy on one seeded synthetic magnetization field.  The
+headline workload is config C5 (512x512x32, BASELINE.json configs[4]): it is one of
+the two meshes the north_star target names, and its compulsory data (M + H + kernel
+spectrum = 410 MB) exceed the 126 MB L2, so back-to-back steps are HBM-cold.  The
+other four configs are timed too (L2 flushed between steps) and reported under
+"all_configs" of the same JSON line.
+
+Multi-GPU: the path does not shard (every output cell depends on every input cell);
+`--gpus N` runs N independent replicas, one per rank, no data-path collective
+(replicas only), so value = N * evaluations / max-over-ranks time.
+
+`--impl reference` times the fp64 CPU oracle (oracle/, test infrastructure) on the
+host cores instead — a deliberately plain program; the ratio to it says nothing about
+kernel quality, parity and the roofline fraction do.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2008_02478_b200 import workloads as W  # noqa: E402
+
+METRIC = "demag_evaluations_per_s"
+UNIT = "eval/s"
+L2_FLUSH_BYTES = 512 << 20
+FP32_LANES_PER_SM = 128
+
+
+def measured_peaks():
+    """HBM GB/s and SM clock from MEASURED_PEAKS.json (driver-written), else the guide's fallback."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, 1965.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# ----------------------------------------------------------------- ledgers
+def kind_bytes(cfg, info):
+    """Algorithmic HBM bytes of each kernel kind over one evaluation: its inputs + outputs once."""
+    nx, ny, nz = cfg.nx, cfg.ny, cfg.nz
+    N = nx * ny * nz
+    NS = nx + 1
+    w = 8 * 3 * NS * nz * ny                 # x-spectrum W, complex64
+    t = 8 * 3 * NS * nz * 2 * ny             # y-padded scratch T over all chunks
+    kst = info["kernel_storage_bytes"]
+    return {"XFwd": 12 * N + w, "Y2D": 2 * w + kst, "YFwd": w + t, "ZFused": 2 * t + kst, "YInv": t + w,
+            "XInv": w + 12 * N}
+
+
+def path_flops(cfg):
+    """SURVEY.md §8(d) count: 5 P log2 P per complex FFT, real x FFT as half-length complex + post pass."""
+    nx, ny, nz = cfg.nx, cfg.ny, cfg.nz
+    Px, Py, Pz = 2 * nx, 2 * ny, (2 * nz if nz > 1 else 1)
+    NS = nx + 1
+    lg = np.log2
+    fx = 3 * nz * ny * (5 * nx * lg(nx) + 8 * nx)               # forward; inverse the same
+    fy = 3 * nz * NS * 5 * Py * lg(Py)
+    fz = 3 * Py * NS * 5 * Pz * lg(Pz) if nz > 1 else 0.0
+    mul = (30 if nz > 1 else 20) * NS * Py * Pz
+    return float(2 * (fx + fy + fz) + mul)
+
+
+# ----------------------------------------------------------------- clocks
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.path = index, None, None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                         stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        rows = [r.split(",") for r in open(self.path).read().strip().splitlines() if r.count(",") >= 6]
+        os.unlink(self.path)
+        if not rows:
+            return out
+        sm = [float(r[0]) for r in rows if r[0].strip().replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[3 + i].strip() == "Active" for r in rows)]
+        out.update(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=float(rows[0][1]), reasons=reasons,
+                   samples=len(rows), power_w_max=max(float(r[2]) for r in rows))
+        return out
+
+
+# ----------------------------------------------------------------- GPU arm
+def time_config(torch, binding, cfg, steps, warmup, flush, peak_gbs, profile_reps=5):
+    """Times `steps` steps of apply+energy on one config.  flush=True: L2 flushed between steps and each
+    step timed with its own event pair; flush=False: one event pair around all steps (inputs > L2)."""
+    M_host = W.make_input(cfg)
+    plan = binding.DemagPlan(cfg.nx, cfg.ny, cfg.nz, *cfg.h)
+    info = plan.info()
+    M = torch.from_numpy(M_host).cuda()
+    H = torch.empty_like(M)
+    E = torch.zeros(1, dtype=torch.float64, device="cuda")
+    scratch = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda") if flush else None
+    st = torch.cuda.current_stream()
+
+    def step():
+        plan.apply(M, H)
+        plan.energy(M, H, E)
+
+    for _ in range(max(warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    if flush:
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for a, b in ev:
+            scratch.fill_(1)
+            a.record(st)
+            step()
+            b.record(st)
+        torch.cuda.synchronize()
+        ms = sum(a.elapsed_time(b) for a, b in ev)
+    else:
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(st)
+        for _ in range(steps):
+            step()
+        b.record(st)
+        torch.cuda.synchronize()
+        ms = a.elapsed_time(b)
+    # per-kernel device time (event pairs around every launch, on the launching stream)
+    kinds = {}
+    for _ in range(profile_reps):
+        if flush:
+            scratch.fill_(1)
+        for k, (t, n) in plan.apply_timed(M, H).items():
+            kinds.setdefault(k, [0.0, 0])
+            kinds[k][0] += t
+            kinds[k][1] += n
+    ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ems = 0.0
+    for _ in range(profile_reps):
+        if flush:
+            scratch.fill_(1)
+        ea.record(st)
+        plan.energy(M, H, E)
+        eb.record(st)
+        torch.cuda.synchronize()
+        ems += ea.elapsed_time(eb)
+    kb = kind_bytes(cfg, info)
+    per_kind = {k: {"ms_per_eval": t / profile_reps, "launches_per_eval": n // profile_reps,
+                    "algorithmic_bytes": kb[k], "gbs": kb[k] / (t / profile_reps) / 1e6}
+                for k, (t, n) in kinds.items()}
+    per_kind["Energy"] = {"ms_per_eval": ems / profile_reps, "launches_per_eval": 2,
+                          "algorithmic_bytes": 24 * cfg.cells, "gbs": 24 * cfg.cells / (ems / profile_reps) / 1e6}
+    ms_step = ms / steps
+    res = {"config": cfg.name, "mesh": [cfg.nx, cfg.ny, cfg.nz], "padded": list(info["padded"]),
+           "ms_per_step": ms_step, "evals_per_s": 1e3 / ms_step, "mcell_per_s": cfg.cells / ms_step / 1e3,
+           "compulsory_bytes": info["compulsory_bytes"], "designed_hbm_bytes": info["designed_hbm_bytes"],
+           "hbm_roofline_frac": info["compulsory_bytes"] / (ms_step * 1e-3) / (peak_gbs * 1e9),
+           "designed_hbm_passes": info["designed_hbm_bytes"] / info["compulsory_bytes"],
+           "launches_per_step": info["kernel_launches"] + 2, "l2": "flushed between steps" if flush else "inputs > L2",
+           "flops": path_flops(cfg), "kernels": per_kind}
+    return res, plan, (M_host, M, H, E)
+
+
+def time_e2e(torch, plan, cfg, M_host, steps, warmup):
+    """Same metric through boris_demag_apply_host with pinned HOST buffers (H2D + kernels + D2H timed)."""
+    Mp = torch.from_numpy(M_host).pin_memory()
+    Hp = torch.empty_like(Mp).pin_memory()
+    for _ in range(max(1, min(warmup, 3))):
+        plan.apply_host(Mp, Hp)
+    torch.cuda.synchronize()
+    n = max(3, min(steps, 20))
+    t0 = time.perf_counter()
+    for _ in range(n):
+        plan.apply_host(Mp, Hp)              # synchronises the stream before returning
+    dt = time.perf_counter() - t0
+    return n, dt / n, Mp.numel() * 4, Hp.numel() * 4 + 8
+
+
+# ----------------------------------------------------------------- oracle arm (CPU baseline / --impl reference)
+def oracle_sample_config(cfg):
+    """Bounded sample of the workload the fp64 oracle finishes in ~1-2 s per evaluation:
+    the same mesh with at most 2^21 cells (fewer z layers, then fewer y rows)."""
+    nz, ny = cfg.nz, cfg.ny
+    while cfg.nx * ny * nz > (1 << 21) and nz > 1:
+        nz //= 2
+    while cfg.nx * ny * nz > (1 << 21):
+        ny //= 2
+    return W.Config(cfg.name + "-sample", cfg.nx, ny, nz, cfg.hx, cfg.hy, cfg.hz, cfg.Ms, cfg.seed, cfg.texture)
+
+
+def oracle_setup(cfg):
+    from oracle.demag_direct import tensor_table          # the only place bench.py touches oracle/
+    from oracle.demag_fft import demag_fft, kernel_spectrum
+    sc = oracle_sample_config(cfg)
+    M = W.make_input(sc)
+    Khat = kernel_spectrum(sc.shape, sc.h, table=tensor_table(sc.shape, sc.h))     # plan-time, excluded (as the GPU plan)
+    what = (f"{sc.nx}x{sc.ny}x{sc.nz} cells of {cfg.name}'s {cfg.nx}x{cfg.ny}x{cfg.nz} mesh "
+            f"({sc.cells / cfg.cells:.3g} of its cells), fp64 zero-padded FFT convolution oracle/demag_fft.py, "
+            "kernel spectrum precomputed; eval/s scaled by the cell ratio")
+    return sc, M, Khat, (lambda: demag_fft(M, sc.h, Khat=Khat)), what
+
+
+def cpu_baseline(cfg, budget_s=15.0):
+    sc, M, Khat, run, what = oracle_setup(cfg)
+    run()
+    n, t0 = 0, time.perf_counter()
+    while True:
+        run()
+        n += 1
+        dt = time.perf_counter() - t0
+        if dt > budget_s or n >= 20:
+            break
+    cells_per_s = sc.cells * n / dt
+    return {"value": cells_per_s / cfg.cells, "unit": UNIT, "mcell_per_s": cells_per_s / 1e6,
+            "cores": os.cpu_count(), "kind": "oracle", "sample": f"{n} evaluations of {what}",
+            "cpu": cpu_model()}
+
+
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def run_reference(args, cfg):
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    sc, M, Khat, run, what = oracle_setup(cfg)
+    for _ in range(args.warmup):
+        run()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        run()
+    dt = time.perf_counter() - t0
+    value = sc.cells * args.steps / dt / cfg.cells
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{cfg.name} {cfg.nx}x{cfg.ny}x{cfg.nz}", "sample": what},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
+                             "sample": f"each step = one evaluation of {what}", "cpu": cpu_model()},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ----------------------------------------------------------------- main
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", default="C5", choices=sorted(W.CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-all-configs", action="store_true", help="skip the four secondary configs")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    cfg = W.CONFIGS[args.config]
+    args.warmup = max(args.warmup, 0)
+    if args.impl == "reference":
+        run_reference(args, cfg)
+        return
+
+    import torch
+    from paper_2008_02478_b200 import binding, build
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
+    if rank == 0:
+        build.build()
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        dist.barrier()
+    binding.lib()
+    peak_gbs, sm_max_mhz, peak_src = measured_peaks()
+    warmup = max(args.warmup, 3)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- headline: K steps, barrier + synchronize on both sides, device time, max over ranks
+    flush = 24 * cfg.cells < (192 << 20)          # M + H smaller than ~1.5 x L2: flush L2 between steps
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    res, plan, (M_host, M, H, E) = time_config(torch, binding, cfg, args.steps, warmup, flush, peak_gbs)
+    barrier()
+    clocks = sampler.stop()
+    ms_step = res["ms_per_step"]
+    if dist is not None:
+        t = torch.tensor([ms_step], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_step = float(t.item())
+    n_e2e, e2e_s, h2d, d2h = time_e2e(torch, plan, cfg, M_host, args.steps, warmup)
+    if dist is not None:
+        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    if rank != 0:
+        barrier()
+        dist.destroy_process_group()
+        return
+
+    kernels = res["kernels"]
+    dom = max((k for k in kernels if k != "Energy"), key=lambda k: kernels[k]["ms_per_eval"])
+    dk = kernels[dom]
+    launches = max(dk["launches_per_eval"], 1)
+    roofline = {"kernel": dom, "bound": "hbm", "achieved": dk["gbs"], "peak": peak_gbs, "unit": "GB/s",
+                "frac": dk["gbs"] / peak_gbs, "traffic": None, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": dk["algorithmic_bytes"] / launches,
+                "avg_launch_ms": dk["ms_per_eval"] / launches, "launches_per_eval": launches,
+                "share_of_eval": dk["ms_per_eval"] / sum(v["ms_per_eval"] for k, v in kernels.items() if k != "Energy")}
+    alu_peak = 148 * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
+    path = {"compulsory_bytes": res["compulsory_bytes"], "hbm_frac_of_peak": res["compulsory_bytes"] / (ms_step * 1e-3) / (peak_gbs * 1e9),
+            "designed_hbm_passes": res["designed_hbm_passes"], "flops_5NlogN": res["flops"],
+            "tflops": res["flops"] / (ms_step * 1e-3) / 1e12, "fp32_fma_peak_tflops": alu_peak,
+            "alu_frac_of_peak": res["flops"] / (ms_step * 1e-3) / 1e12 / alu_peak}
+    line = {"metric": METRIC, "value": world * 1e3 / ms_step, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"{cfg.name} {cfg.nx}x{cfg.ny}x{cfg.nz} cells, padded {'x'.join(map(str, res['padded']))}, "
+                                   f"seeded {cfg.texture} texture; step = boris_demag_apply + boris_demag_energy",
+                       "l2": res["l2"], "parallelism": "replicas only" if world > 1 else "single GPU"},
+            "mcell_per_s": world * cfg.cells / ms_step / 1e3,
+            "e2e": {"value": world / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "steps": n_e2e, "api": "boris_demag_apply_host (pinned host M in, H and E out)"},
+            "gpu_launches": res["launches_per_step"] * args.steps,
+            "clocks": clocks, "roofline": roofline, "path_roofline": path, "kernels": kernels}
+    del plan, M, H, E
+    torch.cuda.empty_cache()
+    if world == 1 and not args.no_all_configs:
+        allc = {cfg.name: {k: v for k, v in res.items() if k != "kernels"}}
+        for name in sorted(W.CONFIGS):
+            if name == cfg.name:
+                continue
+            c = W.CONFIGS[name]
+            steps = 200 if c.cells <= (1 << 20) else 50
+            r, p, bufs = time_config(torch, binding, c, steps, 5, 24 * c.cells < (192 << 20), peak_gbs, profile_reps=3)
+            allc[name] = r
+            p.close()
+            del bufs
+            torch.cuda.empty_cache()
+        line["all_configs"] = allc
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(cfg)
+    print(json.dumps(line))
+    if dist is not None:
+        barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -50,6 +50,15 @@ void boris_demag_plan_destroy(boris_demag_plan* plan);
  * never allocates, never synchronises; bit-identical across calls. */
 int boris_demag_apply(boris_demag_plan* plan, const float* M, float* H, void* stream);
 
+/* boris_demag_apply, instrumented for the measurement harness: a CUDA event pair is
+ * recorded on `stream` around every kernel launch, the stream is synchronised, and the
+ * device time is returned summed per kernel kind, in the order
+ *   0 XFwd (S1)  1 Y2D (S2+S4+S6, nz = 1)  2 YFwd (S2)  3 ZFused (S3+S4+S5)  4 YInv (S6)  5 XInv (S7)
+ * ms_by_kind[6] (milliseconds) and launches_by_kind[6] are HOST arrays.  Synchronous;
+ * computes exactly what boris_demag_apply computes (same kernels, same order). */
+int boris_demag_apply_timed(boris_demag_plan* plan, const float* M, float* H, void* stream,
+                            float ms_by_kind[6], int launches_by_kind[6]);
+
 /* E = -(mu0/2) hx hy hz sum_cells M.H  (PAPER.md:L293 relation between field and
  * energy density, integrated; reading R13).  M, H: DEVICE pointers as in
  * apply.  E_dev: DEVICE pointer to one double, written asynchronously on `stream`.

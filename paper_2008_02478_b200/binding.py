@@ -35,6 +35,9 @@ def lib():
         L.boris_demag_plan_destroy.argtypes = [c_vp]
         L.boris_demag_apply.restype = c_int
         L.boris_demag_apply.argtypes = [c_vp, c_vp, c_vp, c_vp]
+        L.boris_demag_apply_timed.restype = c_int
+        L.boris_demag_apply_timed.argtypes = [c_vp, c_vp, c_vp, c_vp, ctypes.POINTER(ctypes.c_float),
+                                              ctypes.POINTER(c_int)]
         L.boris_demag_energy.restype = c_int
         L.boris_demag_energy.argtypes = [c_vp, c_vp, c_vp, c_vp, c_vp]
         L.boris_demag_apply_host.restype = c_int
@@ -133,6 +136,16 @@ class DemagPlan:
                "boris_demag_apply")
         return H
 
+    KINDS = ("XFwd", "Y2D", "YFwd", "ZFused", "YInv", "XInv")
+
+    def apply_timed(self, M, H, stream=None):
+        """boris_demag_apply_timed: {kind: (ms, launches)} of one evaluation.  Synchronous."""
+        ms = (ctypes.c_float * 6)()
+        nl = (ctypes.c_int * 6)()
+        _check(lib().boris_demag_apply_timed(self._h, self._ptr(M, "M"), self._ptr(H, "H"), self._stream(stream),
+                                             ms, nl), "boris_demag_apply_timed")
+        return {k: (ms[i], nl[i]) for i, k in enumerate(self.KINDS) if nl[i]}
+
     def energy(self, M, H, E=None, stream=None):
         """E (CUDA float64 tensor of 1 element) <- -(mu0/2) dV sum M.H.  Asynchronous."""
         import torch
@@ -156,8 +169,10 @@ class DemagPlan:
         nl = ctypes.c_int()
         _check(lib().boris_demag_plan_info(self._h, ctypes.byref(comp), ctypes.byref(des), ctypes.byref(ws), padded,
                                            ctypes.byref(nl)), "boris_demag_plan_info")
+        wbytes = 3 * (self.nx + 1) * self.nz * self.ny * 8
         return {"compulsory_bytes": comp.value, "designed_hbm_bytes": des.value, "workspace_bytes": ws.value,
-                "padded": tuple(padded), "kernel_launches": nl.value}
+                "padded": tuple(padded), "kernel_launches": nl.value,
+                "kernel_storage_bytes": des.value - 24 * self.nx * self.ny * self.nz - 4 * wbytes}
 
     def kernel_spectrum(self):
         """Natural reduced fp32 spectrum [ncomp][nzr][nyr][nxr] read back from the device."""

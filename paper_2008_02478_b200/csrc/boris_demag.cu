@@ -54,11 +54,28 @@ __global__ void __launch_bounds__(K::NT) phase_kernel(const __grid_constant__ ty
 }
 
 // CUDA launcher policy of bd::enqueue_apply (apply_seq.h)
+struct TimedLaunch { int kind; cudaEvent_t t0, t1; };
+
 struct CudaLauncher {
     cudaStream_t st;
     cudaError_t err = cudaSuccess;
+    std::vector<TimedLaunch>* timed = nullptr;     // boris_demag_apply_timed only
     template <class K>
     int run(bd::Grid g, const typename K::Args& a) {
+        if (timed) {
+            TimedLaunch t{K::KIND, nullptr, nullptr};
+            if ((err = cudaEventCreate(&t.t0)) != cudaSuccess) return -2;
+            if ((err = cudaEventCreate(&t.t1)) != cudaSuccess) { cudaEventDestroy(t.t0); return -2; }
+            timed->push_back(t);
+            cudaEventRecord(t.t0, st);
+            const int rc = launch<K>(g, a);
+            cudaEventRecord(t.t1, st);
+            return rc;
+        }
+        return launch<K>(g, a);
+    }
+    template <class K>
+    int launch(bd::Grid g, const typename K::Args& a) {
         const size_t smem = (size_t)K::smem_elems(a) * sizeof(float2);
         static size_t opted = 48 * 1024;           // per kernel instantiation
         if (smem > opted) {
@@ -338,6 +355,32 @@ int boris_demag_apply(boris_demag_plan* p, const float* M, float* H, void* strea
     const int rc = bd::enqueue_apply(run, pv, M, H);
     if (rc == -2) return cuda_fail(run.err, "kernel launch");
     if (rc) return fail(rc, "unsupported size");
+    return 0;
+}
+
+int boris_demag_apply_timed(boris_demag_plan* p, const float* M, float* H, void* stream, float ms_by_kind[6],
+                            int launches_by_kind[6]) {
+    if (!p || !M || !H || !ms_by_kind || !launches_by_kind) return fail(-1, "null argument");
+    if (M == H) return fail(-1, "M and H must not alias");
+    if (((uintptr_t)M | (uintptr_t)H) & 15) return fail(-1, "M and H must be 16-byte aligned");
+    std::vector<TimedLaunch> timed;
+    CudaLauncher run{(cudaStream_t)stream};
+    run.timed = &timed;
+    const bd::PlanView pv{p->nx, p->ny, p->nz, p->cfg, p->Kst, p->tw_x, p->tw_xpost, p->tw_y, p->tw_z, p->W, p->T};
+    int rc = bd::enqueue_apply(run, pv, M, H);
+    cudaError_t e = cudaStreamSynchronize((cudaStream_t)stream);
+    for (int k = 0; k < bd::kNumKinds; ++k) { ms_by_kind[k] = 0.f; launches_by_kind[k] = 0; }
+    for (const TimedLaunch& t : timed) {
+        float ms = 0.f;
+        if (rc == 0 && e == cudaSuccess && cudaEventElapsedTime(&ms, t.t0, t.t1) == cudaSuccess) {
+            ms_by_kind[t.kind] += ms;
+            launches_by_kind[t.kind] += 1;
+        }
+        cudaEventDestroy(t.t0); cudaEventDestroy(t.t1);
+    }
+    if (rc == -2) return cuda_fail(run.err, "kernel launch");
+    if (rc) return fail(rc, "unsupported size");
+    if (e != cudaSuccess) return cuda_fail(e, "cudaStreamSynchronize");
     return 0;
 }
 

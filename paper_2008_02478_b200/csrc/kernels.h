@@ -22,6 +22,9 @@
 
 namespace bd {
 
+// K::KIND numbers the kernels for the per-kernel timing of boris_demag_apply_timed
+constexpr int kNumKinds = 6;   // XFwd, Y2D, YFwd, ZFused, YInv, XInv
+
 // ------------------------------------------------------------------ accessors
 struct SmemPencil {            // contiguous padded pencils, one buffer per component
     float2* base; int cpitch;
@@ -62,6 +65,7 @@ struct XArgs {
 template <int LX>
 struct XFwd {
     using Args = XArgs;
+    static constexpr int KIND = 0;
     static constexpr int NT = 256;
     static constexpr int NP = dec_np(LX);
     static constexpr int NPHASES = NP + 1;
@@ -127,6 +131,7 @@ struct XFwd {
 template <int LX>
 struct XInv {
     using Args = XArgs;
+    static constexpr int KIND = 5;
     static constexpr int NT = 256;
     static constexpr int NP = dec_np(LX);
     static constexpr int NPHASES = NP + 1;
@@ -205,6 +210,7 @@ struct FusedArgs {
 template <int L>
 struct Y2D {
     using Args = FusedArgs;
+    static constexpr int KIND = 1;
     static constexpr int NT = 128;
     static constexpr int NP = dec_np(L);
     static constexpr int NPHASES = 2 * NP - 1;
@@ -265,6 +271,7 @@ struct Y2D {
 template <int L>
 struct ZFused {
     using Args = FusedArgs;
+    static constexpr int KIND = 3;
     static constexpr int NT = 128;
     static constexpr int NP = dec_np(L);
     static constexpr int NPHASES = 2 * NP - 1;
@@ -333,6 +340,7 @@ struct YArgs {
 template <int L, bool INV>
 struct YPass {
     using Args = YArgs;
+    static constexpr int KIND = INV ? 4 : 2;
     static constexpr int NT = 128;
     static constexpr int NP = dec_np(L);
     static constexpr int NPHASES = NP;

@@ -1,0 +1,261 @@
+"""GPU parity: boris_demag_apply / boris_demag_energy (through the C ABI) vs the fp64 oracle.
+
+Acceptance (BASELINE.json north_star): max|dH| <= 1e-5 Ms and relative L2 <= 2e-6.
+Small meshes: every element against the plain double sum.  Configs
+C2-C5: every element against the fp64 FFT oracle, which is itself
+checked here against the sampled plain sum (pin P14), plus sampled outputs directly.
+"""
+import ctypes
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from oracle import newell
+from oracle.demag_direct import demag_at, demag_direct, tensor_table
+from oracle.demag_fft import demag_fft, kernel_spectrum, padded_shape
+from oracle.energy import demag_energy
+from paper_2008_02478_b200 import binding, build, workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_MAX = 1e-5      # x Ms            (north_star)
+TOL_L2 = 2e-6       # relative L2     (north_star)
+TOL_E = 1e-5        # relative, energy (not fixed by BASELINE.json)
+
+
+@pytest.fixture(scope="module", autouse=True)
+def cuda_library():
+    build.build()
+    assert torch.cuda.is_available(), "-m gpu tests need a CUDA device: there is no CPU fallback"
+    torch.cuda.set_device(0)
+    binding.lib()
+
+
+def gpu_apply(plan, M_host, want_energy=False):
+    M = torch.from_numpy(M_host).cuda()
+    H = torch.full_like(M, float("nan"))
+    plan.apply(M, H)
+    E = plan.energy(M, H) if want_energy else None
+    torch.cuda.synchronize()
+    Hh = H.cpu().numpy()
+    return (Hh, float(E.item())) if want_energy else Hh
+
+
+def errors(H, H_ref, Ms):
+    err = np.abs(H.astype(np.float64) - H_ref)
+    return err.max() / Ms, np.sqrt((err ** 2).sum() / (H_ref ** 2).sum())
+
+
+def assert_parity(H, H_ref, Ms):
+    assert np.isfinite(H).all()
+    emax, el2 = errors(H, H_ref, Ms)
+    assert emax <= TOL_MAX, f"max|dH|/Ms = {emax:.3e}"
+    assert el2 <= TOL_L2, f"rel L2 = {el2:.3e}"
+    return emax, el2
+
+
+# ----------------------------------------------------------------- small meshes, plain double sum
+SMALL = [
+    # (nz, ny, nx), h, texture
+    ((1, 2, 4), (5e-9, 5e-9, 3e-9), "random"),        # smallest supported mesh
+    ((1, 32, 32), (5e-9, 5e-9, 3e-9), "random"),      # C1
+    ((1, 8, 64), (5e-9, 4e-9, 3e-9), "vortex"),       # ragged: fewer rows than a block holds
+    ((1, 64, 4), (2e-9, 3e-9, 1e-9), "helix"),
+    ((2, 2, 4), (2e-9, 2e-9, 1e-9), "random"),        # smallest 3-D mesh
+    ((2, 8, 16), (5e-9, 4e-9, 3e-9), "random"),
+    ((4, 16, 8), (2e-9, 2e-9, 1e-9), "helix"),
+    ((8, 4, 32), (2e-9, 3e-9, 4e-9), "random"),
+    ((16, 8, 8), (2e-9, 2e-9, 2e-9), "random"),
+]
+
+
+@pytest.mark.parametrize("shape,h,texture", SMALL)
+def test_small_meshes_match_the_plain_double_sum(shape, h, texture):
+    nz, ny, nx = shape
+    Ms = 8e5
+    M = W.make_texture(texture, shape, Ms, seed=21)
+    plan = binding.DemagPlan(nx, ny, nz, *h)
+    H, E = gpu_apply(plan, M, want_energy=True)
+    H_ref = demag_direct(M, h)
+    assert_parity(H, H_ref, Ms)
+    E_ref = demag_energy(M, H_ref, h)
+    assert abs(E - E_ref) <= TOL_E * abs(E_ref)
+    assert E > 0                                             # pin P8: N is positive semi-definite
+    plan.close()
+
+
+# ----------------------------------------------------------------- medium meshes (several tiles / chunks), FFT oracle
+MEDIUM = [
+    ((1, 128, 512), (2e-9, 2e-9, 1e-9), "domains"),
+    ((1, 1024, 16), (2e-9, 2e-9, 1e-9), "random"),        # Py = 2048: three passes
+    ((1, 16, 1024), (4e-9, 4e-9, 4e-9), "helix"),         # LX = 1024
+    ((1, 512, 64), (4e-9, 4e-9, 4e-9), "vortex"),
+    ((32, 64, 16), (2e-9, 2e-9, 1e-9), "helix"),
+    ((64, 16, 64), (2e-9, 2e-9, 2e-9), "random"),
+    ((128, 8, 8), (2e-9, 2e-9, 2e-9), "random"),          # Pz = 256 as in C4
+    ((512, 2, 4), (2e-9, 2e-9, 2e-9), "random"),          # Pz = 1024: largest fused z
+    ((2, 256, 128), (5e-9, 5e-9, 3e-9), "vortex"),
+    ((8, 512, 32), (2e-9, 2e-9, 1e-9), "helix"),          # Py = 1024 as in C5
+]
+
+
+@pytest.mark.parametrize("shape,h,texture", MEDIUM)
+def test_medium_meshes_match_the_fft_oracle(shape, h, texture):
+    nz, ny, nx = shape
+    Ms = 1.1e6
+    M = W.make_texture(texture, shape, Ms, seed=22)
+    plan = binding.DemagPlan(nx, ny, nz, *h)
+    H, E = gpu_apply(plan, M, want_energy=True)
+    tab = tensor_table(shape, h)
+    H_ref = demag_fft(M, h, table=tab)
+    assert_parity(H, H_ref, Ms)
+    # sampled outputs by the plain sum, independent of any FFT
+    tg = W.sample_targets(shape, 12, seed=3)
+    Hs = demag_at(M, h, tg, table=tab)
+    for n, p in enumerate(tg):
+        assert np.abs(H[(slice(None),) + p] - Hs[n]).max() <= TOL_MAX * Ms
+    E_ref = demag_energy(M, H_ref, h)
+    assert abs(E - E_ref) <= TOL_E * abs(E_ref)
+    plan.close()
+
+
+# ----------------------------------------------------------------- the five configs at full size
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C5"])
+def test_config_at_full_size(name):
+    cfg = W.CONFIGS[name]
+    M = W.make_input(cfg)
+    plan = binding.DemagPlan(cfg.nx, cfg.ny, cfg.nz, *cfg.h)
+    H, E = gpu_apply(plan, M, want_energy=True)
+    tab = tensor_table(cfg.shape, cfg.h)
+    if name == "C1":
+        H_ref = demag_direct(M, cfg.h, table=tab)
+    else:
+        Khat = kernel_spectrum(cfg.shape, cfg.h, table=tab)
+        H_ref = demag_fft(M, cfg.h, Khat=Khat)
+        del Khat
+    # pin P14: the FFT oracle agrees with the sampled plain sum before it is trusted
+    tg = W.sample_targets(cfg.shape, 64 if cfg.cells <= 2 ** 21 else 32, seed=5)
+    Hs = demag_at(M, cfg.h, tg, table=tab)
+    for n, p in enumerate(tg):
+        assert np.abs(H_ref[(slice(None),) + p] - Hs[n]).max() <= 1e-9 * cfg.Ms
+        assert np.abs(H[(slice(None),) + p] - Hs[n]).max() <= TOL_MAX * cfg.Ms
+    emax, el2 = assert_parity(H, H_ref, cfg.Ms)
+    E_ref = demag_energy(M, H_ref, cfg.h)
+    assert abs(E - E_ref) <= TOL_E * abs(E_ref)
+    print(f"{name}: max|dH|/Ms = {emax:.3e}, rel L2 = {el2:.3e}, E = {E:.6e} J (oracle {E_ref:.6e})")
+    # the host-buffer entry point gives the same bits
+    H2 = np.empty_like(M)
+    E2 = plan.apply_host(M, H2)
+    assert np.array_equal(H2, H)
+    assert E2 == E
+    plan.close()
+
+
+# ----------------------------------------------------------------- properties and edge cases
+def test_P9_delta_readout_reads_the_whole_signed_tensor():
+    """M = Ms e_b at a corner cell: H_a(t) = -Ms N_ab(t - s) over the whole displacement range."""
+    shape, h, Ms = (4, 16, 32), (5e-9, 4e-9, 3e-9), 8e5
+    nz, ny, nx = shape
+    plan = binding.DemagPlan(nx, ny, nz, *h)
+    tab = tensor_table(shape, h)
+    for s, b in [((0, 0, 0), 0), ((nz - 1, ny - 1, nx - 1), 1), ((0, ny - 1, 0), 2)]:
+        M = np.zeros((3,) + shape, np.float32)
+        M[b][s] = Ms
+        H = gpu_apply(plan, M)
+        ks, js, is_ = np.arange(nz) - s[0], np.arange(ny) - s[1], np.arange(nx) - s[2]
+        for a in range(3):
+            c = newell.SYM_INDEX[a, b]
+            px, py, pz = newell.PARITY[c]
+            ref = tab[c][np.ix_(np.abs(ks), np.abs(js), np.abs(is_))].copy()
+            if px < 0:
+                ref *= np.sign(is_)[None, None, :]
+            if py < 0:
+                ref *= np.sign(js)[None, :, None]
+            if pz < 0:
+                ref *= np.sign(ks)[:, None, None]
+            assert np.abs(H[a] + np.float32(Ms).astype(np.float64) * ref).max() <= TOL_MAX * Ms
+    plan.close()
+
+
+def test_P13_linearity_reciprocity_and_zero_input():
+    shape, h, Ms = (8, 32, 64), (2e-9, 2e-9, 1e-9), 8e5
+    nz, ny, nx = shape
+    plan = binding.DemagPlan(nx, ny, nz, *h)
+    M1 = W.make_texture("random", shape, Ms, seed=1)
+    M2 = W.make_texture("helix", shape, Ms, seed=2)
+    H1, H2 = gpu_apply(plan, M1), gpu_apply(plan, M2)
+    H12 = gpu_apply(plan, (2.0 * M1 - 0.5 * M2).astype(np.float32))
+    assert np.abs(H12 - (2.0 * H1.astype(np.float64) - 0.5 * H2)).max() <= 3 * TOL_MAX * Ms
+    r12, r21 = np.sum(M1.astype(np.float64) * H2), np.sum(M2.astype(np.float64) * H1)
+    assert abs(r12 - r21) <= 1e-5 * np.sum(np.abs(M1.astype(np.float64) * H2))
+    Z = gpu_apply(plan, np.zeros_like(M1))
+    assert np.array_equal(Z, np.zeros_like(Z))                      # empty space is legal input
+    plan.close()
+
+
+def test_P7_uniform_thin_film_hz_close_to_minus_mz():
+    cfg = W.CONFIGS["C2"]
+    plan = binding.DemagPlan(cfg.nx, cfg.ny, cfg.nz, *cfg.h)
+    M = np.zeros((3,) + cfg.shape, np.float32)
+    M[2] = cfg.Ms
+    H = gpu_apply(plan, M)
+    # SURVEY.md pin P7 body factor of C2's film [1024, 1024, 4] nm (golden/newell_self_terms.txt)
+    assert abs(H[2].astype(np.float64).mean() / cfg.Ms + 0.984401655301) < 1e-6
+    assert np.abs(H[:2]).max() <= TOL_MAX * cfg.Ms
+    plan.close()
+
+
+def test_apply_is_bit_identical_across_calls_and_streams():
+    cfg = W.CONFIGS["C2"]
+    M_host = W.make_input(cfg)
+    plan = binding.DemagPlan(cfg.nx, cfg.ny, cfg.nz, *cfg.h)
+    M = torch.from_numpy(M_host).cuda()
+    H1, H2 = torch.empty_like(M), torch.empty_like(M)
+    plan.apply(M, H1)
+    E1 = plan.energy(M, H1)
+    torch.cuda.synchronize()
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        plan.apply(M, H2, stream=s)
+        E2 = plan.energy(M, H2, stream=s)
+    s.synchronize()
+    assert torch.equal(H1, H2) and torch.equal(E1, E2)
+    plan.close()
+
+
+def test_P11_uploaded_spectrum_trace_and_oracle_spectrum():
+    """The fp32 spectrum the kernels read: trace == folded factor at every frequency; equals the oracle's rfftn."""
+    for shape, h in [((1, 64, 128), (2e-9, 2e-9, 1e-9)), ((16, 32, 16), (5e-9, 4e-9, 3e-9))]:
+        nz, ny, nx = shape
+        plan = binding.DemagPlan(nx, ny, nz, *h)
+        K = plan.kernel_spectrum().astype(np.float64)
+        Pz, Py, Px = padded_shape(shape)
+        scale = -1.0 / (2.0 * Px * Py * Pz)
+        assert np.abs((K[0] + K[1] + K[2]) / scale - 1).max() < 1e-6
+        Ko = kernel_spectrum(shape, h)
+        for c in range(K.shape[0]):
+            ref = Ko[c][:K.shape[1], :ny + 1, :nx + 1]
+            assert np.abs(ref.imag).max() < 1e-12
+            assert np.abs(K[c] / scale - ref.real).max() < 2e-7 * max(1.0, np.abs(ref.real).max())
+        info = plan.info()
+        assert info["padded"] == (Px, Py, Pz)
+        ncomp = 4 if nz == 1 else 6
+        assert info["compulsory_bytes"] == 24 * nx * ny * nz + 4 * ncomp * (nx + 1) * (ny + 1) * (nz + 1 if nz > 1 else 1)
+        plan.close()
+
+
+def test_error_codes_on_bad_arguments():
+    plan = binding.DemagPlan(32, 32, 1, 5e-9, 5e-9, 3e-9)
+    M = torch.zeros(3, 1, 32, 32, device="cuda")
+    L = binding.lib()
+    assert L.boris_demag_apply(plan._h, M.data_ptr(), M.data_ptr(), None) == -1          # aliasing
+    assert "alias" in binding.last_error()
+    buf = torch.zeros(3 * 32 * 32 + 4, device="cuda")
+    assert L.boris_demag_apply(plan._h, M.data_ptr(), buf.data_ptr() + 4, None) == -1    # misaligned
+    with pytest.raises(binding.DemagError):
+        plan.apply(M.double(), M)
+    with pytest.raises(binding.DemagError):
+        plan.apply(M[:, :, :16], M)
+    plan.close()
