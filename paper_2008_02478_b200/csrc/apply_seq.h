@@ -7,6 +7,8 @@
 
 #include "kernels.h"
 #include "khat_layout.h"
+#include "xt.h"
+#include "yfused.h"
 
 namespace bd {
 
@@ -16,7 +18,15 @@ struct LaunchCfg {
     int nb_y;      // rows per block of YFwd / YInv
     int cs;        // kx slots per chunk of the 3-D path
     int ty;        // y positions per block of ZFused
+    int tiled;     // 1: tiled path (xt.h / yfused.h), 0: the kernels of kernels.h
+    int cols;      // kx columns per tile
+    int rbt;       // rows per block of XFwdT / XInvT
 };
+
+// kx columns per tile of the tiled path: 3 * L * cols complex = 96 KB of shared memory
+// per block at L >= 512 (two blocks per SM)
+BD_HD constexpr int cols_for(int Ly) { return Ly >= 2048 ? 2 : (Ly >= 1024 ? 4 : 8); }
+inline bool tiled_supported(int nx, int ny, int nz) { return nz == 1; }
 
 inline LaunchCfg make_launch_cfg(int nx, int ny, int nz) {
     LaunchCfg c;
@@ -33,6 +43,10 @@ inline LaunchCfg make_launch_cfg(int nx, int ny, int nz) {
     const long slot_bytes = 3L * nz * Py * (long)sizeof(float2);
     long cs = (32L << 20) / slot_bytes;
     c.cs = (int)(cs < 1 ? 1 : (cs > nx + 1 ? nx + 1 : cs));
+    c.tiled = tiled_supported(nx, ny, nz) ? 1 : 0;
+    c.cols = cols_for(Py);
+    c.rbt = nx >= 512 ? 8 : 4096 / nx;
+    while (c.rbt > ny) c.rbt >>= 1;
     return c;
 }
 
@@ -58,6 +72,8 @@ struct PlanView {
     const float* Kst;
     const float2 *tw_x, *tw_xpost, *tw_y, *tw_z;
     float2 *W, *T;
+    const float2 *ptw_x = nullptr, *ptw_y = nullptr;   // per-pass twiddles (tiled path)
+    float2* V = nullptr;                               // tiled spectrum (tiled path)
 };
 
 template <int L> struct IC { static constexpr int value = L; };
@@ -82,12 +98,44 @@ struct Grid { unsigned x, y; };
 
 inline int apply_launch_count(int nx, int nz, const LaunchCfg& c) {
     const int NS = nx + 1;
+    if (c.tiled) return 3;
     return nz == 1 ? 3 : 2 + 3 * ((NS + c.cs - 1) / c.cs);
+}
+
+// tiled path, nz = 1: XFwdT -> YFused -> XInvT
+template <int COLS, class Launcher>
+int enqueue_tiled_2d(Launcher& run, const PlanView& p, const float* M, float* H) {
+    const int nx = p.nx, ny = p.ny, Py = 2 * ny;
+    const int ntl = (nx + 1 + COLS - 1) / COLS;
+    XTArgs xa{M, H, p.V, p.ptw_x, p.tw_xpost, ny, ntl, p.cfg.rbt};
+    const Grid gx{(unsigned)(3L * ny / p.cfg.rbt), 1};
+    int rc = dispatch_len(nx, [&](auto ic) { return run.template run<XFwdT<decltype(ic)::value, COLS>>(gx, xa); });
+    if (rc) return rc;
+    YFArgs ya{p.V, p.Kst, p.ptw_y, ntl, 1};
+    const Grid gy{(unsigned)ntl, 1};
+    rc = dispatch_len(Py, [&](auto ic) {
+        constexpr int L = decltype(ic)::value;
+        if constexpr (cols_for(L) == COLS) return run.template run<YFused<L, 4, COLS>>(gy, ya);
+        else return -1;
+    });
+    if (rc) return rc;
+    return dispatch_len(nx, [&](auto ic) { return run.template run<XInvT<decltype(ic)::value, COLS>>(gx, xa); });
 }
 
 // Launcher::run<K>(Grid, const K::Args&) -> 0 on success.
 template <class Launcher>
 int enqueue_apply(Launcher& run, const PlanView& p, const float* M, float* H) {
+    if (p.cfg.tiled) {
+        if (p.nz == 1) {
+            switch (p.cfg.cols) {
+                case 2: return enqueue_tiled_2d<2>(run, p, M, H);
+                case 4: return enqueue_tiled_2d<4>(run, p, M, H);
+                case 8: return enqueue_tiled_2d<8>(run, p, M, H);
+                default: return -1;
+            }
+        }
+        return -1;
+    }
     const int nx = p.nx, ny = p.ny, nz = p.nz, NS = nx + 1, Py = 2 * ny, Pz = 2 * nz;
     const LaunchCfg& c = p.cfg;
     XArgs xa{M, H, p.W, p.tw_x, p.tw_xpost, ny, nz, c.rb};

@@ -203,6 +203,9 @@ struct boris_demag_plan {
     float2* tw_z = nullptr;          // exp(-2 pi i k / Pz)
     float2* W = nullptr;             // [3][NS][nz][ny]
     float2* T = nullptr;             // [3][cs][nz][Py]   (nz > 1)
+    float2* V = nullptr;             // tiled path: [3][Pz][ntl][ny][cols]
+    float2* ptw_x = nullptr;         // tiled path: per-pass twiddles of the x / y transforms
+    float2* ptw_y = nullptr;
     double* partial = nullptr;       // energy partial sums
     float* stage_M = nullptr;        // apply_host staging
     float* stage_H = nullptr;
@@ -228,6 +231,20 @@ int upload_twiddles(boris_demag_plan* p, float2** dst, int count, int denom) {
     if (int rc = dev_alloc(p, dst, (size_t)count)) return rc;
     BD_CUDA(cudaMemcpy(*dst, h.data(), (size_t)count * sizeof(float2), cudaMemcpyHostToDevice));
     return 0;
+}
+
+int upload_pass_twiddles(boris_demag_plan* p, float2** dst, int L) {
+    std::vector<float2> h((size_t)bd::ptw_total(L));
+    bd::fill_pass_twiddles(h.data(), L);
+    if (int rc = dev_alloc(p, dst, h.size())) return rc;
+    BD_CUDA(cudaMemcpy(*dst, h.data(), h.size() * sizeof(float2), cudaMemcpyHostToDevice));
+    return 0;
+}
+
+bd::PlanView plan_view(const boris_demag_plan* p) {
+    bd::PlanView pv{p->nx, p->ny, p->nz, p->cfg, p->Kst, p->tw_x, p->tw_xpost, p->tw_y, p->tw_z, p->W, p->T};
+    pv.ptw_x = p->ptw_x; pv.ptw_y = p->ptw_y; pv.V = p->V;
+    return pv;
 }
 
 int upload_cs_table(double2** dst, int P) {
@@ -316,6 +333,7 @@ void boris_demag_plan_destroy(boris_demag_plan* p) {
     if (!p) return;
     cudaFree(p->Kst); cudaFree(p->tw_x); cudaFree(p->tw_xpost); cudaFree(p->tw_y); cudaFree(p->tw_z);
     cudaFree(p->W); cudaFree(p->T); cudaFree(p->partial);
+    cudaFree(p->V); cudaFree(p->ptw_x); cudaFree(p->ptw_y);
     cudaFree(p->stage_M); cudaFree(p->stage_H); cudaFree(p->stage_E);
     delete p;
 }
@@ -331,7 +349,7 @@ boris_demag_plan* boris_demag_plan_create(int nx, int ny, int nz, double hx, dou
     p->nx = nx; p->ny = ny; p->nz = nz; p->hx = hx; p->hy = hy; p->hz = hz; p->device = dev;
     const int Py = 2 * ny, Pz = nz > 1 ? 2 * nz : 1;
     p->cfg = bd::make_launch_cfg(nx, ny, nz);
-    p->kl = bd::make_klayout(nx, ny, nz, p->cfg.ty);
+    p->kl = p->cfg.tiled ? bd::make_klayout_tiled(nx, ny, nz, p->cfg.cols) : bd::make_klayout(nx, ny, nz, p->cfg.ty);
     const bd::KLayout& kl = p->kl;
 
     int rc = build_spectrum(p);
@@ -339,8 +357,17 @@ boris_demag_plan* boris_demag_plan_create(int nx, int ny, int nz, double hx, dou
     if (!rc) rc = upload_twiddles(p, &p->tw_xpost, nx / 2 + 1, 2 * nx);
     if (!rc) rc = upload_twiddles(p, &p->tw_y, Py, Py);
     if (!rc && nz > 1) rc = upload_twiddles(p, &p->tw_z, Pz, Pz);
-    if (!rc) rc = dev_alloc(p, &p->W, (size_t)3 * kl.nxr() * nz * ny);
-    if (!rc && nz > 1) rc = dev_alloc(p, &p->T, (size_t)3 * p->cfg.cs * nz * Py);
+    if (p->cfg.tiled) {
+        const size_t nv = (size_t)3 * Pz * kl.ntl * ny * kl.cols;
+        if (!rc) rc = dev_alloc(p, &p->V, nv);
+        // the padding columns of the last tile are transformed along with the rest: keep them finite
+        if (!rc && cudaMemset(p->V, 0, nv * sizeof(float2)) != cudaSuccess) rc = fail(-2, "cudaMemset");
+        if (!rc) rc = upload_pass_twiddles(p, &p->ptw_x, nx);
+        if (!rc) rc = upload_pass_twiddles(p, &p->ptw_y, Py);
+    } else {
+        if (!rc) rc = dev_alloc(p, &p->W, (size_t)3 * kl.nxr() * nz * ny);
+        if (!rc && nz > 1) rc = dev_alloc(p, &p->T, (size_t)3 * p->cfg.cs * nz * Py);
+    }
     if (!rc) rc = dev_alloc(p, &p->partial, (size_t)kEnergyBlocks);
     if (rc) { std::string keep = g_err; boris_demag_plan_destroy(p); g_err = keep; return nullptr; }
     return p;
@@ -351,7 +378,7 @@ int boris_demag_apply(boris_demag_plan* p, const float* M, float* H, void* strea
     if (M == H) return fail(-1, "M and H must not alias");
     if (((uintptr_t)M | (uintptr_t)H) & 15) return fail(-1, "M and H must be 16-byte aligned");
     CudaLauncher run{(cudaStream_t)stream};
-    const bd::PlanView pv{p->nx, p->ny, p->nz, p->cfg, p->Kst, p->tw_x, p->tw_xpost, p->tw_y, p->tw_z, p->W, p->T};
+    const bd::PlanView pv = plan_view(p);
     const int rc = bd::enqueue_apply(run, pv, M, H);
     if (rc == -2) return cuda_fail(run.err, "kernel launch");
     if (rc) return fail(rc, "unsupported size");
@@ -366,7 +393,7 @@ int boris_demag_apply_timed(boris_demag_plan* p, const float* M, float* H, void*
     std::vector<TimedLaunch> timed;
     CudaLauncher run{(cudaStream_t)stream};
     run.timed = &timed;
-    const bd::PlanView pv{p->nx, p->ny, p->nz, p->cfg, p->Kst, p->tw_x, p->tw_xpost, p->tw_y, p->tw_z, p->W, p->T};
+    const bd::PlanView pv = plan_view(p);
     int rc = bd::enqueue_apply(run, pv, M, H);
     cudaError_t e = cudaStreamSynchronize((cudaStream_t)stream);
     for (int k = 0; k < bd::kNumKinds; ++k) { ms_by_kind[k] = 0.f; launches_by_kind[k] = 0; }
@@ -428,6 +455,11 @@ int boris_demag_plan_info(const boris_demag_plan* p, long long* compulsory_bytes
     // M in, W out | W in, stored spectrum in, W out | W in, H out.  The scratch T of the
     // 3-D path is sized to stay in L2 and is not counted.
     if (designed_hbm_bytes) *designed_hbm_bytes = 24 * N + 4 * wbytes + 4LL * kl.storage_elems();
+    if (designed_hbm_bytes && p->cfg.tiled) {
+        // M in, V out | V in, stored spectrum in, V out | V in, H out
+        const long long vbytes = 3LL * kl.Pz * kl.ntl * p->ny * kl.cols * (long long)sizeof(float2);
+        *designed_hbm_bytes = 24 * N + 4 * vbytes + 4LL * kl.storage_elems();
+    }
     if (workspace_bytes) *workspace_bytes = p->bytes;
     if (padded) { padded[0] = kl.Px; padded[1] = kl.Py; padded[2] = kl.Pz; }
     if (kernel_launches) *kernel_launches = bd::apply_launch_count(p->nx, p->nz, p->cfg);

@@ -26,11 +26,16 @@ struct KLayout {
     int Lf;                // fused FFT length: Py (nz = 1) or Pz
     int RL, nrows;         // last radix and canonical rows of the fused dimension
     int ty, ntiles;        // y tile of ZFused (ty = ntiles = 1... for nz = 1: ty = 1, ntiles = 1)
+    // tiled path (yfused.h): K[kzr][tile][row (NR)][col][c][q (RLy)], fused dimension y
+    int tiled;             // 1: tiled layout below, 0: the layouts above
+    int cols, ntl;         // kx columns per tile, tiles
+    int RLy, Fy, NRy;      // last radix of the y transform, its items, stored rows Fy/2 + 1
     BD_HD int nxr() const { return nx + 1; }
     BD_HD int nyr() const { return ny + 1; }
     BD_HD int nzr() const { return nz > 1 ? nz + 1 : 1; }
     BD_HD long reduced_elems() const { return (long)ncomp * nzr() * nyr() * nxr(); }
     BD_HD long storage_elems() const {
+        if (tiled) return (long)nzr() * ntl * NRy * cols * ncomp * RLy;
         return nz == 1 ? (long)nxr() * 4 * RL * nrows : (long)nxr() * ntiles * 6 * RL * nrows * ty;
     }
     BD_HD long reduced_index(int c, int kz, int ky, int kx) const {
@@ -48,6 +53,13 @@ BD_HD KLayout make_klayout(int nx, int ny, int nz, int ty) {
     k.nrows = khat_rows(k.Lf);
     k.ty = nz > 1 ? ty : 1;
     k.ntiles = nz > 1 ? k.Py / ty : 1;
+    k.tiled = 0; k.cols = 1; k.ntl = nx + 1;
+    k.RLy = dec_rlast(k.Py); k.Fy = k.Py / k.RLy; k.NRy = k.Fy / 2 + 1;
+    return k;
+}
+BD_HD KLayout make_klayout_tiled(int nx, int ny, int nz, int cols) {
+    KLayout k = make_klayout(nx, ny, nz, 1);
+    k.tiled = 1; k.cols = cols; k.ntl = (nx + 1 + cols - 1) / cols;
     return k;
 }
 
@@ -61,6 +73,17 @@ BD_HD int fold_freq(int L, int k, bool odd, double& sign) {
 // value of storage element idx, read from the natural reduced array
 BD_HD double storage_value(const KLayout& kl, long idx, const double* Kred) {
     double sign = 1.0;
+    if (kl.tiled) {
+        const int q = (int)(idx % kl.RLy); idx /= kl.RLy;
+        const int c = (int)(idx % kl.ncomp); idx /= kl.ncomp;
+        const int col = (int)(idx % kl.cols); idx /= kl.cols;
+        const int row = (int)(idx % kl.NRy); idx /= kl.NRy;
+        const int tile = (int)(idx % kl.ntl); const int kzr = (int)(idx / kl.ntl);
+        const int kx = tile * kl.cols + col;
+        if (kx > kl.nx) return 0.0;                      // padding columns of the last tile
+        const int kyr = fold_freq(kl.Py, row + kl.Fy * q, comp_is_odd(c, 1), sign);
+        return sign * Kred[kl.reduced_index(c, kzr, kyr, kx)];
+    }
     if (kl.nz == 1) {
         const int row = (int)(idx % kl.nrows); idx /= kl.nrows;
         const int q = (int)(idx % kl.RL); idx /= kl.RL;
@@ -84,6 +107,14 @@ BD_HD double storage_value(const KLayout& kl, long idx, const double* Kred) {
 // storage index and sign that hold the natural reduced entry (c, kz, ky, kx)
 BD_HD long storage_index_of(const KLayout& kl, int c, int kz, int ky, int kx, float& sign) {
     sign = 1.f;
+    if (kl.tiled) {
+        int f = ky % kl.Fy, q = ky / kl.Fy;
+        if (2 * f > kl.Fy) {        // stored in the row of its mirror item, q reversed
+            f = kl.Fy - f; q = kl.RLy - 1 - q;
+            if (comp_is_odd(c, 1)) sign = -1.f;
+        }
+        return (((((long)kz * kl.ntl + kx / kl.cols) * kl.NRy + f) * kl.cols + kx % kl.cols) * kl.ncomp + c) * kl.RLy + q;
+    }
     const int L = kl.Lf, F = dec_items(L), kf = kl.nz == 1 ? ky : kz;
     int f = kf % F, q = kf / F;
     if (2 * f > F) {            // stored under its mirror item, q reversed

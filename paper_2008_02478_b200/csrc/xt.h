@@ -1,0 +1,144 @@
+// xt.h — x transforms of the tiled 2-D path (nz = 1): S1 and S7 of SURVEY.md §8(a)
+// ("1D FFTs along the x ... direction"; zero padding PAPER.md:L283).
+//
+//   XFwdT  rows of nx reals, zero-padded to Px = 2 nx -> half spectrum kx = 0..nx,
+//          written into the kx-tiled array V[c][0][tile][y][col] that YFused reads
+//   XInvT  the mirror: V -> rows of H, first nx outputs kept
+//
+// The real row is transformed as a complex row of half the padded length
+// (z[m] = x[2m] + i x[2m+1], LX = nx points of which the first nx/2 are non-zero):
+//   2 X[k]      = A + w_k (-i B),   A = Z[k] + conj Z[LX-k],  B = Z[k] - conj Z[LX-k]
+//   2 X[LX-k]   = conj(A - w_k (-i B)),                       w_k = exp(-2 pi i k / Px)
+// and back:
+//   Z[k]    = E' + i O',  E' = Y[k] + conj Y[LX-k],  O' = conj(w_k) (Y[k] - conj Y[LX-k])
+//   Z[LX-k] = conj(E') + i conj(O')
+// The factors 2 are folded into the kernel spectrum (reading R12).
+#pragma once
+#include "yfused.h"
+
+namespace bd {
+
+template <int L>
+struct SRows {                 // shared rows of L points at pitch L + 1, swizzled like a 1-column tile
+    float2* p;
+    static constexpr int PITCH = L + 1;
+    BD_HD float2 get(int row, int e) const { return p[row * PITCH + swz<L, 1>(e)]; }
+    BD_HD void put(int row, int e, float2 v) const { p[row * PITCH + swz<L, 1>(e)] = v; }
+};
+struct GRowsIn {               // rows of a real array read as (x[2m], x[2m+1]) pairs
+    const float* p; long pitch;
+    BD_HD float2 get(int row, int e) const { return BD_LDG(reinterpret_cast<const float2*>(p + row * pitch) + e); }
+};
+struct GRowsOut {
+    float* p; long pitch;
+    BD_HD void put(int row, int e, float2 v) const { reinterpret_cast<float2*>(p + row * pitch)[e] = v; }
+};
+
+struct XTArgs {
+    const float* M;        // [3][ny][nx]
+    float* H;              // [3][ny][nx]            (XInvT)
+    float2* V;             // [3][1][ntl][ny][COLS]
+    const float2* ptw;     // per-pass twiddles of length LX
+    const float2* twx;     // exp(-2 pi i k / Px), k <= LX/2
+    int ny;
+    int ntl;
+    int rb;                // rows (consecutive y of one component) per block; divides ny
+};
+
+// all rows of a block through pass P; a thread keeps its butterfly index (and twiddles)
+// and walks over rows
+template <int LX, int P, bool INV, int NT, class In, class Out>
+BD_HD void x_rows_pass(int tid, int nrows, const In& in, const Out& out, const float2* ptw) {
+    constexpr int IPR = LX / dec_r(LX, P);                 // butterflies per row
+    if constexpr (IPR <= NT) {
+        constexpr int G = NT / IPR;
+        const int it = tid % IPR, rg = tid / IPR;
+        if (rg >= G) return;
+        if constexpr (!INV) fwd_passM<LX, P>(it, rg, G, nrows, in, out, ptw);
+        else inv_passM<LX, P>(it, rg, G, nrows, in, out, ptw);
+    } else {
+        for (int it = tid; it < IPR; it += NT) {
+            if constexpr (!INV) fwd_passM<LX, P>(it, 0, 1, nrows, in, out, ptw);
+            else inv_passM<LX, P>(it, 0, 1, nrows, in, out, ptw);
+        }
+    }
+}
+
+template <int LX, int COLS>
+struct XFwdT {
+    using Args = XTArgs;
+    static constexpr int KIND = kKindXFwdT;
+    static constexpr int NT = 256;
+    static constexpr int NP = dec_np(LX);
+    static constexpr int NPHASES = NP + 1;
+    static BD_HD long smem_elems(const Args& a) { return (long)a.rb * SRows<LX>::PITCH; }
+
+    template <int PH>
+    static BD_HD void phase(int tid, int bx, int by, const Args& a, float2* sm) {
+        const long g0 = (long)bx * a.rb;                   // first global row (c, y0)
+        SRows<LX> s{sm};
+        if constexpr (PH == 0) {
+            GRowsIn in{a.M + g0 * LX, LX};
+            x_rows_pass<LX, 0, false, NT>(tid, a.rb, in, s, a.ptw);
+        } else if constexpr (PH < NP) {
+            x_rows_pass<LX, PH, false, NT>(tid, a.rb, s, s, a.ptw);
+        } else {
+            const int c = (int)(g0 / a.ny), y0 = (int)(g0 - (long)c * a.ny);
+            const int items = (LX / 2 + 1) * a.rb;
+            float2* vc = a.V + (long)c * a.ntl * a.ny * COLS;
+            for (int w = tid; w < items; w += NT) {
+                const int kp = w / a.rb, row = w - kp * a.rb;
+                const int km = LX - kp;
+                const float2 Zk = s.get(row, pos_of_freq(LX, kp));
+                const float2 Zm = s.get(row, pos_of_freq(LX, km & (LX - 1)));
+                const float2 A = bd_f2(Zk.x + Zm.x, Zk.y - Zm.y);
+                const float2 B = bd_f2(Zk.x - Zm.x, Zk.y + Zm.y);
+                const float2 T = pk_cmul(bd_f2(B.y, -B.x), make_tw(BD_LDG(&a.twx[kp])));
+                const float2 Xk = pk_add(A, T), Xm = bd_f2(A.x - T.x, T.y - A.y);
+                const int y = y0 + row;
+                vc[((long)(kp / COLS) * a.ny + y) * COLS + kp % COLS] = Xk;
+                if (2 * kp != LX) vc[((long)(km / COLS) * a.ny + y) * COLS + km % COLS] = Xm;
+            }
+        }
+    }
+};
+
+template <int LX, int COLS>
+struct XInvT {
+    using Args = XTArgs;
+    static constexpr int KIND = kKindXInvT;
+    static constexpr int NT = 256;
+    static constexpr int NP = dec_np(LX);
+    static constexpr int NPHASES = NP + 1;
+    static BD_HD long smem_elems(const Args& a) { return (long)a.rb * SRows<LX>::PITCH; }
+
+    template <int PH>
+    static BD_HD void phase(int tid, int bx, int by, const Args& a, float2* sm) {
+        const long g0 = (long)bx * a.rb;
+        SRows<LX> s{sm};
+        if constexpr (PH == 0) {
+            const int c = (int)(g0 / a.ny), y0 = (int)(g0 - (long)c * a.ny);
+            const int items = (LX / 2 + 1) * a.rb;
+            const float2* vc = a.V + (long)c * a.ntl * a.ny * COLS;
+            for (int w = tid; w < items; w += NT) {
+                const int kp = w / a.rb, row = w - kp * a.rb;
+                const int km = LX - kp, y = y0 + row;
+                float2 Yk = vc[((long)(kp / COLS) * a.ny + y) * COLS + kp % COLS];
+                float2 Ym = vc[((long)(km / COLS) * a.ny + y) * COLS + km % COLS];
+                if (kp == 0) { Yk.y = 0.f; Ym.y = 0.f; }          // DC and Nyquist of a real row are real
+                const float2 E = bd_f2(Yk.x + Ym.x, Yk.y - Ym.y);
+                const float2 D = bd_f2(Yk.x - Ym.x, Yk.y + Ym.y);
+                const float2 O = pk_cmulc(D, make_tw(BD_LDG(&a.twx[kp])));
+                s.put(row, pos_of_freq(LX, kp), bd_f2(E.x - O.y, E.y + O.x));
+                if (kp != 0 && 2 * kp != LX) s.put(row, pos_of_freq(LX, km), bd_f2(E.x + O.y, O.x - E.y));
+            }
+        } else if constexpr (PH < NP) {
+            x_rows_pass<LX, NP - PH, true, NT>(tid, a.rb, s, s, a.ptw);
+        } else {
+            GRowsOut out{a.H + g0 * LX, LX};
+            x_rows_pass<LX, 0, true, NT>(tid, a.rb, s, out, a.ptw);
+        }
+    }
+};
+
+}  // namespace bd

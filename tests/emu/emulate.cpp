@@ -49,7 +49,8 @@ int emu_apply(int nx, int ny, int nz, const double* Kred, const float* M, float*
     using namespace bd;
     LaunchCfg cfg = make_launch_cfg(nx, ny, nz);
     if (cs_override > 0) cfg.cs = cs_override;
-    const KLayout kl = make_klayout(nx, ny, nz, cfg.ty);
+    if (cs_override < 0) cfg.tiled = 0;          // force the untiled kernels
+    const KLayout kl = cfg.tiled ? make_klayout_tiled(nx, ny, nz, cfg.cols) : make_klayout(nx, ny, nz, cfg.ty);
     const int Py = 2 * ny, Pz = nz > 1 ? 2 * nz : 1, NS = nx + 1;
     std::vector<float> Kst((size_t)kl.storage_elems());
     for (long i = 0; i < kl.storage_elems(); ++i) Kst[(size_t)i] = (float)storage_value(kl, i, Kred);
@@ -62,6 +63,11 @@ int emu_apply(int nx, int ny, int nz, const double* Kred, const float* M, float*
     float2 poison; poison.x = nan; poison.y = nan;
     std::vector<float2> W((size_t)3 * NS * nz * ny, poison), T(nz > 1 ? (size_t)3 * cfg.cs * nz * Py : 1, poison);
     PlanView pv{nx, ny, nz, cfg, Kst.data(), twx.data(), twxp.data(), twy.data(), twz.data(), W.data(), T.data()};
+    std::vector<float2> ptwx((size_t)ptw_total(nx)), ptwy((size_t)ptw_total(Py));
+    fill_pass_twiddles(ptwx.data(), nx);
+    fill_pass_twiddles(ptwy.data(), Py);
+    std::vector<float2> V(cfg.tiled ? (size_t)3 * Pz * kl.ntl * ny * kl.cols : 1, bd_f2(0.f, 0.f));
+    pv.ptw_x = ptwx.data(); pv.ptw_y = ptwy.data(); pv.V = V.data();
     HostLauncher run;
     const int rc = enqueue_apply(run, pv, M, H);
     if (rc) return rc;
@@ -72,7 +78,7 @@ int emu_apply(int nx, int ny, int nz, const double* Kred, const float* M, float*
 int emu_storage_roundtrip(int nx, int ny, int nz, const double* Kred, double* out) {
     using namespace bd;
     const LaunchCfg cfg = make_launch_cfg(nx, ny, nz);
-    const KLayout kl = make_klayout(nx, ny, nz, cfg.ty);
+    const KLayout kl = cfg.tiled ? make_klayout_tiled(nx, ny, nz, cfg.cols) : make_klayout(nx, ny, nz, cfg.ty);
     std::vector<double> Kst((size_t)kl.storage_elems());
     for (long i = 0; i < kl.storage_elems(); ++i) Kst[(size_t)i] = storage_value(kl, i, Kred);
     for (int c = 0; c < kl.ncomp; ++c)
