@@ -107,7 +107,7 @@ template <int COLS, class Launcher>
 int enqueue_tiled_2d(Launcher& run, const PlanView& p, const float* M, float* H) {
     const int nx = p.nx, ny = p.ny, Py = 2 * ny;
     const int ntl = (nx + 1 + COLS - 1) / COLS;
-    XTArgs xa{M, H, p.V, p.ptw_x, p.tw_xpost, ny, ntl, p.cfg.rbt};
+    XTArgs xa{M, H, p.V, p.ptw_x, p.tw_xpost, ny, ntl, p.cfg.rbt, ilog2c(p.cfg.rbt)};
     const Grid gx{(unsigned)(3L * ny / p.cfg.rbt), 1};
     int rc = dispatch_len(nx, [&](auto ic) { return run.template run<XFwdT<decltype(ic)::value, COLS>>(gx, xa); });
     if (rc) return rc;

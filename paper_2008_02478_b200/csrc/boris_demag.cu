@@ -10,6 +10,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <type_traits>
 #include <vector>
 
 #include "../../include/boris_demag.h"
@@ -47,8 +48,13 @@ __device__ __forceinline__ void run_phases(const typename K::Args& a, float2* sm
     }
 }
 
+template <class K, class = void>
+struct MinBlocks { static constexpr int value = 1; };
 template <class K>
-__global__ void __launch_bounds__(K::NT) phase_kernel(const __grid_constant__ typename K::Args a) {
+struct MinBlocks<K, std::void_t<decltype(K::MINB)>> { static constexpr int value = K::MINB; };
+
+template <class K>
+__global__ void __launch_bounds__(K::NT, MinBlocks<K>::value) phase_kernel(const __grid_constant__ typename K::Args a) {
     extern __shared__ __align__(16) float2 bd_smem[];
     run_phases<K, 0>(a, bd_smem);
 }

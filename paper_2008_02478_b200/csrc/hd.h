@@ -26,3 +26,12 @@
 #include <vector_types.h>   // float2, float4, double2 (plain structs on the host)
 
 BD_HD float2 bd_f2(float x, float y) { float2 r; r.x = x; r.y = y; return r; }
+
+// hint: bring the 128-byte line at p into L2 (no-op in the host emulation)
+BD_HD void bd_prefetch_l2(const void* p) {
+#if defined(__CUDA_ARCH__)
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+#else
+    (void)p;
+#endif
+}

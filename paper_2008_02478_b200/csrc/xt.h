@@ -19,19 +19,23 @@
 namespace bd {
 
 template <int L>
-struct SRows {                 // shared rows of L points at pitch L + 1, swizzled like a 1-column tile
+struct SRows {                 // shared rows of L points, padded like the tiles (yfused.h), pitch odd
     float2* p;
-    static constexpr int PITCH = L + 1;
-    BD_HD float2 get(int row, int e) const { return p[row * PITCH + swz<L, 1>(e)]; }
-    BD_HD void put(int row, int e, float2 v) const { p[row * PITCH + swz<L, 1>(e)] = v; }
+    static constexpr int PITCH = padlen8(L) | 1;
+    static BD_HD constexpr int step(int S) { return pstep(S); }
+    BD_HD float2* ptr(int row, int e) const { return p + row * PITCH + pidx(e); }
+    static BD_HD float2 ld(const float2* q) { return *q; }
 };
 struct GRowsIn {               // rows of a real array read as (x[2m], x[2m+1]) pairs
     const float* p; long pitch;
-    BD_HD float2 get(int row, int e) const { return BD_LDG(reinterpret_cast<const float2*>(p + row * pitch) + e); }
+    static BD_HD constexpr int step(int S) { return S; }
+    BD_HD const float2* ptr(int row, int e) const { return reinterpret_cast<const float2*>(p + row * pitch) + e; }
+    static BD_HD float2 ld(const float2* q) { return BD_LDG(q); }
 };
 struct GRowsOut {
     float* p; long pitch;
-    BD_HD void put(int row, int e, float2 v) const { reinterpret_cast<float2*>(p + row * pitch)[e] = v; }
+    static BD_HD constexpr int step(int S) { return S; }
+    BD_HD float2* ptr(int row, int e) const { return reinterpret_cast<float2*>(p + row * pitch) + e; }
 };
 
 struct XTArgs {
@@ -42,7 +46,8 @@ struct XTArgs {
     const float2* twx;     // exp(-2 pi i k / Px), k <= LX/2
     int ny;
     int ntl;
-    int rb;                // rows (consecutive y of one component) per block; divides ny
+    int rb;                // rows (consecutive y of one component) per block; a power of two dividing ny
+    int rbs;               // log2(rb)
 };
 
 // all rows of a block through pass P; a thread keeps its butterfly index (and twiddles)
@@ -69,6 +74,7 @@ struct XFwdT {
     using Args = XTArgs;
     static constexpr int KIND = kKindXFwdT;
     static constexpr int NT = 256;
+    static constexpr int MINB = 3;
     static constexpr int NP = dec_np(LX);
     static constexpr int NPHASES = NP + 1;
     static BD_HD long smem_elems(const Args& a) { return (long)a.rb * SRows<LX>::PITCH; }
@@ -86,18 +92,34 @@ struct XFwdT {
             const int c = (int)(g0 / a.ny), y0 = (int)(g0 - (long)c * a.ny);
             const int items = (LX / 2 + 1) * a.rb;
             float2* vc = a.V + (long)c * a.ntl * a.ny * COLS;
-            for (int w = tid; w < items; w += NT) {
-                const int kp = w / a.rb, row = w - kp * a.rb;
-                const int km = LX - kp;
-                const float2 Zk = s.get(row, pos_of_freq(LX, kp));
-                const float2 Zm = s.get(row, pos_of_freq(LX, km & (LX - 1)));
-                const float2 A = bd_f2(Zk.x + Zm.x, Zk.y - Zm.y);
-                const float2 B = bd_f2(Zk.x - Zm.x, Zk.y + Zm.y);
-                const float2 T = pk_cmul(bd_f2(B.y, -B.x), make_tw(BD_LDG(&a.twx[kp])));
-                const float2 Xk = pk_add(A, T), Xm = bd_f2(A.x - T.x, T.y - A.y);
-                const int y = y0 + row;
-                vc[((long)(kp / COLS) * a.ny + y) * COLS + kp % COLS] = Xk;
-                if (2 * kp != LX) vc[((long)(km / COLS) * a.ny + y) * COLS + km % COLS] = Xm;
+            // four independent items per trip: loads first, then arithmetic and stores
+            for (int w0 = tid; w0 < items; w0 += 4 * NT) {
+                float2 Zk[4], Zm[4], tw[4];
+                BD_UNROLL
+                for (int u = 0; u < 4; ++u) {
+                    const int w = w0 + u * NT;
+                    if (w < items) {
+                        const int kp = w >> a.rbs, row = w & (a.rb - 1);
+                        Zk[u] = *s.ptr(row, pos_of_freq(LX, kp));
+                        Zm[u] = *s.ptr(row, pos_of_freq(LX, (LX - kp) & (LX - 1)));
+                        tw[u] = BD_LDG(&a.twx[kp]);
+                    }
+                }
+                BD_UNROLL
+                for (int u = 0; u < 4; ++u) {
+                    const int w = w0 + u * NT;
+                    if (w < items) {
+                        const int kp = w >> a.rbs, row = w & (a.rb - 1);
+                        const int km = LX - kp;
+                        const float2 A = bd_f2(Zk[u].x + Zm[u].x, Zk[u].y - Zm[u].y);
+                        const float2 B = bd_f2(Zk[u].x - Zm[u].x, Zk[u].y + Zm[u].y);
+                        const float2 T = pk_cmul(bd_f2(B.y, -B.x), make_tw(tw[u]));
+                        const float2 Xk = pk_add(A, T), Xm = bd_f2(A.x - T.x, T.y - A.y);
+                        const int y = y0 + row;
+                        vc[((long)(kp / COLS) * a.ny + y) * COLS + kp % COLS] = Xk;
+                        if (2 * kp != LX) vc[((long)(km / COLS) * a.ny + y) * COLS + km % COLS] = Xm;
+                    }
+                }
             }
         }
     }
@@ -108,6 +130,7 @@ struct XInvT {
     using Args = XTArgs;
     static constexpr int KIND = kKindXInvT;
     static constexpr int NT = 256;
+    static constexpr int MINB = 3;
     static constexpr int NP = dec_np(LX);
     static constexpr int NPHASES = NP + 1;
     static BD_HD long smem_elems(const Args& a) { return (long)a.rb * SRows<LX>::PITCH; }
@@ -120,17 +143,33 @@ struct XInvT {
             const int c = (int)(g0 / a.ny), y0 = (int)(g0 - (long)c * a.ny);
             const int items = (LX / 2 + 1) * a.rb;
             const float2* vc = a.V + (long)c * a.ntl * a.ny * COLS;
-            for (int w = tid; w < items; w += NT) {
-                const int kp = w / a.rb, row = w - kp * a.rb;
-                const int km = LX - kp, y = y0 + row;
-                float2 Yk = vc[((long)(kp / COLS) * a.ny + y) * COLS + kp % COLS];
-                float2 Ym = vc[((long)(km / COLS) * a.ny + y) * COLS + km % COLS];
-                if (kp == 0) { Yk.y = 0.f; Ym.y = 0.f; }          // DC and Nyquist of a real row are real
-                const float2 E = bd_f2(Yk.x + Ym.x, Yk.y - Ym.y);
-                const float2 D = bd_f2(Yk.x - Ym.x, Yk.y + Ym.y);
-                const float2 O = pk_cmulc(D, make_tw(BD_LDG(&a.twx[kp])));
-                s.put(row, pos_of_freq(LX, kp), bd_f2(E.x - O.y, E.y + O.x));
-                if (kp != 0 && 2 * kp != LX) s.put(row, pos_of_freq(LX, km), bd_f2(E.x + O.y, O.x - E.y));
+            for (int w0 = tid; w0 < items; w0 += 4 * NT) {
+                float2 Yk[4], Ym[4], tw[4];
+                BD_UNROLL
+                for (int u = 0; u < 4; ++u) {
+                    const int w = w0 + u * NT;
+                    if (w < items) {
+                        const int kp = w >> a.rbs, row = w & (a.rb - 1);
+                        const int km = LX - kp, y = y0 + row;
+                        Yk[u] = vc[((long)(kp / COLS) * a.ny + y) * COLS + kp % COLS];
+                        Ym[u] = vc[((long)(km / COLS) * a.ny + y) * COLS + km % COLS];
+                        tw[u] = BD_LDG(&a.twx[kp]);
+                    }
+                }
+                BD_UNROLL
+                for (int u = 0; u < 4; ++u) {
+                    const int w = w0 + u * NT;
+                    if (w < items) {
+                        const int kp = w >> a.rbs, row = w & (a.rb - 1);
+                        const int km = LX - kp;
+                        if (kp == 0) { Yk[u].y = 0.f; Ym[u].y = 0.f; }    // DC and Nyquist of a real row are real
+                        const float2 E = bd_f2(Yk[u].x + Ym[u].x, Yk[u].y - Ym[u].y);
+                        const float2 D = bd_f2(Yk[u].x - Ym[u].x, Yk[u].y + Ym[u].y);
+                        const float2 O = pk_cmulc(D, make_tw(tw[u]));
+                        *s.ptr(row, pos_of_freq(LX, kp)) = bd_f2(E.x - O.y, E.y + O.x);
+                        if (kp != 0 && 2 * kp != LX) *s.ptr(row, pos_of_freq(LX, km)) = bd_f2(E.x + O.y, O.x - E.y);
+                    }
+                }
             }
         } else if constexpr (PH < NP) {
             x_rows_pass<LX, NP - PH, true, NT>(tid, a.rb, s, s, a.ptw);

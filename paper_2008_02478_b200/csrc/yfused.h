@@ -54,39 +54,37 @@ inline void fill_pass_twiddles(float2* h, int L) {
     }
 }
 
-// ------------------------------------------------------------------ shared-memory order
+// ------------------------------------------------------------------ accessors
+// Shared pencils are padded by one element per 8: physical index p(e) = e + (e >> 3).
+// Every pass reads e = base + r S with S = 1 (base a multiple of 8) or S >= 8 (a power
+// of two, r S bit-disjoint from base), so p(base + r S) = p(base) + r * pstep(S):
+// addresses are one base plus compile-time offsets.  Half warps touch 16/COLS
+// consecutive base indices, or items 8 apart in the last pass (stride 9): no bank
+// conflicts beyond one 2-way overlap per 16 consecutive elements.
 BD_HD constexpr int ilog2c(int v) { return v <= 1 ? 0 : 1 + ilog2c(v >> 1); }
-// XOR swizzle of the pencil index: a half warp touches 16/COLS different e per access;
-// they must differ in their low bits.  Plain passes give consecutive e; the last pass
-// gives e = 8 i + q with consecutive i; the multiply gives i = (f % R0) R1 + f / R0
-// with consecutive f.
-template <int L, int COLS>
-BD_HD int swz(int e) {
-    constexpr int SW = 16 / COLS;
-    if constexpr (dec_np(L) == 1 || SW <= 1) {
-        return e;
-    } else if constexpr (dec_np(L) == 2) {
-        return e ^ ((e >> 3) & (SW - 1));
-    } else {
-        constexpr int SH = 3 + ilog2c(dec_r(L, 1));
-        return e ^ (((e >> 3) ^ (e >> SH)) & (SW - 1));
-    }
-}
+BD_HD constexpr int padlen8(int L) { return L + (L >> 3); }
+BD_HD int pidx(int e) { return e + (e >> 3); }
+BD_HD constexpr int pstep(int S) { return S >= 8 ? S + (S >> 3) : S; }
 
+// An accessor gives ptr(c, e) -> address of element e of pencil c, STEP(S) -> distance
+// (in elements of the pointer) between e and e + S, and ld() to read.
 template <int L, int COLS>
-struct STile {                 // shared: S[c][swz(e)][col]
+struct STile {                 // shared: S[c][p(e)][col]
     float2* p;                 // already offset by col
-    BD_HD float2 get(int c, int e) const { return p[(c * L + swz<L, COLS>(e)) * COLS]; }
-    BD_HD void put(int c, int e, float2 v) const { p[(c * L + swz<L, COLS>(e)) * COLS] = v; }
+    static constexpr int CP = padlen8(L) * COLS;
+    static BD_HD constexpr int step(int S) { return pstep(S) * COLS; }
+    BD_HD float2* ptr(int c, int e) const { return p + c * CP + pidx(e) * COLS; }
+    static BD_HD float2 ld(const float2* q) { return *q; }
 };
 template <int COLS>
 struct GTile {                 // global: V tile [y][col], component stride cstride
     float2* p; long cstride;   // already offset by col
-    BD_HD float2 get(int c, int e) const { return p[c * cstride + (long)e * COLS]; }
-    BD_HD void put(int c, int e, float2 v) const { p[c * cstride + (long)e * COLS] = v; }
+    static BD_HD constexpr int step(int S) { return S * COLS; }
+    BD_HD float2* ptr(int c, int e) const { return p + c * cstride + (long)e * COLS; }
+    static BD_HD float2 ld(const float2* q) { return *q; }
 };
 
-// ------------------------------------------------------------------ passes, 3 components per thread
+// ------------------------------------------------------------------ passes
 // pencils c = c0, c0 + cstep, ... < cend share the butterfly index `it` and its twiddles
 template <int L, int P, class In, class Out>
 BD_HD void fwd_passM(int it, int c0, int cstep, int cend, const In& in, const Out& out, const float2* __restrict__ ptw) {
@@ -97,23 +95,32 @@ BD_HD void fwd_passM(int it, int c0, int cstep, int cend, const In& in, const Ou
         BD_UNROLL
         for (int q = 1; q < R; ++q) tw[q] = make_tw(BD_LDG(&ptw[ptw_off(L, P) + (q - 1) * S + j]));
     }
+    // the inputs of the next pencil are loaded before the current one is transformed
+    constexpr int NIN = P == 0 ? R / 2 : R;
+    float2 nxt[NIN];
+    {
+        const auto* pi = in.ptr(c0, base);
+        BD_UNROLL
+        for (int r = 0; r < NIN; ++r) nxt[r] = In::ld(pi + r * In::step(S));
+    }
     for (int c = c0; c < cend; c += cstep) {
         float2 v[R];
-        if constexpr (P == 0) {
+        BD_UNROLL
+        for (int r = 0; r < NIN; ++r) v[r] = nxt[r];
+        if (c + cstep < cend) {
+            const auto* pi = in.ptr(c + cstep, base);
             BD_UNROLL
-            for (int r = 0; r < R / 2; ++r) v[r] = in.get(c, base + r * S);
-            PkDftPruned<R, -1>::run(v);
-        } else {
-            BD_UNROLL
-            for (int r = 0; r < R; ++r) v[r] = in.get(c, base + r * S);
-            PkDft<R, -1>::run(v);
+            for (int r = 0; r < NIN; ++r) nxt[r] = In::ld(pi + r * In::step(S));
         }
+        if constexpr (P == 0) PkDftPruned<R, -1>::run(v);
+        else PkDft<R, -1>::run(v);
         if constexpr (P < NP - 1) {
             BD_UNROLL
             for (int q = 1; q < R; ++q) v[q] = pk_cmul(v[q], tw[q]);
         }
+        float2* po = out.ptr(c, base);
         BD_UNROLL
-        for (int q = 0; q < R; ++q) out.put(c, base + q * S, v[q]);
+        for (int q = 0; q < R; ++q) po[q * Out::step(S)] = v[q];
     }
 }
 
@@ -126,22 +133,34 @@ BD_HD void inv_passM(int it, int c0, int cstep, int cend, const In& in, const Ou
         BD_UNROLL
         for (int q = 1; q < R; ++q) tw[q] = make_tw(BD_LDG(&ptw[ptw_off(L, P) + (q - 1) * S + j]));
     }
+    float2 nxt[R];
+    {
+        const auto* pi = in.ptr(c0, base);
+        BD_UNROLL
+        for (int q = 0; q < R; ++q) nxt[q] = In::ld(pi + q * In::step(S));
+    }
     for (int c = c0; c < cend; c += cstep) {
         float2 v[R];
         BD_UNROLL
-        for (int q = 0; q < R; ++q) v[q] = in.get(c, base + q * S);
+        for (int q = 0; q < R; ++q) v[q] = nxt[q];
+        if (c + cstep < cend) {
+            const auto* pi = in.ptr(c + cstep, base);
+            BD_UNROLL
+            for (int q = 0; q < R; ++q) nxt[q] = In::ld(pi + q * In::step(S));
+        }
         if constexpr (P < NP - 1) {
             BD_UNROLL
             for (int q = 1; q < R; ++q) v[q] = pk_cmulc(v[q], tw[q]);
         }
+        float2* po = out.ptr(c, base);
         if constexpr (P == 0) {
             PkDftTrunc<R, +1>::run(v);
             BD_UNROLL
-            for (int r = 0; r < R / 2; ++r) out.put(c, base + r * S, v[r]);
+            for (int r = 0; r < R / 2; ++r) po[r * Out::step(S)] = v[r];
         } else {
             PkDft<R, +1>::run(v);
             BD_UNROLL
-            for (int r = 0; r < R; ++r) out.put(c, base + r * S, v[r]);
+            for (int r = 0; r < R; ++r) po[r * Out::step(S)] = v[r];
         }
     }
 }
@@ -172,19 +191,6 @@ struct KTile {
 template <int L, int NC, bool REV, class In, class Out>
 BD_HD void mid3(int i, const float* __restrict__ krow, float sz, const In& in, const Out& out) {
     constexpr int NP = dec_np(L), RL = dec_rlast(L);
-    float2 v[3][RL];
-    BD_UNROLL
-    for (int c = 0; c < 3; ++c) {
-        if constexpr (NP == 1) {
-            BD_UNROLL
-            for (int q = 0; q < RL / 2; ++q) v[c][q] = in.get(c, i * RL + q);
-            PkDftPruned<RL, -1>::run(v[c]);
-        } else {
-            BD_UNROLL
-            for (int q = 0; q < RL; ++q) v[c][q] = in.get(c, i * RL + q);
-            PkDft<RL, -1>::run(v[c]);
-        }
-    }
     float k[NC][RL];
     BD_UNROLL
     for (int c = 0; c < NC; ++c) {
@@ -197,6 +203,19 @@ BD_HD void mid3(int i, const float* __restrict__ krow, float sz, const In& in, c
         } else {
             BD_UNROLL
             for (int q = 0; q < RL; ++q) k[c][q] = BD_LDG(krow + c * RL + q);
+        }
+    }
+    float2 v[3][RL];
+    BD_UNROLL
+    for (int c = 0; c < 3; ++c) {
+        if constexpr (NP == 1) {
+            BD_UNROLL
+            for (int q = 0; q < RL / 2; ++q) v[c][q] = In::ld(in.ptr(c, i * RL) + q * In::step(1));
+            PkDftPruned<RL, -1>::run(v[c]);
+        } else {
+            BD_UNROLL
+            for (int q = 0; q < RL; ++q) v[c][q] = In::ld(in.ptr(c, i * RL) + q * In::step(1));
+            PkDft<RL, -1>::run(v[c]);
         }
     }
     // odd-component signs moved onto the data: with my' = sy my, mz' = sz mz the products
@@ -230,11 +249,11 @@ BD_HD void mid3(int i, const float* __restrict__ krow, float sz, const In& in, c
         if constexpr (NP == 1) {
             PkDftTrunc<RL, +1>::run(v[c]);
             BD_UNROLL
-            for (int q = 0; q < RL / 2; ++q) out.put(c, i * RL + q, v[c][q]);
+            for (int q = 0; q < RL / 2; ++q) out.ptr(c, i * RL)[q * Out::step(1)] = v[c][q];
         } else {
             PkDft<RL, +1>::run(v[c]);
             BD_UNROLL
-            for (int q = 0; q < RL; ++q) out.put(c, i * RL + q, v[c][q]);
+            for (int q = 0; q < RL; ++q) out.ptr(c, i * RL)[q * Out::step(1)] = v[c][q];
         }
     }
 }
@@ -270,11 +289,12 @@ struct YFused {
     using Args = YFArgs;
     static constexpr int KIND = kKindYFused;
     static constexpr int NT = 256;
+    static constexpr int MINB = 2;
     static constexpr int NP = dec_np(L);
     static constexpr int NPHASES = 2 * NP - 1;
     static constexpr int RL = dec_rlast(L), F = L / RL, NR = F / 2 + 1;
     static constexpr int NY = L / 2;
-    static BD_HD long smem_elems(const Args&) { return NP == 1 ? 0 : 3L * L * COLS; }
+    static BD_HD long smem_elems(const Args&) { return NP == 1 ? 0 : 3L * padlen8(L) * COLS; }
 
     struct Blk { int tile, kz, kzr; float sz; };
     static BD_HD Blk decode(int bx, const Args& a) {
@@ -296,6 +316,12 @@ struct YFused {
     static BD_HD void pass(int tid, int bx, const Args& a, float2* sm) {
         constexpr int ITEMS = (L / dec_r(L, P)) * COLS;
         const Blk b = decode(bx, a);
+        if constexpr (P == 0 && !INV) {
+            // start the block's kernel-spectrum tile on its way to L2 while the pencils are transformed
+            constexpr long KB = (long)NR * COLS * NC * RL * sizeof(float);
+            const char* kt = reinterpret_cast<const char*>(a.K) + ((long)b.kzr * a.ntl + b.tile) * KB;
+            for (long o = (long)tid * 128; o < KB; o += NT * 128) bd_prefetch_l2(kt + o);
+        }
         for (int w = tid; w < ITEMS; w += NT) {
             const int col = w % COLS, it = w / COLS;
             STile<L, COLS> s{sm + col};
@@ -314,16 +340,20 @@ struct YFused {
         const float* kt = a.K + ((long)b.kzr * a.ntl + b.tile) * ((long)NR * COLS * NC * RL);
         for (int w = tid; w < ITEMS; w += NT) {
             const int col = w % COLS, u = w / COLS;
-            // units u < F/2: items f = u as stored; u >= F/2: f = F/2 (u = F/2, its own
-            // mirror) then the mirrored items f = F - (u - F/2)
-            int f = u, row = u;
-            bool rev = false;
-            if (F >= 2 && u >= F / 2) {
-                const int up = u - F / 2;
-                if (up == 0) { f = F / 2; row = F / 2; }
-                else { f = F - up; row = up; rev = true; }
+            // thread order of the multiply: first the items whose frequencies are stored as
+            // they are, then their mirrors, so that a warp takes one branch; inside each
+            // half the item index i = a + R1 b runs over a first (shared-memory stride 9)
+            int i, f;
+            if constexpr (NP <= 2) {
+                i = u; f = u;
+            } else {
+                constexpr int R0 = dec_r(L, 0), R1 = dec_r(L, 1), HA = R1 / 2;
+                const int h = u / (F / 2), t = u - h * (F / 2);
+                const int av = t % HA + h * HA, bv = t / HA;
+                i = av + R1 * bv; f = bv + R0 * av;
             }
-            const int i = item_of_partial_freq(L, f);
+            const bool rev = 2 * f > F;
+            const int row = rev ? F - f : f;
             const float* krow = kt + ((long)row * COLS + col) * (NC * RL);
             if constexpr (NP == 1) {
                 GTile<COLS> g = gtile(b, col, a);
