@@ -74,6 +74,7 @@ struct PlanView {
     float2 *W, *T;
     const float2 *ptw_x = nullptr, *ptw_y = nullptr;   // per-pass twiddles (tiled path)
     float2* V = nullptr;                               // tiled spectrum (tiled path)
+    const float4* xpost = nullptr;                     // fill_xpost table (tiled path)
 };
 
 template <int L> struct IC { static constexpr int value = L; };
@@ -107,7 +108,7 @@ template <int COLS, class Launcher>
 int enqueue_tiled_2d(Launcher& run, const PlanView& p, const float* M, float* H) {
     const int nx = p.nx, ny = p.ny, Py = 2 * ny;
     const int ntl = (nx + 1 + COLS - 1) / COLS;
-    XTArgs xa{M, H, p.V, p.ptw_x, p.tw_xpost, ny, ntl, p.cfg.rbt, ilog2c(p.cfg.rbt)};
+    XTArgs xa{M, H, p.V, p.ptw_x, p.xpost, ny, ntl, p.cfg.rbt, ilog2c(p.cfg.rbt)};
     const Grid gx{(unsigned)(3L * ny / p.cfg.rbt), 1};
     int rc = dispatch_len(nx, [&](auto ic) { return run.template run<XFwdT<decltype(ic)::value, COLS>>(gx, xa); });
     if (rc) return rc;

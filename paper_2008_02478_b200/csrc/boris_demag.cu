@@ -212,6 +212,7 @@ struct boris_demag_plan {
     float2* V = nullptr;             // tiled path: [3][Pz][ntl][ny][cols]
     float2* ptw_x = nullptr;         // tiled path: per-pass twiddles of the x / y transforms
     float2* ptw_y = nullptr;
+    float4* xpost = nullptr;         // tiled path: fill_xpost table
     double* partial = nullptr;       // energy partial sums
     float* stage_M = nullptr;        // apply_host staging
     float* stage_H = nullptr;
@@ -249,7 +250,7 @@ int upload_pass_twiddles(boris_demag_plan* p, float2** dst, int L) {
 
 bd::PlanView plan_view(const boris_demag_plan* p) {
     bd::PlanView pv{p->nx, p->ny, p->nz, p->cfg, p->Kst, p->tw_x, p->tw_xpost, p->tw_y, p->tw_z, p->W, p->T};
-    pv.ptw_x = p->ptw_x; pv.ptw_y = p->ptw_y; pv.V = p->V;
+    pv.ptw_x = p->ptw_x; pv.ptw_y = p->ptw_y; pv.V = p->V; pv.xpost = p->xpost;
     return pv;
 }
 
@@ -339,7 +340,7 @@ void boris_demag_plan_destroy(boris_demag_plan* p) {
     if (!p) return;
     cudaFree(p->Kst); cudaFree(p->tw_x); cudaFree(p->tw_xpost); cudaFree(p->tw_y); cudaFree(p->tw_z);
     cudaFree(p->W); cudaFree(p->T); cudaFree(p->partial);
-    cudaFree(p->V); cudaFree(p->ptw_x); cudaFree(p->ptw_y);
+    cudaFree(p->V); cudaFree(p->ptw_x); cudaFree(p->ptw_y); cudaFree(p->xpost);
     cudaFree(p->stage_M); cudaFree(p->stage_H); cudaFree(p->stage_E);
     delete p;
 }
@@ -370,6 +371,13 @@ boris_demag_plan* boris_demag_plan_create(int nx, int ny, int nz, double hx, dou
         if (!rc && cudaMemset(p->V, 0, nv * sizeof(float2)) != cudaSuccess) rc = fail(-2, "cudaMemset");
         if (!rc) rc = upload_pass_twiddles(p, &p->ptw_x, nx);
         if (!rc) rc = upload_pass_twiddles(p, &p->ptw_y, Py);
+        if (!rc) {
+            std::vector<float4> h((size_t)nx / 2 + 1);
+            bd::fill_xpost(h.data(), nx);
+            rc = dev_alloc(p, &p->xpost, h.size());
+            if (!rc && cudaMemcpy(p->xpost, h.data(), h.size() * sizeof(float4), cudaMemcpyHostToDevice) != cudaSuccess)
+                rc = fail(-2, "cudaMemcpy xpost");
+        }
     } else {
         if (!rc) rc = dev_alloc(p, &p->W, (size_t)3 * kl.nxr() * nz * ny);
         if (!rc && nz > 1) rc = dev_alloc(p, &p->T, (size_t)3 * p->cfg.cs * nz * Py);

@@ -16,6 +16,7 @@
 #pragma once
 #include "fft_core.h"
 #include "plan_math.h"
+#include "yfused.h"
 
 namespace bd {
 
@@ -74,23 +75,17 @@ BD_HD int fold_freq(int L, int k, bool odd, double& sign) {
 BD_HD double storage_value(const KLayout& kl, long idx, const double* Kred) {
     double sign = 1.0;
     if (kl.tiled) {
-        const int q = (int)(idx % kl.RLy); idx /= kl.RLy;
-        const int c = (int)(idx % kl.ncomp); idx /= kl.ncomp;
+        const int CH = k_chunk(kl.Py), NCH = kl.RLy / CH;
+        const int qi = (int)(idx % CH); idx /= CH;
         const int col = (int)(idx % kl.cols); idx /= kl.cols;
-        const int row = (int)(idx % kl.NRy); idx /= kl.NRy;
+        const int slot = (int)(idx % kl.NRy); idx /= kl.NRy;
+        const int ch = (int)(idx % NCH); idx /= NCH;
+        const int c = (int)(idx % kl.ncomp); idx /= kl.ncomp;
         const int tile = (int)(idx % kl.ntl); const int kzr = (int)(idx / kl.ntl);
-        const int kx = tile * kl.cols + col;
+        const int kx = tile * kl.cols + col, q = ch * CH + qi;
         if (kx > kl.nx) return 0.0;                      // padding columns of the last tile
-        const int kyr = fold_freq(kl.Py, row + kl.Fy * q, comp_is_odd(c, 1), sign);
+        const int kyr = fold_freq(kl.Py, slot_to_f(kl.Py, slot) + kl.Fy * q, comp_is_odd(c, 1), sign);
         return sign * Kred[kl.reduced_index(c, kzr, kyr, kx)];
-    }
-    if (kl.nz == 1) {
-        const int row = (int)(idx % kl.nrows); idx /= kl.nrows;
-        const int q = (int)(idx % kl.RL); idx /= kl.RL;
-        const int c = (int)(idx % 4); const int slot = (int)(idx / 4);
-        const int k = khat_f_of_row(kl.Py, row) + dec_items(kl.Py) * q;
-        const int kyr = fold_freq(kl.Py, k, comp_is_odd(c, 1), sign);
-        return sign * Kred[kl.reduced_index(c, 0, kyr, slot)];
     }
     const int t = (int)(idx % kl.ty); idx /= kl.ty;
     const int row = (int)(idx % kl.nrows); idx /= kl.nrows;
@@ -113,7 +108,9 @@ BD_HD long storage_index_of(const KLayout& kl, int c, int kz, int ky, int kx, fl
             f = kl.Fy - f; q = kl.RLy - 1 - q;
             if (comp_is_odd(c, 1)) sign = -1.f;
         }
-        return (((((long)kz * kl.ntl + kx / kl.cols) * kl.NRy + f) * kl.cols + kx % kl.cols) * kl.ncomp + c) * kl.RLy + q;
+        const int CH = k_chunk(kl.Py), NCH = kl.RLy / CH;
+        return ((((((long)kz * kl.ntl + kx / kl.cols) * kl.ncomp + c) * NCH + q / CH) * kl.NRy + f_to_slot(kl.Py, f)) * kl.cols
+                + kx % kl.cols) * CH + q % CH;
     }
     const int L = kl.Lf, F = dec_items(L), kf = kl.nz == 1 ? ky : kz;
     int f = kf % F, q = kf / F;

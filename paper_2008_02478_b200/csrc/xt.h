@@ -14,6 +14,8 @@
 //   Z[LX-k] = conj(E') + i conj(O')
 // The factors 2 are folded into the kernel spectrum (reading R12).
 #pragma once
+#include <cstring>
+
 #include "yfused.h"
 
 namespace bd {
@@ -43,12 +45,34 @@ struct XTArgs {
     float* H;              // [3][ny][nx]            (XInvT)
     float2* V;             // [3][1][ntl][ny][COLS]
     const float2* ptw;     // per-pass twiddles of length LX
-    const float2* twx;     // exp(-2 pi i k / Px), k <= LX/2
+    const float4* xpost;   // per kp <= LX/2: (cos, sin) of exp(-2 pi i kp / Px) and, as int bits, the padded
+                           // shared positions of Z[kp] and Z[LX-kp] (fill_xpost)
     int ny;
     int ntl;
     int rb;                // rows (consecutive y of one component) per block; a power of two dividing ny
     int rbs;               // log2(rb)
 };
+
+BD_HD int bd_float_as_int(float f) {
+#if defined(__CUDA_ARCH__)
+    return __float_as_int(f);
+#else
+    int i; std::memcpy(&i, &f, sizeof i); return i;
+#endif
+}
+inline void fill_xpost(float4* h, int LX) {
+    const double pi = 3.14159265358979323846264338327950288;
+    for (int kp = 0; kp <= LX / 2; ++kp) {
+        const double a = -2.0 * pi * (double)kp / (double)(2 * LX);
+        float2 w = bd_f2((float)std::cos(a), (float)std::sin(a));
+        if (kp == 0) w = bd_f2(1.f, 0.f);
+        if (2 * kp == LX) w = bd_f2(0.f, -1.f);
+        const int pk = pidx(pos_of_freq(LX, kp)), pm = pidx(pos_of_freq(LX, (LX - kp) & (LX - 1)));
+        float fk, fm;
+        std::memcpy(&fk, &pk, sizeof fk); std::memcpy(&fm, &pm, sizeof fm);
+        h[kp].x = w.x; h[kp].y = w.y; h[kp].z = fk; h[kp].w = fm;
+    }
+}
 
 // all rows of a block through pass P; a thread keeps its butterfly index (and twiddles)
 // and walks over rows
@@ -100,9 +124,11 @@ struct XFwdT {
                     const int w = w0 + u * NT;
                     if (w < items) {
                         const int kp = w >> a.rbs, row = w & (a.rb - 1);
-                        Zk[u] = *s.ptr(row, pos_of_freq(LX, kp));
-                        Zm[u] = *s.ptr(row, pos_of_freq(LX, (LX - kp) & (LX - 1)));
-                        tw[u] = BD_LDG(&a.twx[kp]);
+                        const float4 xp = BD_LDG(&a.xpost[kp]);
+                        const float2* zr = sm + row * SRows<LX>::PITCH;
+                        Zk[u] = zr[bd_float_as_int(xp.z)];
+                        Zm[u] = zr[bd_float_as_int(xp.w)];
+                        tw[u] = bd_f2(xp.x, xp.y);
                     }
                 }
                 BD_UNROLL
@@ -116,8 +142,8 @@ struct XFwdT {
                         const float2 T = pk_cmul(bd_f2(B.y, -B.x), make_tw(tw[u]));
                         const float2 Xk = pk_add(A, T), Xm = bd_f2(A.x - T.x, T.y - A.y);
                         const int y = y0 + row;
-                        vc[((long)(kp / COLS) * a.ny + y) * COLS + kp % COLS] = Xk;
-                        if (2 * kp != LX) vc[((long)(km / COLS) * a.ny + y) * COLS + km % COLS] = Xm;
+                        vc[((kp / COLS) * a.ny + y) * COLS + kp % COLS] = Xk;
+                        if (2 * kp != LX) vc[((km / COLS) * a.ny + y) * COLS + km % COLS] = Xm;
                     }
                 }
             }
@@ -144,16 +170,17 @@ struct XInvT {
             const int items = (LX / 2 + 1) * a.rb;
             const float2* vc = a.V + (long)c * a.ntl * a.ny * COLS;
             for (int w0 = tid; w0 < items; w0 += 4 * NT) {
-                float2 Yk[4], Ym[4], tw[4];
+                float2 Yk[4], Ym[4];
+                float4 xp[4];
                 BD_UNROLL
                 for (int u = 0; u < 4; ++u) {
                     const int w = w0 + u * NT;
                     if (w < items) {
                         const int kp = w >> a.rbs, row = w & (a.rb - 1);
                         const int km = LX - kp, y = y0 + row;
-                        Yk[u] = vc[((long)(kp / COLS) * a.ny + y) * COLS + kp % COLS];
-                        Ym[u] = vc[((long)(km / COLS) * a.ny + y) * COLS + km % COLS];
-                        tw[u] = BD_LDG(&a.twx[kp]);
+                        Yk[u] = vc[((kp / COLS) * a.ny + y) * COLS + kp % COLS];
+                        Ym[u] = vc[((km / COLS) * a.ny + y) * COLS + km % COLS];
+                        xp[u] = BD_LDG(&a.xpost[kp]);
                     }
                 }
                 BD_UNROLL
@@ -165,9 +192,10 @@ struct XInvT {
                         if (kp == 0) { Yk[u].y = 0.f; Ym[u].y = 0.f; }    // DC and Nyquist of a real row are real
                         const float2 E = bd_f2(Yk[u].x + Ym[u].x, Yk[u].y - Ym[u].y);
                         const float2 D = bd_f2(Yk[u].x - Ym[u].x, Yk[u].y + Ym[u].y);
-                        const float2 O = pk_cmulc(D, make_tw(tw[u]));
-                        *s.ptr(row, pos_of_freq(LX, kp)) = bd_f2(E.x - O.y, E.y + O.x);
-                        if (kp != 0 && 2 * kp != LX) *s.ptr(row, pos_of_freq(LX, km)) = bd_f2(E.x + O.y, O.x - E.y);
+                        const float2 O = pk_cmulc(D, make_tw(bd_f2(xp[u].x, xp[u].y)));
+                        float2* zr = sm + row * SRows<LX>::PITCH;
+                        zr[bd_float_as_int(xp[u].z)] = bd_f2(E.x - O.y, E.y + O.x);
+                        if (kp != 0 && 2 * kp != LX) zr[bd_float_as_int(xp[u].w)] = bd_f2(E.x + O.y, O.x - E.y);
                     }
                 }
             }

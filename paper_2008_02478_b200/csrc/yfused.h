@@ -175,34 +175,49 @@ BD_HD void inv_pass3(int it, const In& in, const Out& out, const float2* __restr
 }
 
 // ------------------------------------------------------------------ kernel-spectrum tile
-// K[kzr (Pz/2+1)][tile][row (F/2+1)][col][c (NC)][q (RL)], fp32.  Row r, entry q holds the
-// natural spectrum at ky = r + F q folded to [0, L/2] with the sign of the components
-// odd in y applied (F = L / RL items of the last pass).  Item f <= F/2 reads row f
-// as stored; item f > F/2 reads row F - f with q reversed and the y-odd components
-// negated (its frequencies are the mirrors L - k of that row).  Rows 0 and F/2 are
-// their own mirrors.  A block at kz > Pz/2 reads the tile of Pz - kz and negates the
-// z-odd components.
-template <int L>
-struct KTile {
-    static constexpr int RL = dec_rlast(L), F = L / RL, NR = F / 2 + 1;
-};
+// K[kzr (Pz/2+1)][tile][c (NC)][chunk (RL/CH)][slot (F/2+1)][col][CH], fp32, CH = 4 floats
+// (one 16-byte load; CH = RL when RL < 4).  F = L / RL items of the last pass.  Slot s
+// stands for the item with frequency offset f = slot_to_f(s) <= F/2; its entry q holds
+// the natural spectrum at ky = f + F q folded to [0, L/2] with the sign of the components
+// odd in y applied.  Item f <= F/2 reads its slot as stored; item f > F/2 reads the slot
+// of F - f with q reversed and the y-odd components negated (its frequencies are the
+// mirrors L - k of that slot).  f = 0 and f = F/2 are their own mirrors.  Slots are
+// numbered in the thread order of the multiply, so a warp reads consecutive 16-byte
+// pieces.  A block at kz > Pz/2 reads the tile of Pz - kz and negates the z-odd components.
+BD_HD constexpr int k_chunk(int L) { return dec_rlast(L) % 4 == 0 ? 4 : dec_rlast(L); }
+BD_HD int slot_to_f(int L, int slot) {
+    const int RL = dec_rlast(L), F = L / RL;
+    if (dec_np(L) <= 2 || 2 * slot == F) return slot;
+    const int R0 = dec_r(L, 0), HA = dec_r(L, 1) / 2;
+    return slot / HA + R0 * (slot % HA);
+}
+BD_HD int f_to_slot(int L, int f) {       // f <= F/2
+    const int RL = dec_rlast(L), F = L / RL;
+    if (dec_np(L) <= 2 || 2 * f == F) return f;
+    const int R0 = dec_r(L, 0), HA = dec_r(L, 1) / 2;
+    return f / R0 + HA * (f % R0);
+}
 
 // last forward pass + multiply + first inverse pass of item i (frequency offset f)
 template <int L, int NC, bool REV, class In, class Out>
-BD_HD void mid3(int i, const float* __restrict__ krow, float sz, const In& in, const Out& out) {
+BD_HD void mid3(int i, const float* __restrict__ kslot, int cstride, float sz, const In& in, const Out& out) {
     constexpr int NP = dec_np(L), RL = dec_rlast(L);
+    // kslot points at chunk 0 of component 0 for this thread's (slot, col); consecutive
+    // chunks are cstride floats apart
+    constexpr int CH = k_chunk(L), NCH = RL / CH;
     float k[NC][RL];
     BD_UNROLL
     for (int c = 0; c < NC; ++c) {
-        if constexpr (RL % 4 == 0) {
-            BD_UNROLL
-            for (int q4 = 0; q4 < RL / 4; ++q4) {
-                const float4 t = BD_LDG(reinterpret_cast<const float4*>(krow + c * RL) + q4);
-                k[c][4 * q4] = t.x; k[c][4 * q4 + 1] = t.y; k[c][4 * q4 + 2] = t.z; k[c][4 * q4 + 3] = t.w;
+        BD_UNROLL
+        for (int ch = 0; ch < NCH; ++ch) {
+            const float* kp = kslot + (long)(c * NCH + ch) * cstride;
+            if constexpr (CH == 4) {
+                const float4 t = BD_LDG(reinterpret_cast<const float4*>(kp));
+                k[c][4 * ch] = t.x; k[c][4 * ch + 1] = t.y; k[c][4 * ch + 2] = t.z; k[c][4 * ch + 3] = t.w;
+            } else {
+                BD_UNROLL
+                for (int q = 0; q < CH; ++q) k[c][ch * CH + q] = BD_LDG(kp + q);
             }
-        } else {
-            BD_UNROLL
-            for (int q = 0; q < RL; ++q) k[c][q] = BD_LDG(krow + c * RL + q);
         }
     }
     float2 v[3][RL];
@@ -270,7 +285,7 @@ BD_HD int item_of_partial_freq(int L, int f) {
 // ------------------------------------------------------------------ YFused (S2+S4+S6)
 struct YFArgs {
     float2* V;            // [3][Pz][ntl][ny][COLS]
-    const float* K;       // [Pz/2+1][ntl][NR][COLS][NC][RL]
+    const float* K;       // [Pz/2+1][ntl][NC][RL/CH][F/2+1][COLS][CH]
     const float2* ptw;    // per-pass twiddles of length L
     int ntl;              // kx tiles
     int pz;               // padded z length (1 in 2-D mode)
@@ -354,14 +369,15 @@ struct YFused {
             }
             const bool rev = 2 * f > F;
             const int row = rev ? F - f : f;
-            const float* krow = kt + ((long)row * COLS + col) * (NC * RL);
+            constexpr int CH = k_chunk(L), KCS = NR * COLS * CH;
+            const float* krow = kt + ((long)f_to_slot(L, row) * COLS + col) * CH;
             if constexpr (NP == 1) {
                 GTile<COLS> g = gtile(b, col, a);
-                mid3<L, NC, false>(i, krow, b.sz, g, g);
+                mid3<L, NC, false>(i, krow, KCS, b.sz, g, g);
             } else {
                 STile<L, COLS> s{sm + col};
-                if (rev) mid3<L, NC, true>(i, krow, b.sz, s, s);
-                else mid3<L, NC, false>(i, krow, b.sz, s, s);
+                if (rev) mid3<L, NC, true>(i, krow, KCS, b.sz, s, s);
+                else mid3<L, NC, false>(i, krow, KCS, b.sz, s, s);
             }
         }
     }

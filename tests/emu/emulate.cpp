@@ -67,7 +67,9 @@ int emu_apply(int nx, int ny, int nz, const double* Kred, const float* M, float*
     fill_pass_twiddles(ptwx.data(), nx);
     fill_pass_twiddles(ptwy.data(), Py);
     std::vector<float2> V(cfg.tiled ? (size_t)3 * Pz * kl.ntl * ny * kl.cols : 1, bd_f2(0.f, 0.f));
-    pv.ptw_x = ptwx.data(); pv.ptw_y = ptwy.data(); pv.V = V.data();
+    std::vector<float4> xpost((size_t)nx / 2 + 1);
+    fill_xpost(xpost.data(), nx);
+    pv.ptw_x = ptwx.data(); pv.ptw_y = ptwy.data(); pv.V = V.data(); pv.xpost = xpost.data();
     HostLauncher run;
     const int rc = enqueue_apply(run, pv, M, H);
     if (rc) return rc;
