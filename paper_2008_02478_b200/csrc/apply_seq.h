@@ -8,6 +8,7 @@
 #include "kernels.h"
 #include "khat_layout.h"
 #include "xt.h"
+#include "xz.h"
 #include "yfused.h"
 
 namespace bd {
@@ -26,7 +27,13 @@ struct LaunchCfg {
 // kx columns per tile of the tiled path: 3 * L * cols complex = 96 KB of shared memory
 // per block at L >= 512 (two blocks per SM)
 BD_HD constexpr int cols_for(int Ly) { return Ly >= 2048 ? 2 : (Ly >= 1024 ? 4 : 8); }
-inline bool tiled_supported(int nx, int ny, int nz) { return nz == 1; }
+constexpr long kMaxDynSmem = 227L * 1024;
+// the 3-D tiled path keeps the nz rows of one (component, y) in shared memory and each
+// z column (2 nz points) in registers
+inline bool tiled_supported(int nx, int ny, int nz) {
+    if (nz == 1) return true;
+    return nz <= 32 && (long)nz * (padlen8(nx) | 1) * (long)sizeof(float2) <= kMaxDynSmem;
+}
 
 inline LaunchCfg make_launch_cfg(int nx, int ny, int nz) {
     LaunchCfg c;
@@ -123,6 +130,47 @@ int enqueue_tiled_2d(Launcher& run, const PlanView& p, const float* M, float* H)
     return dispatch_len(nx, [&](auto ic) { return run.template run<XInvT<decltype(ic)::value, COLS>>(gx, xa); });
 }
 
+// tiled path, nz = 2..32: XZFwd -> YFused -> ZXInv
+template <class Launcher>
+int enqueue_tiled_3d(Launcher& run, const PlanView& p, const float* M, float* H) {
+    const int nx = p.nx, ny = p.ny, nz = p.nz, Py = 2 * ny, Pz = 2 * nz, cols = p.cfg.cols;
+    const int ntl = (nx + 1 + cols - 1) / cols;
+    XZArgs xa{M, H, p.V, p.ptw_x, p.xpost, ny, ntl, ilog2c(cols)};
+    const Grid gx{(unsigned)(3 * ny), 1};
+    auto xz = [&](auto fwd) {
+        return dispatch_len(nx, [&](auto ic) {
+            constexpr int LX = decltype(ic)::value;
+            auto go = [&](auto nzc) {
+                constexpr int NZ = decltype(nzc)::value;
+                if constexpr ((long)NZ * (padlen8(LX) | 1) * (long)sizeof(float2) <= kMaxDynSmem && LX <= 1024) {
+                    if constexpr (decltype(fwd)::value) return run.template run<XZFwd<LX, NZ>>(gx, xa);
+                    else return run.template run<ZXInv<LX, NZ>>(gx, xa);
+                } else {
+                    return -1;
+                }
+            };
+            switch (nz) {
+                case 2: return go(IC<2>{});
+                case 4: return go(IC<4>{});
+                case 8: return go(IC<8>{});
+                case 16: return go(IC<16>{});
+                case 32: return go(IC<32>{});
+                default: return -1;
+            }
+        });
+    };
+    int rc = xz(IC<1>{});
+    if (rc) return rc;
+    YFArgs ya{p.V, p.Kst, p.ptw_y, ntl, Pz};
+    const Grid gy{(unsigned)(ntl * Pz), 1};
+    rc = dispatch_len(Py, [&](auto ic) {
+        constexpr int L = decltype(ic)::value;
+        return run.template run<YFused<L, 6, cols_for(L)>>(gy, ya);
+    });
+    if (rc) return rc;
+    return xz(IC<0>{});
+}
+
 // Launcher::run<K>(Grid, const K::Args&) -> 0 on success.
 template <class Launcher>
 int enqueue_apply(Launcher& run, const PlanView& p, const float* M, float* H) {
@@ -135,7 +183,7 @@ int enqueue_apply(Launcher& run, const PlanView& p, const float* M, float* H) {
                 default: return -1;
             }
         }
-        return -1;
+        return enqueue_tiled_3d(run, p, M, H);
     }
     const int nx = p.nx, ny = p.ny, nz = p.nz, NS = nx + 1, Py = 2 * ny, Pz = 2 * nz;
     const LaunchCfg& c = p.cfg;

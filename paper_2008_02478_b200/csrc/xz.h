@@ -1,0 +1,405 @@
+// xz.h — x and z transforms of the tiled 3-D path (nz = 2..32): S1+S3 and S5+S7 of
+// SURVEY.md §8(a) ("1D FFTs along the x, y, z directions"; zero padding L283).
+//
+//   XZFwd  one block per (component, y): the nz rows M[c][:][y][:] are transformed along
+//          x in shared memory (real rows as half-length complex rows, xt.h), then every
+//          kx column is transformed along z in registers (nz -> Pz = 2 nz, pruned) and
+//          written to the kx-tiled spectrum V[c][kz][tile][y][col] that YFused reads.
+//   ZXInv  the mirror: V -> inverse z (first nz outputs kept) -> inverse x -> H rows.
+//
+// The kx = 0 and kx = nx (Nyquist) columns of a real row are real; they travel through
+// the z transform as the one complex column P = X[0] + i X[nx] and are separated after it
+// (X0^[kz] = (P^[kz] + conj P^[Pz-kz]) / 2, XN^[kz] = (P^[kz] - conj P^[Pz-kz]) / 2i), so
+// a block has exactly nx columns of work.
+#pragma once
+#include "xt.h"
+
+namespace bd {
+
+BD_HD constexpr float cos64(int m) {
+    switch (m & 63) {
+        case 0: return 1.000000000e+00f;
+        case 1: return 9.951847267e-01f;
+        case 2: return 9.807852804e-01f;
+        case 3: return 9.569403357e-01f;
+        case 4: return 9.238795325e-01f;
+        case 5: return 8.819212643e-01f;
+        case 6: return 8.314696123e-01f;
+        case 7: return 7.730104534e-01f;
+        case 8: return 7.071067812e-01f;
+        case 9: return 6.343932842e-01f;
+        case 10: return 5.555702330e-01f;
+        case 11: return 4.713967368e-01f;
+        case 12: return 3.826834324e-01f;
+        case 13: return 2.902846773e-01f;
+        case 14: return 1.950903220e-01f;
+        case 15: return 9.801714033e-02f;
+        case 16: return 0.000000000e+00f;
+        case 17: return -9.801714033e-02f;
+        case 18: return -1.950903220e-01f;
+        case 19: return -2.902846773e-01f;
+        case 20: return -3.826834324e-01f;
+        case 21: return -4.713967368e-01f;
+        case 22: return -5.555702330e-01f;
+        case 23: return -6.343932842e-01f;
+        case 24: return -7.071067812e-01f;
+        case 25: return -7.730104534e-01f;
+        case 26: return -8.314696123e-01f;
+        case 27: return -8.819212643e-01f;
+        case 28: return -9.238795325e-01f;
+        case 29: return -9.569403357e-01f;
+        case 30: return -9.807852804e-01f;
+        case 31: return -9.951847267e-01f;
+        case 32: return -1.000000000e+00f;
+        case 33: return -9.951847267e-01f;
+        case 34: return -9.807852804e-01f;
+        case 35: return -9.569403357e-01f;
+        case 36: return -9.238795325e-01f;
+        case 37: return -8.819212643e-01f;
+        case 38: return -8.314696123e-01f;
+        case 39: return -7.730104534e-01f;
+        case 40: return -7.071067812e-01f;
+        case 41: return -6.343932842e-01f;
+        case 42: return -5.555702330e-01f;
+        case 43: return -4.713967368e-01f;
+        case 44: return -3.826834324e-01f;
+        case 45: return -2.902846773e-01f;
+        case 46: return -1.950903220e-01f;
+        case 47: return -9.801714033e-02f;
+        case 48: return 0.000000000e+00f;
+        case 49: return 9.801714033e-02f;
+        case 50: return 1.950903220e-01f;
+        case 51: return 2.902846773e-01f;
+        case 52: return 3.826834324e-01f;
+        case 53: return 4.713967368e-01f;
+        case 54: return 5.555702330e-01f;
+        case 55: return 6.343932842e-01f;
+        case 56: return 7.071067812e-01f;
+        case 57: return 7.730104534e-01f;
+        case 58: return 8.314696123e-01f;
+        case 59: return 8.819212643e-01f;
+        case 60: return 9.238795325e-01f;
+        case 61: return 9.569403357e-01f;
+        case 62: return 9.807852804e-01f;
+        case 63: return 9.951847267e-01f;
+        default: return 0.f;
+    }
+}
+BD_HD constexpr float sin64(int m) {
+    switch (m & 63) {
+        case 0: return 0.000000000e+00f;
+        case 1: return 9.801714033e-02f;
+        case 2: return 1.950903220e-01f;
+        case 3: return 2.902846773e-01f;
+        case 4: return 3.826834324e-01f;
+        case 5: return 4.713967368e-01f;
+        case 6: return 5.555702330e-01f;
+        case 7: return 6.343932842e-01f;
+        case 8: return 7.071067812e-01f;
+        case 9: return 7.730104534e-01f;
+        case 10: return 8.314696123e-01f;
+        case 11: return 8.819212643e-01f;
+        case 12: return 9.238795325e-01f;
+        case 13: return 9.569403357e-01f;
+        case 14: return 9.807852804e-01f;
+        case 15: return 9.951847267e-01f;
+        case 16: return 1.000000000e+00f;
+        case 17: return 9.951847267e-01f;
+        case 18: return 9.807852804e-01f;
+        case 19: return 9.569403357e-01f;
+        case 20: return 9.238795325e-01f;
+        case 21: return 8.819212643e-01f;
+        case 22: return 8.314696123e-01f;
+        case 23: return 7.730104534e-01f;
+        case 24: return 7.071067812e-01f;
+        case 25: return 6.343932842e-01f;
+        case 26: return 5.555702330e-01f;
+        case 27: return 4.713967368e-01f;
+        case 28: return 3.826834324e-01f;
+        case 29: return 2.902846773e-01f;
+        case 30: return 1.950903220e-01f;
+        case 31: return 9.801714033e-02f;
+        case 32: return 0.000000000e+00f;
+        case 33: return -9.801714033e-02f;
+        case 34: return -1.950903220e-01f;
+        case 35: return -2.902846773e-01f;
+        case 36: return -3.826834324e-01f;
+        case 37: return -4.713967368e-01f;
+        case 38: return -5.555702330e-01f;
+        case 39: return -6.343932842e-01f;
+        case 40: return -7.071067812e-01f;
+        case 41: return -7.730104534e-01f;
+        case 42: return -8.314696123e-01f;
+        case 43: return -8.819212643e-01f;
+        case 44: return -9.238795325e-01f;
+        case 45: return -9.569403357e-01f;
+        case 46: return -9.807852804e-01f;
+        case 47: return -9.951847267e-01f;
+        case 48: return -1.000000000e+00f;
+        case 49: return -9.951847267e-01f;
+        case 50: return -9.807852804e-01f;
+        case 51: return -9.569403357e-01f;
+        case 52: return -9.238795325e-01f;
+        case 53: return -8.819212643e-01f;
+        case 54: return -8.314696123e-01f;
+        case 55: return -7.730104534e-01f;
+        case 56: return -7.071067812e-01f;
+        case 57: return -6.343932842e-01f;
+        case 58: return -5.555702330e-01f;
+        case 59: return -4.713967368e-01f;
+        case 60: return -3.826834324e-01f;
+        case 61: return -2.902846773e-01f;
+        case 62: return -1.950903220e-01f;
+        case 63: return -9.801714033e-02f;
+        default: return 0.f;
+    }
+}
+
+// z * exp(DIR 2 pi i m / 64), m known after unrolling
+template <int DIR>
+BD_HD float2 pk_mul_w64(float2 z, int m) {
+    m &= 63;
+    if (m == 0) return z;
+    if (m == 32) return pk_neg(z);
+    if (m == 16) return pk_ib<DIR>(z);
+    if (m == 48) return pk_ib<-DIR>(z);
+    const float c = cos64(m), s = (float)DIR * sin64(m);
+    return pk_fma(pk_swap(z), bd_f2(-s, s), pk_mul(z, pk_bc(c)));
+}
+
+// Column transforms in registers.  fwd: v[0..PZ/2) -> v[0..PZ) (natural order, zero-padded
+// input); inv: v[0..PZ) -> v[0..PZ/2) (unnormalised, upper half dropped).
+template <int PZ>
+struct ZCol {
+    static BD_HD void fwd(float2* v) { PkDftPruned<PZ, -1>::run(v); }
+    static BD_HD void inv(float2* v) { PkDftTrunc<PZ, +1>::run(v); }
+};
+template <>
+struct ZCol<64> {
+    // kz = q0 + 8 q1, z = j + 8 r:  X[kz] = sum_j W8^(j q1) [ W64^(j q0) sum_r x[j + 8r] W8^(r q0) ]
+    static BD_HD void fwd(float2* v) {
+        float2 t[8][8];
+        BD_UNROLL
+        for (int j = 0; j < 8; ++j) {
+            float2 u[8];
+            BD_UNROLL
+            for (int r = 0; r < 4; ++r) u[r] = v[j + 8 * r];
+            PkDftPruned<8, -1>::run(u);
+            BD_UNROLL
+            for (int q0 = 0; q0 < 8; ++q0) t[j][q0] = pk_mul_w64<-1>(u[q0], j * q0);
+        }
+        BD_UNROLL
+        for (int q0 = 0; q0 < 8; ++q0) {
+            float2 a[8];
+            BD_UNROLL
+            for (int j = 0; j < 8; ++j) a[j] = t[j][q0];
+            PkDft<8, -1>::run(a);
+            BD_UNROLL
+            for (int q1 = 0; q1 < 8; ++q1) v[q0 + 8 * q1] = a[q1];
+        }
+    }
+    static BD_HD void inv(float2* v) {
+        float2 t[8][8];
+        BD_UNROLL
+        for (int q0 = 0; q0 < 8; ++q0) {
+            float2 a[8];
+            BD_UNROLL
+            for (int q1 = 0; q1 < 8; ++q1) a[q1] = v[q0 + 8 * q1];
+            PkDft<8, +1>::run(a);
+            BD_UNROLL
+            for (int j = 0; j < 8; ++j) t[j][q0] = pk_mul_w64<+1>(a[j], j * q0);
+        }
+        BD_UNROLL
+        for (int j = 0; j < 8; ++j) {
+            float2 u[8];
+            BD_UNROLL
+            for (int q0 = 0; q0 < 8; ++q0) u[q0] = t[j][q0];
+            PkDftTrunc<8, +1>::run(u);
+            BD_UNROLL
+            for (int r = 0; r < 4; ++r) v[j + 8 * r] = u[r];
+        }
+    }
+};
+
+struct XZArgs {
+    const float* M;        // [3][nz][ny][nx]
+    float* H;              // [3][nz][ny][nx]            (ZXInv)
+    float2* V;             // [3][Pz][ntl][ny][cols]
+    const float2* ptw;     // per-pass twiddles of length LX
+    const float4* xpost;   // fill_xpost table
+    int ny;
+    int ntl;
+    int cs;                // log2(cols)
+};
+
+// shared position of X[kx] (kx < LX) inside a row, from the xpost table
+BD_HD int xz_pos(const float4* __restrict__ xpost, int LX, int kx) {
+    return 2 * kx <= LX ? bd_float_as_int(BD_LDG(&xpost[kx]).z) : bd_float_as_int(BD_LDG(&xpost[LX - kx]).w);
+}
+
+template <int LX, int NZ>
+struct XZFwd {
+    using Args = XZArgs;
+    static constexpr int KIND = kKindXZFwd;
+    static constexpr int NT = 256;
+    static constexpr int MINB = 1;
+    static constexpr int NP = dec_np(LX);
+    static constexpr int NPHASES = NP + 2;
+    static constexpr int PZ = 2 * NZ;
+    static constexpr int PITCH = SRows<LX>::PITCH;
+    static BD_HD long smem_elems(const Args&) { return (long)NZ * PITCH; }
+
+    template <int PH>
+    static BD_HD void phase(int tid, int bx, int by, const Args& a, float2* sm) {
+        const int c = bx / a.ny, y = bx - c * a.ny;
+        SRows<LX> s{sm};
+        if constexpr (PH == 0) {
+            GRowsIn in{a.M + ((long)c * NZ * a.ny + y) * LX, (long)a.ny * LX};
+            x_rows_pass<LX, 0, false, NT>(tid, NZ, in, s, a.ptw);
+        } else if constexpr (PH < NP) {
+            x_rows_pass<LX, PH, false, NT>(tid, NZ, s, s, a.ptw);
+        } else if constexpr (PH == NP) {
+            // untangle in place: Z[kp], Z[LX-kp] -> X[kp], X[LX-kp]; kp = 0 -> P = (X[0], X[LX])
+            constexpr int items = (LX / 2 + 1) * NZ;
+            for (int w0 = tid; w0 < items; w0 += 4 * NT) {
+                float2 Zk[4], Zm[4];
+                float4 xp[4];
+                BD_UNROLL
+                for (int u = 0; u < 4; ++u) {
+                    const int w = w0 + u * NT;
+                    if (w < items) {
+                        const int kp = w / NZ, row = w % NZ;
+                        xp[u] = BD_LDG(&a.xpost[kp]);
+                        const float2* zr = sm + row * PITCH;
+                        Zk[u] = zr[bd_float_as_int(xp[u].z)];
+                        Zm[u] = zr[bd_float_as_int(xp[u].w)];
+                    }
+                }
+                BD_UNROLL
+                for (int u = 0; u < 4; ++u) {
+                    const int w = w0 + u * NT;
+                    if (w < items) {
+                        const int kp = w / NZ, row = w % NZ;
+                        const float2 A = bd_f2(Zk[u].x + Zm[u].x, Zk[u].y - Zm[u].y);
+                        const float2 B = bd_f2(Zk[u].x - Zm[u].x, Zk[u].y + Zm[u].y);
+                        const float2 T = pk_cmul(bd_f2(B.y, -B.x), make_tw(bd_f2(xp[u].x, xp[u].y)));
+                        const float2 Xk = pk_add(A, T), Xm = bd_f2(A.x - T.x, T.y - A.y);
+                        float2* zr = sm + row * PITCH;
+                        if (kp == 0) {
+                            zr[bd_float_as_int(xp[u].z)] = bd_f2(Xk.x, Xm.x);
+                        } else {
+                            zr[bd_float_as_int(xp[u].z)] = Xk;
+                            if (2 * kp != LX) zr[bd_float_as_int(xp[u].w)] = Xm;
+                        }
+                    }
+                }
+            }
+        } else {
+            const int cols = 1 << a.cs;
+            const long kzs = (long)a.ntl * a.ny * cols;                 // elements between kz planes
+            float2* vc = a.V + (long)c * PZ * kzs;
+            for (int kx = tid; kx < LX; kx += NT) {
+                const float2* col = sm + xz_pos(a.xpost, LX, kx);
+                float2 v[PZ];
+                BD_UNROLL
+                for (int z = 0; z < NZ; ++z) v[z] = col[z * PITCH];
+                ZCol<PZ>::fwd(v);
+                float2* out = vc + ((long)((kx >> a.cs) * a.ny + y) << a.cs) + (kx & (cols - 1));
+                if (kx != 0) {
+                    BD_UNROLL
+                    for (int kz = 0; kz < PZ; ++kz) out[kz * kzs] = v[kz];
+                } else {
+                    float2* outn = vc + ((long)((LX >> a.cs) * a.ny + y) << a.cs) + (LX & (cols - 1));
+                    BD_UNROLL
+                    for (int kz = 0; kz < PZ; ++kz) {
+                        const float2 p = v[kz], m = v[(PZ - kz) % PZ];
+                        out[kz * kzs] = bd_f2(0.5f * (p.x + m.x), 0.5f * (p.y - m.y));
+                        outn[kz * kzs] = bd_f2(0.5f * (p.y + m.y), 0.5f * (m.x - p.x));
+                    }
+                }
+            }
+        }
+    }
+};
+
+template <int LX, int NZ>
+struct ZXInv {
+    using Args = XZArgs;
+    static constexpr int KIND = kKindZXInv;
+    static constexpr int NT = 256;
+    static constexpr int MINB = 1;
+    static constexpr int NP = dec_np(LX);
+    static constexpr int NPHASES = NP + 2;
+    static constexpr int PZ = 2 * NZ;
+    static constexpr int PITCH = SRows<LX>::PITCH;
+    static BD_HD long smem_elems(const Args&) { return (long)NZ * PITCH; }
+
+    template <int PH>
+    static BD_HD void phase(int tid, int bx, int by, const Args& a, float2* sm) {
+        const int c = bx / a.ny, y = bx - c * a.ny;
+        SRows<LX> s{sm};
+        if constexpr (PH == 0) {
+            const int cols = 1 << a.cs;
+            const long kzs = (long)a.ntl * a.ny * cols;
+            const float2* vc = a.V + (long)c * PZ * kzs;
+            for (int kx = tid; kx < LX; kx += NT) {
+                const float2* in = vc + ((long)((kx >> a.cs) * a.ny + y) << a.cs) + (kx & (cols - 1));
+                float2 v[PZ];
+                BD_UNROLL
+                for (int kz = 0; kz < PZ; ++kz) v[kz] = in[kz * kzs];
+                if (kx == 0) {
+                    // P^ = Y0^ + i YN^
+                    const float2* inn = vc + ((long)((LX >> a.cs) * a.ny + y) << a.cs) + (LX & (cols - 1));
+                    BD_UNROLL
+                    for (int kz = 0; kz < PZ; ++kz) {
+                        const float2 n = inn[kz * kzs];
+                        v[kz] = bd_f2(v[kz].x - n.y, v[kz].y + n.x);
+                    }
+                }
+                ZCol<PZ>::inv(v);
+                float2* col = sm + xz_pos(a.xpost, LX, kx);
+                BD_UNROLL
+                for (int z = 0; z < NZ; ++z) col[z * PITCH] = v[z];
+            }
+        } else if constexpr (PH == 1) {
+            constexpr int items = (LX / 2 + 1) * NZ;
+            for (int w0 = tid; w0 < items; w0 += 4 * NT) {
+                float2 Yk[4], Ym[4];
+                float4 xp[4];
+                BD_UNROLL
+                for (int u = 0; u < 4; ++u) {
+                    const int w = w0 + u * NT;
+                    if (w < items) {
+                        const int kp = w / NZ, row = w % NZ;
+                        xp[u] = BD_LDG(&a.xpost[kp]);
+                        const float2* zr = sm + row * PITCH;
+                        Yk[u] = zr[bd_float_as_int(xp[u].z)];
+                        Ym[u] = zr[bd_float_as_int(xp[u].w)];
+                    }
+                }
+                BD_UNROLL
+                for (int u = 0; u < 4; ++u) {
+                    const int w = w0 + u * NT;
+                    if (w < items) {
+                        const int kp = w / NZ, row = w % NZ;
+                        if (kp == 0) { Ym[u] = bd_f2(Yk[u].y, 0.f); Yk[u].y = 0.f; }   // P = (Y[0], Y[LX]), both real
+                        const float2 E = bd_f2(Yk[u].x + Ym[u].x, Yk[u].y - Ym[u].y);
+                        const float2 D = bd_f2(Yk[u].x - Ym[u].x, Yk[u].y + Ym[u].y);
+                        const float2 O = pk_cmulc(D, make_tw(bd_f2(xp[u].x, xp[u].y)));
+                        float2* zr = sm + row * PITCH;
+                        zr[bd_float_as_int(xp[u].z)] = bd_f2(E.x - O.y, E.y + O.x);
+                        if (kp != 0 && 2 * kp != LX) zr[bd_float_as_int(xp[u].w)] = bd_f2(E.x + O.y, O.x - E.y);
+                    }
+                }
+            }
+        } else if constexpr (PH <= NP) {
+            // phases 2..NP run inverse passes NP-1..1
+            x_rows_pass<LX, NP + 1 - PH, true, NT>(tid, NZ, s, s, a.ptw);
+        } else {
+            GRowsOut out{a.H + ((long)c * NZ * a.ny + y) * LX, (long)a.ny * LX};
+            x_rows_pass<LX, 0, true, NT>(tid, NZ, s, out, a.ptw);
+        }
+    }
+};
+
+}  // namespace bd
