@@ -18,9 +18,12 @@
 #if defined(__CUDA_ARCH__)
 #define BD_LDG(p) __ldg(p)
 #define BD_UNROLL _Pragma("unroll")
+#define BD_PRAGMA_(x) _Pragma(#x)
+#define BD_UNROLL_N(n) BD_PRAGMA_(unroll n)
 #else
 #define BD_LDG(p) (*(p))
 #define BD_UNROLL
+#define BD_UNROLL_N(n)
 #endif
 
 #include <vector_types.h>   // float2, float4, double2 (plain structs on the host)

@@ -167,56 +167,29 @@ BD_HD float2 pk_mul_w64(float2 z, int m) {
     return pk_fma(pk_swap(z), bd_f2(-s, s), pk_mul(z, pk_bc(c)));
 }
 
-// Column transforms in registers.  fwd: v[0..PZ/2) -> v[0..PZ) (natural order, zero-padded
-// input); inv: v[0..PZ) -> v[0..PZ/2) (unnormalised, upper half dropped).
+// Column transforms in registers, one half of the padded spectrum at a time (a column of
+// PZ = 2 NZ points would not fit the register budget of a 512-thread block):
+//   fwd_half<PAR>: x[0..NZ) (zero-padded to PZ) -> v[k] = X[2k + PAR]
+//                  X[2k + PAR] = sum_z (x[z] W_PZ^(PAR z)) W_NZ^(k z)
+//   inv_half<PAR>: v[k] = Y[2k + PAR] -> the part of x[z], z < NZ, carried by those
+//                  frequencies: W_PZ^(-PAR z) sum_k Y[2k + PAR] W_NZ^(-k z)   (unnormalised)
 template <int PZ>
 struct ZCol {
-    static BD_HD void fwd(float2* v) { PkDftPruned<PZ, -1>::run(v); }
-    static BD_HD void inv(float2* v) { PkDftTrunc<PZ, +1>::run(v); }
-};
-template <>
-struct ZCol<64> {
-    // kz = q0 + 8 q1, z = j + 8 r:  X[kz] = sum_j W8^(j q1) [ W64^(j q0) sum_r x[j + 8r] W8^(r q0) ]
-    static BD_HD void fwd(float2* v) {
-        float2 t[8][8];
-        BD_UNROLL
-        for (int j = 0; j < 8; ++j) {
-            float2 u[8];
+    static constexpr int NZ = PZ / 2;
+    template <int PAR>
+    static BD_HD void fwd_half(float2* v) {
+        if constexpr (PAR == 1) {
             BD_UNROLL
-            for (int r = 0; r < 4; ++r) u[r] = v[j + 8 * r];
-            PkDftPruned<8, -1>::run(u);
-            BD_UNROLL
-            for (int q0 = 0; q0 < 8; ++q0) t[j][q0] = pk_mul_w64<-1>(u[q0], j * q0);
+            for (int z = 0; z < NZ; ++z) v[z] = pk_mul_w64<-1>(v[z], z * (64 / PZ));
         }
-        BD_UNROLL
-        for (int q0 = 0; q0 < 8; ++q0) {
-            float2 a[8];
-            BD_UNROLL
-            for (int j = 0; j < 8; ++j) a[j] = t[j][q0];
-            PkDft<8, -1>::run(a);
-            BD_UNROLL
-            for (int q1 = 0; q1 < 8; ++q1) v[q0 + 8 * q1] = a[q1];
-        }
+        PkDft<NZ, -1>::run(v);
     }
-    static BD_HD void inv(float2* v) {
-        float2 t[8][8];
-        BD_UNROLL
-        for (int q0 = 0; q0 < 8; ++q0) {
-            float2 a[8];
+    template <int PAR>
+    static BD_HD void inv_half(float2* v) {
+        PkDft<NZ, +1>::run(v);
+        if constexpr (PAR == 1) {
             BD_UNROLL
-            for (int q1 = 0; q1 < 8; ++q1) a[q1] = v[q0 + 8 * q1];
-            PkDft<8, +1>::run(a);
-            BD_UNROLL
-            for (int j = 0; j < 8; ++j) t[j][q0] = pk_mul_w64<+1>(a[j], j * q0);
-        }
-        BD_UNROLL
-        for (int j = 0; j < 8; ++j) {
-            float2 u[8];
-            BD_UNROLL
-            for (int q0 = 0; q0 < 8; ++q0) u[q0] = t[j][q0];
-            PkDftTrunc<8, +1>::run(u);
-            BD_UNROLL
-            for (int r = 0; r < 4; ++r) v[j + 8 * r] = u[r];
+            for (int z = 0; z < NZ; ++z) v[z] = pk_mul_w64<+1>(v[z], z * (64 / PZ));
         }
     }
 };
@@ -241,13 +214,35 @@ template <int LX, int NZ>
 struct XZFwd {
     using Args = XZArgs;
     static constexpr int KIND = kKindXZFwd;
-    static constexpr int NT = 256;
+    static constexpr int NT = 512;
     static constexpr int MINB = 1;
     static constexpr int NP = dec_np(LX);
     static constexpr int NPHASES = NP + 2;
     static constexpr int PZ = 2 * NZ;
     static constexpr int PITCH = SRows<LX>::PITCH;
     static BD_HD long smem_elems(const Args&) { return (long)NZ * PITCH; }
+
+    // frequencies kz = 2k + PAR of one column; column 0 carries P = X[0] + i X[LX]
+    template <int PAR>
+    static BD_HD void zhalf(const float2* col, float2* out, float2* outn, long kzs, int kx) {
+        float2 v[NZ];
+        BD_UNROLL
+        for (int z = 0; z < NZ; ++z) v[z] = col[z * PITCH];
+        ZCol<PZ>::template fwd_half<PAR>(v);
+        if (kx != 0) {
+            BD_UNROLL
+            for (int k = 0; k < NZ; ++k) out[(2 * k + PAR) * kzs] = v[k];
+        } else {
+            BD_UNROLL
+            for (int k = 0; k < NZ; ++k) {
+                // mirror frequency PZ - (2k + PAR) sits in the same half at index km
+                const int km = PAR ? NZ - 1 - k : (NZ - k) % NZ;
+                const float2 p = v[k], m = v[km];
+                out[(2 * k + PAR) * kzs] = bd_f2(0.5f * (p.x + m.x), 0.5f * (p.y - m.y));
+                outn[(2 * k + PAR) * kzs] = bd_f2(0.5f * (p.y + m.y), 0.5f * (m.x - p.x));
+            }
+        }
+    }
 
     template <int PH>
     static BD_HD void phase(int tid, int bx, int by, const Args& a, float2* sm) {
@@ -300,23 +295,10 @@ struct XZFwd {
             float2* vc = a.V + (long)c * PZ * kzs;
             for (int kx = tid; kx < LX; kx += NT) {
                 const float2* col = sm + xz_pos(a.xpost, LX, kx);
-                float2 v[PZ];
-                BD_UNROLL
-                for (int z = 0; z < NZ; ++z) v[z] = col[z * PITCH];
-                ZCol<PZ>::fwd(v);
                 float2* out = vc + ((long)((kx >> a.cs) * a.ny + y) << a.cs) + (kx & (cols - 1));
-                if (kx != 0) {
-                    BD_UNROLL
-                    for (int kz = 0; kz < PZ; ++kz) out[kz * kzs] = v[kz];
-                } else {
-                    float2* outn = vc + ((long)((LX >> a.cs) * a.ny + y) << a.cs) + (LX & (cols - 1));
-                    BD_UNROLL
-                    for (int kz = 0; kz < PZ; ++kz) {
-                        const float2 p = v[kz], m = v[(PZ - kz) % PZ];
-                        out[kz * kzs] = bd_f2(0.5f * (p.x + m.x), 0.5f * (p.y - m.y));
-                        outn[kz * kzs] = bd_f2(0.5f * (p.y + m.y), 0.5f * (m.x - p.x));
-                    }
-                }
+                float2* outn = vc + ((long)((LX >> a.cs) * a.ny + y) << a.cs) + (LX & (cols - 1));
+                zhalf<0>(col, out, outn, kzs, kx);
+                zhalf<1>(col, out, outn, kzs, kx);
             }
         }
     }
@@ -326,13 +308,37 @@ template <int LX, int NZ>
 struct ZXInv {
     using Args = XZArgs;
     static constexpr int KIND = kKindZXInv;
-    static constexpr int NT = 256;
+    static constexpr int NT = 512;
     static constexpr int MINB = 1;
     static constexpr int NP = dec_np(LX);
     static constexpr int NPHASES = NP + 2;
     static constexpr int PZ = 2 * NZ;
     static constexpr int PITCH = SRows<LX>::PITCH;
     static BD_HD long smem_elems(const Args&) { return (long)NZ * PITCH; }
+
+    // frequencies kz = 2k + PAR of one column -> their part of x[z]; the odd half adds to
+    // what the even half left in shared memory.  Column 0 carries P^ = Y0^ + i YN^.
+    template <int PAR>
+    static BD_HD void zhalf(const float2* in, const float2* inn, float2* col, long kzs, int kx) {
+        float2 v[NZ];
+        BD_UNROLL
+        for (int k = 0; k < NZ; ++k) v[k] = in[(2 * k + PAR) * kzs];
+        if (kx == 0) {
+            BD_UNROLL
+            for (int k = 0; k < NZ; ++k) {
+                const float2 n = inn[(2 * k + PAR) * kzs];
+                v[k] = bd_f2(v[k].x - n.y, v[k].y + n.x);
+            }
+        }
+        ZCol<PZ>::template inv_half<PAR>(v);
+        if constexpr (PAR == 0) {
+            BD_UNROLL
+            for (int z = 0; z < NZ; ++z) col[z * PITCH] = v[z];
+        } else {
+            BD_UNROLL
+            for (int z = 0; z < NZ; ++z) col[z * PITCH] = pk_add(col[z * PITCH], v[z]);
+        }
+    }
 
     template <int PH>
     static BD_HD void phase(int tid, int bx, int by, const Args& a, float2* sm) {
@@ -344,22 +350,10 @@ struct ZXInv {
             const float2* vc = a.V + (long)c * PZ * kzs;
             for (int kx = tid; kx < LX; kx += NT) {
                 const float2* in = vc + ((long)((kx >> a.cs) * a.ny + y) << a.cs) + (kx & (cols - 1));
-                float2 v[PZ];
-                BD_UNROLL
-                for (int kz = 0; kz < PZ; ++kz) v[kz] = in[kz * kzs];
-                if (kx == 0) {
-                    // P^ = Y0^ + i YN^
-                    const float2* inn = vc + ((long)((LX >> a.cs) * a.ny + y) << a.cs) + (LX & (cols - 1));
-                    BD_UNROLL
-                    for (int kz = 0; kz < PZ; ++kz) {
-                        const float2 n = inn[kz * kzs];
-                        v[kz] = bd_f2(v[kz].x - n.y, v[kz].y + n.x);
-                    }
-                }
-                ZCol<PZ>::inv(v);
+                const float2* inn = vc + ((long)((LX >> a.cs) * a.ny + y) << a.cs) + (LX & (cols - 1));
                 float2* col = sm + xz_pos(a.xpost, LX, kx);
-                BD_UNROLL
-                for (int z = 0; z < NZ; ++z) col[z * PITCH] = v[z];
+                zhalf<0>(in, inn, col, kzs, kx);
+                zhalf<1>(in, inn, col, kzs, kx);
             }
         } else if constexpr (PH == 1) {
             constexpr int items = (LX / 2 + 1) * NZ;

@@ -86,7 +86,7 @@ struct GTile {                 // global: V tile [y][col], component stride cstr
 
 // ------------------------------------------------------------------ passes
 // pencils c = c0, c0 + cstep, ... < cend share the butterfly index `it` and its twiddles
-template <int L, int P, class In, class Out>
+template <int L, int P, int NCT = 0, class In, class Out>
 BD_HD void fwd_passM(int it, int c0, int cstep, int cend, const In& in, const Out& out, const float2* __restrict__ ptw) {
     constexpr int NP = dec_np(L), R = dec_r(L, P), Lp = dec_sublen(L, P), S = Lp / R;
     const int blk = it / S, j = it - blk * S, base = blk * Lp + j;
@@ -103,6 +103,8 @@ BD_HD void fwd_passM(int it, int c0, int cstep, int cend, const In& in, const Ou
         BD_UNROLL
         for (int r = 0; r < NIN; ++r) nxt[r] = In::ld(pi + r * In::step(S));
     }
+    // NCT > 0: the pencil count is known, the loop is unrolled and the copies below vanish
+    BD_UNROLL_N(NCT > 0 ? NCT : 1)
     for (int c = c0; c < cend; c += cstep) {
         float2 v[R];
         BD_UNROLL
@@ -124,7 +126,7 @@ BD_HD void fwd_passM(int it, int c0, int cstep, int cend, const In& in, const Ou
     }
 }
 
-template <int L, int P, class In, class Out>
+template <int L, int P, int NCT = 0, class In, class Out>
 BD_HD void inv_passM(int it, int c0, int cstep, int cend, const In& in, const Out& out, const float2* __restrict__ ptw) {
     constexpr int NP = dec_np(L), R = dec_r(L, P), Lp = dec_sublen(L, P), S = Lp / R;
     const int blk = it / S, j = it - blk * S, base = blk * Lp + j;
@@ -139,6 +141,7 @@ BD_HD void inv_passM(int it, int c0, int cstep, int cend, const In& in, const Ou
         BD_UNROLL
         for (int q = 0; q < R; ++q) nxt[q] = In::ld(pi + q * In::step(S));
     }
+    BD_UNROLL_N(NCT > 0 ? NCT : 1)
     for (int c = c0; c < cend; c += cstep) {
         float2 v[R];
         BD_UNROLL
@@ -167,11 +170,11 @@ BD_HD void inv_passM(int it, int c0, int cstep, int cend, const In& in, const Ou
 
 template <int L, int P, class In, class Out>
 BD_HD void fwd_pass3(int it, const In& in, const Out& out, const float2* __restrict__ ptw) {
-    fwd_passM<L, P>(it, 0, 1, 3, in, out, ptw);
+    fwd_passM<L, P, 3>(it, 0, 1, 3, in, out, ptw);
 }
 template <int L, int P, class In, class Out>
 BD_HD void inv_pass3(int it, const In& in, const Out& out, const float2* __restrict__ ptw) {
-    inv_passM<L, P>(it, 0, 1, 3, in, out, ptw);
+    inv_passM<L, P, 3>(it, 0, 1, 3, in, out, ptw);
 }
 
 // ------------------------------------------------------------------ kernel-spectrum tile
@@ -199,8 +202,8 @@ BD_HD int f_to_slot(int L, int f) {       // f <= F/2
 }
 
 // last forward pass + multiply + first inverse pass of item i (frequency offset f)
-template <int L, int NC, bool REV, class In, class Out>
-BD_HD void mid3(int i, const float* __restrict__ kslot, int cstride, float sz, const In& in, const Out& out) {
+template <int L, int NC, bool REV, bool ZREV, class In, class Out>
+BD_HD void mid3(int i, const float* __restrict__ kslot, int cstride, const In& in, const Out& out) {
     constexpr int NP = dec_np(L), RL = dec_rlast(L);
     // kslot points at chunk 0 of component 0 for this thread's (slot, col); consecutive
     // chunks are cstride floats apart
@@ -234,7 +237,7 @@ BD_HD void mid3(int i, const float* __restrict__ kslot, int cstride, float sz, c
         }
     }
     // odd-component signs moved onto the data: with my' = sy my, mz' = sz mz the products
-    // use the stored values and Hy = sy Hy', Hz = sz Hz'  (sy = -1 for REV, else +1)
+    // use the stored values and Hy = sy Hy', Hz = sz Hz'  (sy = -1 for REV, sz = -1 for ZREV)
     BD_UNROLL
     for (int q = 0; q < RL; ++q) {
         const int qq = REV ? RL - 1 - q : q;
@@ -249,14 +252,14 @@ BD_HD void mid3(int i, const float* __restrict__ kslot, int cstride, float sz, c
             v[1][q] = REV ? pk_neg(hy) : hy;
             v[2][q] = pk_mul(kzz, v[2][q]);
         } else {
-            const float2 mz = pk_mul(pk_bc(sz), v[2][q]);
+            const float2 mz = ZREV ? pk_neg(v[2][q]) : v[2][q];
             const float2 kxz = pk_bc(k[4][qq]), kyz = pk_bc(k[5][qq]);
             const float2 hx = pk_fma(kxz, mz, pk_fma(kxy, my, pk_mul(kxx, mx)));
             const float2 hy = pk_fma(kyz, mz, pk_fma(kyy, my, pk_mul(kxy, mx)));
             const float2 hz = pk_fma(kzz, mz, pk_fma(kyz, my, pk_mul(kxz, mx)));
             v[0][q] = hx;
             v[1][q] = REV ? pk_neg(hy) : hy;
-            v[2][q] = pk_mul(pk_bc(sz), hz);
+            v[2][q] = ZREV ? pk_neg(hz) : hz;
         }
     }
     BD_UNROLL
@@ -373,11 +376,17 @@ struct YFused {
             const float* krow = kt + ((long)f_to_slot(L, row) * COLS + col) * CH;
             if constexpr (NP == 1) {
                 GTile<COLS> g = gtile(b, col, a);
-                mid3<L, NC, false>(i, krow, KCS, b.sz, g, g);
+                if (b.sz < 0.f) mid3<L, NC, false, true>(i, krow, KCS, g, g);
+                else mid3<L, NC, false, false>(i, krow, KCS, g, g);
             } else {
                 STile<L, COLS> s{sm + col};
-                if (rev) mid3<L, NC, true>(i, krow, KCS, b.sz, s, s);
-                else mid3<L, NC, false>(i, krow, KCS, b.sz, s, s);
+                if (b.sz < 0.f) {
+                    if (rev) mid3<L, NC, true, true>(i, krow, KCS, s, s);
+                    else mid3<L, NC, false, true>(i, krow, KCS, s, s);
+                } else {
+                    if (rev) mid3<L, NC, true, false>(i, krow, KCS, s, s);
+                    else mid3<L, NC, false, false>(i, krow, KCS, s, s);
+                }
             }
         }
     }
