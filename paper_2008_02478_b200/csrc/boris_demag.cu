@@ -173,8 +173,19 @@ __global__ void __launch_bounds__(kEnergyThreads) k_energy_partial(const float4*
                                                                     long n4, double* partial) {
     __shared__ double sh[32];
     double acc = 0.0;
-    for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < n4; i += (long)gridDim.x * blockDim.x) {
-        const float4 m = __ldg(&M[i]), h = __ldg(&H[i]);
+    const long stride = (long)gridDim.x * blockDim.x;
+    long i = blockIdx.x * (long)blockDim.x + threadIdx.x;
+    // four independent 16-byte load pairs in flight per thread
+    for (; i + 3 * stride < n4; i += 4 * stride) {
+        float4 m[4], h[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { m[u] = __ldcg(&M[i + u * stride]); h[u] = __ldcg(&H[i + u * stride]); }
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            acc += (double)m[u].x * h[u].x + (double)m[u].y * h[u].y + (double)m[u].z * h[u].z + (double)m[u].w * h[u].w;
+    }
+    for (; i < n4; i += stride) {
+        const float4 m = __ldcg(&M[i]), h = __ldcg(&H[i]);
         acc += (double)m.x * h.x + (double)m.y * h.y + (double)m.z * h.z + (double)m.w * h.w;
     }
     acc = block_sum(acc, sh);

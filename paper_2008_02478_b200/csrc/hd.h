@@ -17,11 +17,15 @@
 
 #if defined(__CUDA_ARCH__)
 #define BD_LDG(p) __ldg(p)
+#define BD_LDCG(p) __ldcg(p)
+#define BD_STCG(p, v) __stcg((p), (v))
 #define BD_UNROLL _Pragma("unroll")
 #define BD_PRAGMA_(x) _Pragma(#x)
 #define BD_UNROLL_N(n) BD_PRAGMA_(unroll n)
 #else
 #define BD_LDG(p) (*(p))
+#define BD_LDCG(p) (*(p))
+#define BD_STCG(p, v) (*(p) = (v))
 #define BD_UNROLL
 #define BD_UNROLL_N(n)
 #endif

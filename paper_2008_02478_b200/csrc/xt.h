@@ -32,7 +32,7 @@ struct GRowsIn {               // rows of a real array read as (x[2m], x[2m+1]) 
     const float* p; long pitch;
     static BD_HD constexpr int step(int S) { return S; }
     BD_HD const float2* ptr(int row, int e) const { return reinterpret_cast<const float2*>(p + row * pitch) + e; }
-    static BD_HD float2 ld(const float2* q) { return BD_LDG(q); }
+    static BD_HD float2 ld(const float2* q) { return BD_LDCG(q); }
 };
 struct GRowsOut {
     float* p; long pitch;
@@ -142,8 +142,8 @@ struct XFwdT {
                         const float2 T = pk_cmul(bd_f2(B.y, -B.x), make_tw(tw[u]));
                         const float2 Xk = pk_add(A, T), Xm = bd_f2(A.x - T.x, T.y - A.y);
                         const int y = y0 + row;
-                        vc[((kp / COLS) * a.ny + y) * COLS + kp % COLS] = Xk;
-                        if (2 * kp != LX) vc[((km / COLS) * a.ny + y) * COLS + km % COLS] = Xm;
+                        BD_STCG(&vc[((kp / COLS) * a.ny + y) * COLS + kp % COLS], Xk);
+                        if (2 * kp != LX) BD_STCG(&vc[((km / COLS) * a.ny + y) * COLS + km % COLS], Xm);
                     }
                 }
             }
@@ -178,8 +178,8 @@ struct XInvT {
                     if (w < items) {
                         const int kp = w >> a.rbs, row = w & (a.rb - 1);
                         const int km = LX - kp, y = y0 + row;
-                        Yk[u] = vc[((kp / COLS) * a.ny + y) * COLS + kp % COLS];
-                        Ym[u] = vc[((km / COLS) * a.ny + y) * COLS + km % COLS];
+                        Yk[u] = BD_LDCG(&vc[((kp / COLS) * a.ny + y) * COLS + kp % COLS]);
+                        Ym[u] = BD_LDCG(&vc[((km / COLS) * a.ny + y) * COLS + km % COLS]);
                         xp[u] = BD_LDG(&a.xpost[kp]);
                     }
                 }

@@ -229,17 +229,19 @@ struct XZFwd {
         BD_UNROLL
         for (int z = 0; z < NZ; ++z) v[z] = col[z * PITCH];
         ZCol<PZ>::template fwd_half<PAR>(v);
+        out += PAR * kzs; outn += PAR * kzs;
         if (kx != 0) {
             BD_UNROLL
-            for (int k = 0; k < NZ; ++k) out[(2 * k + PAR) * kzs] = v[k];
+            for (int k = 0; k < NZ; ++k) { BD_STCG(out, v[k]); out += 2 * kzs; }
         } else {
             BD_UNROLL
             for (int k = 0; k < NZ; ++k) {
                 // mirror frequency PZ - (2k + PAR) sits in the same half at index km
                 const int km = PAR ? NZ - 1 - k : (NZ - k) % NZ;
                 const float2 p = v[k], m = v[km];
-                out[(2 * k + PAR) * kzs] = bd_f2(0.5f * (p.x + m.x), 0.5f * (p.y - m.y));
-                outn[(2 * k + PAR) * kzs] = bd_f2(0.5f * (p.y + m.y), 0.5f * (m.x - p.x));
+                BD_STCG(out, bd_f2(0.5f * (p.x + m.x), 0.5f * (p.y - m.y)));
+                BD_STCG(outn, bd_f2(0.5f * (p.y + m.y), 0.5f * (m.x - p.x)));
+                out += 2 * kzs; outn += 2 * kzs;
             }
         }
     }
@@ -322,11 +324,13 @@ struct ZXInv {
     static BD_HD void zhalf(const float2* in, const float2* inn, float2* col, long kzs, int kx) {
         float2 v[NZ];
         BD_UNROLL
-        for (int k = 0; k < NZ; ++k) v[k] = in[(2 * k + PAR) * kzs];
+        in += PAR * kzs; inn += PAR * kzs;
+        for (int k = 0; k < NZ; ++k) { v[k] = BD_LDCG(in); in += 2 * kzs; }
         if (kx == 0) {
             BD_UNROLL
             for (int k = 0; k < NZ; ++k) {
-                const float2 n = inn[(2 * k + PAR) * kzs];
+                const float2 n = BD_LDCG(inn);
+                inn += 2 * kzs;
                 v[k] = bd_f2(v[k].x - n.y, v[k].y + n.x);
             }
         }

@@ -81,7 +81,7 @@ struct GTile {                 // global: V tile [y][col], component stride cstr
     float2* p; long cstride;   // already offset by col
     static BD_HD constexpr int step(int S) { return S * COLS; }
     BD_HD float2* ptr(int c, int e) const { return p + c * cstride + (long)e * COLS; }
-    static BD_HD float2 ld(const float2* q) { return *q; }
+    static BD_HD float2 ld(const float2* q) { return BD_LDCG(q); }     // streamed once: keep it out of L1
 };
 
 // ------------------------------------------------------------------ passes
@@ -215,7 +215,7 @@ BD_HD void mid3(int i, const float* __restrict__ kslot, int cstride, const In& i
         for (int ch = 0; ch < NCH; ++ch) {
             const float* kp = kslot + (long)(c * NCH + ch) * cstride;
             if constexpr (CH == 4) {
-                const float4 t = BD_LDG(reinterpret_cast<const float4*>(kp));
+                const float4 t = BD_LDCG(reinterpret_cast<const float4*>(kp));
                 k[c][4 * ch] = t.x; k[c][4 * ch + 1] = t.y; k[c][4 * ch + 2] = t.z; k[c][4 * ch + 3] = t.w;
             } else {
                 BD_UNROLL
