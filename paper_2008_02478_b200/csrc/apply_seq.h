@@ -32,7 +32,7 @@ constexpr long kMaxDynSmem = 227L * 1024;
 // z column (2 nz points) in registers
 inline bool tiled_supported(int nx, int ny, int nz) {
     if (nz == 1) return true;
-    return nz <= 32 && (long)nz * (padlen8(nx) | 1) * (long)sizeof(float2) <= kMaxDynSmem;
+    return nz <= 32 && (long)nz * ((prow(nx, nx - 1) + 1) | 1) * (long)sizeof(float2) <= kMaxDynSmem;
 }
 
 inline LaunchCfg make_launch_cfg(int nx, int ny, int nz) {
@@ -142,7 +142,7 @@ int enqueue_tiled_3d(Launcher& run, const PlanView& p, const float* M, float* H)
             constexpr int LX = decltype(ic)::value;
             auto go = [&](auto nzc) {
                 constexpr int NZ = decltype(nzc)::value;
-                if constexpr ((long)NZ * (padlen8(LX) | 1) * (long)sizeof(float2) <= kMaxDynSmem && LX <= 1024) {
+                if constexpr ((long)NZ * SRows<LX>::PITCH * (long)sizeof(float2) <= kMaxDynSmem && LX <= 1024) {
                     if constexpr (decltype(fwd)::value) return run.template run<XZFwd<LX, NZ>>(gx, xa);
                     else return run.template run<ZXInv<LX, NZ>>(gx, xa);
                 } else {

@@ -20,23 +20,29 @@
 
 namespace bd {
 
+// Shared rows (one pencil per row, threads of a half warp on 16 consecutive elements, on
+// items 8 apart, or — the z columns of xz.h — on consecutive kx, whose positions are L/R0
+// apart): padded by one element per 16 and crow(L) per 128, which keeps those patterns on
+// different banks (at most 2-way conflicts) and still gives p(base + r S) = p(base) + p(r S).
+BD_HD constexpr int crow(int L) { return L == 256 ? 2 : 1; }
+BD_HD constexpr int prow(int L, int e) { return e + (e >> 4) + crow(L) * (e >> 7); }
 template <int L>
-struct SRows {                 // shared rows of L points, padded like the tiles (yfused.h), pitch odd
+struct SRows {
     float2* p;
-    static constexpr int PITCH = padlen8(L) | 1;
-    static BD_HD constexpr int step(int S) { return pstep(S); }
-    BD_HD float2* ptr(int row, int e) const { return p + row * PITCH + pidx(e); }
+    static constexpr int PITCH = (prow(L, L - 1) + 1) | 1;
+    static BD_HD constexpr int off(int S, int r) { return prow(L, r * S); }
+    BD_HD float2* ptr(int row, int e) const { return p + row * PITCH + prow(L, e); }
     static BD_HD float2 ld(const float2* q) { return *q; }
 };
 struct GRowsIn {               // rows of a real array read as (x[2m], x[2m+1]) pairs
     const float* p; long pitch;
-    static BD_HD constexpr int step(int S) { return S; }
+    static BD_HD constexpr int off(int S, int r) { return r * S; }
     BD_HD const float2* ptr(int row, int e) const { return reinterpret_cast<const float2*>(p + row * pitch) + e; }
     static BD_HD float2 ld(const float2* q) { return BD_LDCG(q); }
 };
 struct GRowsOut {
     float* p; long pitch;
-    static BD_HD constexpr int step(int S) { return S; }
+    static BD_HD constexpr int off(int S, int r) { return r * S; }
     BD_HD float2* ptr(int row, int e) const { return reinterpret_cast<float2*>(p + row * pitch) + e; }
 };
 
@@ -67,7 +73,7 @@ inline void fill_xpost(float4* h, int LX) {
         float2 w = bd_f2((float)std::cos(a), (float)std::sin(a));
         if (kp == 0) w = bd_f2(1.f, 0.f);
         if (2 * kp == LX) w = bd_f2(0.f, -1.f);
-        const int pk = pidx(pos_of_freq(LX, kp)), pm = pidx(pos_of_freq(LX, (LX - kp) & (LX - 1)));
+        const int pk = prow(LX, pos_of_freq(LX, kp)), pm = prow(LX, pos_of_freq(LX, (LX - kp) & (LX - 1)));
         float fk, fm;
         std::memcpy(&fk, &pk, sizeof fk); std::memcpy(&fm, &pm, sizeof fm);
         h[kp].x = w.x; h[kp].y = w.y; h[kp].z = fk; h[kp].w = fm;

@@ -66,20 +66,20 @@ BD_HD constexpr int padlen8(int L) { return L + (L >> 3); }
 BD_HD int pidx(int e) { return e + (e >> 3); }
 BD_HD constexpr int pstep(int S) { return S >= 8 ? S + (S >> 3) : S; }
 
-// An accessor gives ptr(c, e) -> address of element e of pencil c, STEP(S) -> distance
-// (in elements of the pointer) between e and e + S, and ld() to read.
+// An accessor gives ptr(c, e) -> address of element e of pencil c, off(S, r) -> distance
+// (in elements of the pointer) between e and e + r S, and ld() to read.
 template <int L, int COLS>
 struct STile {                 // shared: S[c][p(e)][col]
     float2* p;                 // already offset by col
     static constexpr int CP = padlen8(L) * COLS;
-    static BD_HD constexpr int step(int S) { return pstep(S) * COLS; }
+    static BD_HD constexpr int off(int S, int r) { return r * pstep(S) * COLS; }
     BD_HD float2* ptr(int c, int e) const { return p + c * CP + pidx(e) * COLS; }
     static BD_HD float2 ld(const float2* q) { return *q; }
 };
 template <int COLS>
 struct GTile {                 // global: V tile [y][col], component stride cstride
     float2* p; long cstride;   // already offset by col
-    static BD_HD constexpr int step(int S) { return S * COLS; }
+    static BD_HD constexpr int off(int S, int r) { return r * S * COLS; }
     BD_HD float2* ptr(int c, int e) const { return p + c * cstride + (long)e * COLS; }
     static BD_HD float2 ld(const float2* q) { return BD_LDCG(q); }     // streamed once: keep it out of L1
 };
@@ -101,7 +101,7 @@ BD_HD void fwd_passM(int it, int c0, int cstep, int cend, const In& in, const Ou
     {
         const auto* pi = in.ptr(c0, base);
         BD_UNROLL
-        for (int r = 0; r < NIN; ++r) nxt[r] = In::ld(pi + r * In::step(S));
+        for (int r = 0; r < NIN; ++r) nxt[r] = In::ld(pi + In::off(S, r));
     }
     // NCT > 0: the pencil count is known, the loop is unrolled and the copies below vanish
     BD_UNROLL_N(NCT > 0 ? NCT : 1)
@@ -112,7 +112,7 @@ BD_HD void fwd_passM(int it, int c0, int cstep, int cend, const In& in, const Ou
         if (c + cstep < cend) {
             const auto* pi = in.ptr(c + cstep, base);
             BD_UNROLL
-            for (int r = 0; r < NIN; ++r) nxt[r] = In::ld(pi + r * In::step(S));
+            for (int r = 0; r < NIN; ++r) nxt[r] = In::ld(pi + In::off(S, r));
         }
         if constexpr (P == 0) PkDftPruned<R, -1>::run(v);
         else PkDft<R, -1>::run(v);
@@ -122,7 +122,7 @@ BD_HD void fwd_passM(int it, int c0, int cstep, int cend, const In& in, const Ou
         }
         float2* po = out.ptr(c, base);
         BD_UNROLL
-        for (int q = 0; q < R; ++q) po[q * Out::step(S)] = v[q];
+        for (int q = 0; q < R; ++q) po[Out::off(S, q)] = v[q];
     }
 }
 
@@ -139,7 +139,7 @@ BD_HD void inv_passM(int it, int c0, int cstep, int cend, const In& in, const Ou
     {
         const auto* pi = in.ptr(c0, base);
         BD_UNROLL
-        for (int q = 0; q < R; ++q) nxt[q] = In::ld(pi + q * In::step(S));
+        for (int q = 0; q < R; ++q) nxt[q] = In::ld(pi + In::off(S, q));
     }
     BD_UNROLL_N(NCT > 0 ? NCT : 1)
     for (int c = c0; c < cend; c += cstep) {
@@ -149,7 +149,7 @@ BD_HD void inv_passM(int it, int c0, int cstep, int cend, const In& in, const Ou
         if (c + cstep < cend) {
             const auto* pi = in.ptr(c + cstep, base);
             BD_UNROLL
-            for (int q = 0; q < R; ++q) nxt[q] = In::ld(pi + q * In::step(S));
+            for (int q = 0; q < R; ++q) nxt[q] = In::ld(pi + In::off(S, q));
         }
         if constexpr (P < NP - 1) {
             BD_UNROLL
@@ -159,11 +159,11 @@ BD_HD void inv_passM(int it, int c0, int cstep, int cend, const In& in, const Ou
         if constexpr (P == 0) {
             PkDftTrunc<R, +1>::run(v);
             BD_UNROLL
-            for (int r = 0; r < R / 2; ++r) po[r * Out::step(S)] = v[r];
+            for (int r = 0; r < R / 2; ++r) po[Out::off(S, r)] = v[r];
         } else {
             PkDft<R, +1>::run(v);
             BD_UNROLL
-            for (int r = 0; r < R; ++r) po[r * Out::step(S)] = v[r];
+            for (int r = 0; r < R; ++r) po[Out::off(S, r)] = v[r];
         }
     }
 }
@@ -228,11 +228,11 @@ BD_HD void mid3(int i, const float* __restrict__ kslot, int cstride, const In& i
     for (int c = 0; c < 3; ++c) {
         if constexpr (NP == 1) {
             BD_UNROLL
-            for (int q = 0; q < RL / 2; ++q) v[c][q] = In::ld(in.ptr(c, i * RL) + q * In::step(1));
+            for (int q = 0; q < RL / 2; ++q) v[c][q] = In::ld(in.ptr(c, i * RL) + In::off(1, q));
             PkDftPruned<RL, -1>::run(v[c]);
         } else {
             BD_UNROLL
-            for (int q = 0; q < RL; ++q) v[c][q] = In::ld(in.ptr(c, i * RL) + q * In::step(1));
+            for (int q = 0; q < RL; ++q) v[c][q] = In::ld(in.ptr(c, i * RL) + In::off(1, q));
             PkDft<RL, -1>::run(v[c]);
         }
     }
@@ -267,11 +267,11 @@ BD_HD void mid3(int i, const float* __restrict__ kslot, int cstride, const In& i
         if constexpr (NP == 1) {
             PkDftTrunc<RL, +1>::run(v[c]);
             BD_UNROLL
-            for (int q = 0; q < RL / 2; ++q) out.ptr(c, i * RL)[q * Out::step(1)] = v[c][q];
+            for (int q = 0; q < RL / 2; ++q) out.ptr(c, i * RL)[Out::off(1, q)] = v[c][q];
         } else {
             PkDft<RL, +1>::run(v[c]);
             BD_UNROLL
-            for (int q = 0; q < RL; ++q) out.ptr(c, i * RL)[q * Out::step(1)] = v[c][q];
+            for (int q = 0; q < RL; ++q) out.ptr(c, i * RL)[Out::off(1, q)] = v[c][q];
         }
     }
 }
