@@ -54,12 +54,15 @@ def kind_bytes(cfg, info):
     """Algorithmic HBM bytes of each kernel kind over one evaluation: its inputs + outputs once."""
     nx, ny, nz = cfg.nx, cfg.ny, cfg.nz
     N = nx * ny * nz
-    NS = nx + 1
-    w = 8 * 3 * NS * nz * ny                 # x-spectrum W, complex64
-    t = 8 * 3 * NS * nz * 2 * ny             # y-padded scratch T over all chunks
+    sp = info["spectrum_bytes"]              # intermediate spectrum (V tiled / W), complex64
     kst = info["kernel_storage_bytes"]
-    return {"XFwd": 12 * N + w, "Y2D": 2 * w + kst, "YFwd": w + t, "ZFused": 2 * t + kst, "YInv": t + w,
-            "XInv": w + 12 * N}
+    if info["path"] == 2:
+        return {"XFwdT": 12 * N + sp, "YFused": 2 * sp + kst, "XInvT": sp + 12 * N}
+    if info["path"] == 3:
+        return {"XZFwd": 12 * N + sp, "YFused": 2 * sp + kst, "ZXInv": sp + 12 * N}
+    t = 8 * 3 * (nx + 1) * nz * 2 * ny       # y-padded scratch T over all chunks
+    return {"XFwd": 12 * N + sp, "Y2D": 2 * sp + kst, "YFwd": sp + t, "ZFused": 2 * t + kst, "YInv": t + sp,
+            "XInv": sp + 12 * N}
 
 
 def path_flops(cfg):

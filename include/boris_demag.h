@@ -87,6 +87,16 @@ int boris_demag_plan_info(const boris_demag_plan* plan, long long* compulsory_by
                           long long* designed_hbm_bytes, long long* workspace_bytes,
                           int padded[3], int* kernel_launches);
 
+/* Which kernel path the plan uses and how much it stores (harness bookkeeping).
+ * Any out pointer may be NULL.
+ *   path                 = 2: tiled 2-D (XFwdT, YFused, XInvT), 3: tiled 3-D (XZFwd, YFused, ZXInv),
+ *                          0: chunked fallback (XFwd, [Y2D | YFwd, ZFused, YInv per chunk], XInv)
+ *   spectrum_bytes       = bytes of the intermediate spectrum array in HBM (V or W)
+ *   kernel_storage_bytes = bytes of the stored fp32 kernel spectrum (with layout padding)
+ *   cols                 = kx columns per tile of the tiled paths (0 otherwise) */
+int boris_demag_plan_layout(const boris_demag_plan* plan, int* path, long long* spectrum_bytes,
+                            long long* kernel_storage_bytes, int* cols);
+
 /* Copy the plan's kernel spectrum back to the host in natural, symmetry-reduced
  * order: out[c][kz][ky][kx], c in (xx,yy,zz,xy[,xz,yz]), kz <= Pz/2 (1 plane if nz = 1),
  * ky <= Py/2, kx <= Px/2, INCLUDING the folded factor -1/(2 Px Py Pz) (DESIGN.md

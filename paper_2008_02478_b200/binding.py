@@ -48,6 +48,9 @@ def lib():
         L.boris_demag_plan_info.argtypes = [c_vp, ctypes.POINTER(ctypes.c_longlong), ctypes.POINTER(ctypes.c_longlong),
                                             ctypes.POINTER(ctypes.c_longlong), ctypes.POINTER(c_int), ctypes.POINTER(c_int)]
         L.boris_demag_plan_kernel_spectrum.restype = c_int
+        L.boris_demag_plan_layout.restype = c_int
+        L.boris_demag_plan_layout.argtypes = [c_vp, ctypes.POINTER(c_int), ctypes.POINTER(ctypes.c_longlong),
+                                              ctypes.POINTER(ctypes.c_longlong), ctypes.POINTER(c_int)]
         L.boris_demag_plan_kernel_spectrum.argtypes = [c_vp, c_vp]
         L.boris_demag_tensor_host.restype = c_int
         L.boris_demag_tensor_host.argtypes = [c_int, c_int, c_int, c_dbl, c_dbl, c_dbl, c_vp]
@@ -136,7 +139,10 @@ class DemagPlan:
                "boris_demag_apply")
         return H
 
-    KINDS = ("XFwd", "Y2D", "YFwd", "ZFused", "YInv", "XInv")
+    # timing slots of boris_demag_apply_timed, named per kernel path (boris_demag_plan_layout)
+    KINDS = {0: ("XFwd", "Y2D", "YFwd", "ZFused", "YInv", "XInv"),
+             2: ("XFwdT", "YFused", "-", "-", "-", "XInvT"),
+             3: ("XZFwd", "YFused", "-", "-", "-", "ZXInv")}
 
     def apply_timed(self, M, H, stream=None):
         """boris_demag_apply_timed: {kind: (ms, launches)} of one evaluation.  Synchronous."""
@@ -144,7 +150,15 @@ class DemagPlan:
         nl = (ctypes.c_int * 6)()
         _check(lib().boris_demag_apply_timed(self._h, self._ptr(M, "M"), self._ptr(H, "H"), self._stream(stream),
                                              ms, nl), "boris_demag_apply_timed")
-        return {k: (ms[i], nl[i]) for i, k in enumerate(self.KINDS) if nl[i]}
+        return {k: (ms[i], nl[i]) for i, k in enumerate(self.KINDS[self.layout()["path"]]) if nl[i]}
+
+    def layout(self):
+        """boris_demag_plan_layout: kernel path, intermediate spectrum bytes, stored kernel bytes, tile columns."""
+        path, cols = ctypes.c_int(), ctypes.c_int()
+        sb, kb = ctypes.c_longlong(), ctypes.c_longlong()
+        _check(lib().boris_demag_plan_layout(self._h, ctypes.byref(path), ctypes.byref(sb), ctypes.byref(kb),
+                                             ctypes.byref(cols)), "boris_demag_plan_layout")
+        return {"path": path.value, "spectrum_bytes": sb.value, "kernel_storage_bytes": kb.value, "cols": cols.value}
 
     def energy(self, M, H, E=None, stream=None):
         """E (CUDA float64 tensor of 1 element) <- -(mu0/2) dV sum M.H.  Asynchronous."""
@@ -169,10 +183,9 @@ class DemagPlan:
         nl = ctypes.c_int()
         _check(lib().boris_demag_plan_info(self._h, ctypes.byref(comp), ctypes.byref(des), ctypes.byref(ws), padded,
                                            ctypes.byref(nl)), "boris_demag_plan_info")
-        wbytes = 3 * (self.nx + 1) * self.nz * self.ny * 8
+        lay = self.layout()
         return {"compulsory_bytes": comp.value, "designed_hbm_bytes": des.value, "workspace_bytes": ws.value,
-                "padded": tuple(padded), "kernel_launches": nl.value,
-                "kernel_storage_bytes": des.value - 24 * self.nx * self.ny * self.nz - 4 * wbytes}
+                "padded": tuple(padded), "kernel_launches": nl.value, **lay}
 
     def kernel_spectrum(self):
         """Natural reduced fp32 spectrum [ncomp][nzr][nyr][nxr] read back from the device."""

@@ -491,6 +491,19 @@ int boris_demag_plan_info(const boris_demag_plan* p, long long* compulsory_bytes
     return 0;
 }
 
+int boris_demag_plan_layout(const boris_demag_plan* p, int* path, long long* spectrum_bytes,
+                            long long* kernel_storage_bytes, int* cols) {
+    if (!p) return fail(-1, "null plan");
+    const bd::KLayout& kl = p->kl;
+    if (path) *path = p->cfg.tiled ? (p->nz == 1 ? 2 : 3) : 0;
+    if (spectrum_bytes)
+        *spectrum_bytes = p->cfg.tiled ? 3LL * kl.Pz * kl.ntl * p->ny * kl.cols * (long long)sizeof(float2)
+                                       : 3LL * kl.nxr() * p->nz * p->ny * (long long)sizeof(float2);
+    if (kernel_storage_bytes) *kernel_storage_bytes = 4LL * kl.storage_elems();
+    if (cols) *cols = p->cfg.tiled ? kl.cols : 0;
+    return 0;
+}
+
 int boris_demag_plan_kernel_spectrum(const boris_demag_plan* p, float* out_host) {
     if (!p || !out_host) return fail(-1, "null argument");
     const long n = p->kl.reduced_elems();
