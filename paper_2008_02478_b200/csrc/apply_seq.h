@@ -27,6 +27,9 @@ struct LaunchCfg {
 // kx columns per tile of the tiled path: 3 * L * cols complex = 96 KB of shared memory
 // per block at L >= 512 (two blocks per SM)
 BD_HD constexpr int cols_for(int Ly) { return Ly >= 2048 ? 2 : (Ly >= 1024 ? 4 : 8); }
+// 3-D: same rule.  (8-column tiles at Ly = 1024 were measured: the x/z kernels gain 7 % from
+// the 64-byte pieces, YFused loses 17 % with one 512-thread block per SM; profiles/r01_tiled.md)
+BD_HD constexpr int cols_for3d(int Ly) { return cols_for(Ly); }
 constexpr long kMaxDynSmem = 227L * 1024;
 // the 3-D tiled path keeps the nz rows of one (component, y) in shared memory and each
 // z column (2 nz points) in registers
@@ -51,7 +54,7 @@ inline LaunchCfg make_launch_cfg(int nx, int ny, int nz) {
     long cs = (32L << 20) / slot_bytes;
     c.cs = (int)(cs < 1 ? 1 : (cs > nx + 1 ? nx + 1 : cs));
     c.tiled = tiled_supported(nx, ny, nz) ? 1 : 0;
-    c.cols = cols_for(Py);
+    c.cols = nz == 1 ? cols_for(Py) : cols_for3d(Py);
     c.rbt = nx >= 512 ? 8 : 4096 / nx;
     while (c.rbt > ny) c.rbt >>= 1;
     return c;
@@ -165,7 +168,7 @@ int enqueue_tiled_3d(Launcher& run, const PlanView& p, const float* M, float* H)
     const Grid gy{(unsigned)(ntl * Pz), 1};
     rc = dispatch_len(Py, [&](auto ic) {
         constexpr int L = decltype(ic)::value;
-        return run.template run<YFused<L, 6, cols_for(L)>>(gy, ya);
+        return run.template run<YFused<L, 6, cols_for3d(L)>>(gy, ya);
     });
     if (rc) return rc;
     return xz(IC<0>{});

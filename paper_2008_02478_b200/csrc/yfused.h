@@ -306,8 +306,10 @@ template <int L, int NC, int COLS>
 struct YFused {
     using Args = YFArgs;
     static constexpr int KIND = kKindYFused;
-    static constexpr int NT = 256;
-    static constexpr int MINB = 2;
+    // two 256-thread blocks per SM while two tiles fit in shared memory, else one of 512
+    static constexpr bool BIG = 3L * padlen8(L) * COLS * (long)sizeof(float2) > 113L * 1024;
+    static constexpr int NT = BIG ? 512 : 256;
+    static constexpr int MINB = BIG ? 1 : 2;
     static constexpr int NP = dec_np(L);
     static constexpr int NPHASES = 2 * NP - 1;
     static constexpr int RL = dec_rlast(L), F = L / RL, NR = F / 2 + 1;
