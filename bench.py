@@ -341,12 +341,15 @@ def main():
         dist.destroy_process_group()
         return
 
+    # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the ncu --set full
+    # captures summarised in profiles/r01_tiled.md (one capture per workload; None where none was taken)
+    ncu_traffic = {("C5", "YFused"): 618432768 + 356407296, ("C3", "YFused"): 42230784 + 26368}
     kernels = res["kernels"]
     dom = max((k for k in kernels if k != "Energy"), key=lambda k: kernels[k]["ms_per_eval"])
     dk = kernels[dom]
     launches = max(dk["launches_per_eval"], 1)
     roofline = {"kernel": dom, "bound": "hbm", "achieved": dk["gbs"], "peak": peak_gbs, "unit": "GB/s",
-                "frac": dk["gbs"] / peak_gbs, "traffic": None, "peak_source": peak_src,
+                "frac": dk["gbs"] / peak_gbs, "traffic": ncu_traffic.get((cfg.name, dom)), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": dk["algorithmic_bytes"] / launches,
                 "avg_launch_ms": dk["ms_per_eval"] / launches, "launches_per_eval": launches,
                 "share_of_eval": dk["ms_per_eval"] / sum(v["ms_per_eval"] for k, v in kernels.items() if k != "Energy")}

@@ -35,7 +35,7 @@ constexpr long kMaxDynSmem = 227L * 1024;
 // z column (2 nz points) in registers
 inline bool tiled_supported(int nx, int ny, int nz) {
     if (nz == 1) return true;
-    return nz <= 32 && (long)nz * ((prow(nx, nx - 1) + 1) | 1) * (long)sizeof(float2) <= kMaxDynSmem;
+    return nz <= 256 && (long)nz * ((prow(nx, nx) + 1) | 1) * (long)sizeof(float2) <= kMaxDynSmem;
 }
 
 inline LaunchCfg make_launch_cfg(int nx, int ny, int nz) {
@@ -138,7 +138,7 @@ template <class Launcher>
 int enqueue_tiled_3d(Launcher& run, const PlanView& p, const float* M, float* H) {
     const int nx = p.nx, ny = p.ny, nz = p.nz, Py = 2 * ny, Pz = 2 * nz, cols = p.cfg.cols;
     const int ntl = (nx + 1 + cols - 1) / cols;
-    XZArgs xa{M, H, p.V, p.ptw_x, p.xpost, ny, ntl, ilog2c(cols)};
+    XZArgs xa{M, H, p.V, p.ptw_x, p.xpost, ny, ntl, ilog2c(cols), p.tw_z};
     const Grid gx{(unsigned)(3 * ny), 1};
     auto xz = [&](auto fwd) {
         return dispatch_len(nx, [&](auto ic) {
@@ -158,6 +158,9 @@ int enqueue_tiled_3d(Launcher& run, const PlanView& p, const float* M, float* H)
                 case 8: return go(IC<8>{});
                 case 16: return go(IC<16>{});
                 case 32: return go(IC<32>{});
+                case 64: return go(IC<64>{});
+                case 128: return go(IC<128>{});
+                case 256: return go(IC<256>{});
                 default: return -1;
             }
         });
@@ -195,10 +198,7 @@ int enqueue_apply(Launcher& run, const PlanView& p, const float* M, float* H) {
     int rc = dispatch_len(nx, [&](auto ic) { return run.template run<XFwd<decltype(ic)::value>>(gx, xa); });
     if (rc) return rc;
     if (nz == 1) {
-        FusedArgs fa{p.W, p.Kst, p.tw_y, NS, c.nb_y2d, 0, 0, 0, 1};
-        const Grid g{(unsigned)((NS + c.nb_y2d - 1) / c.nb_y2d), 1};
-        rc = dispatch_len(Py, [&](auto ic) { return run.template run<Y2D<decltype(ic)::value>>(g, fa); });
-        if (rc) return rc;
+        return -1;               // 2-D meshes always take the tiled path
     } else {
         const long w_cstride = (long)NS * nz * ny;
         for (int s0 = 0; s0 < NS; s0 += c.cs) {

@@ -29,7 +29,7 @@ BD_HD constexpr int prow(int L, int e) { return e + (e >> 4) + crow(L) * (e >> 7
 template <int L>
 struct SRows {
     float2* p;
-    static constexpr int PITCH = (prow(L, L - 1) + 1) | 1;
+    static constexpr int PITCH = (prow(L, L) + 1) | 1;        // one spare slot after the row (xz.h)
     static BD_HD constexpr int off(int S, int r) { return prow(L, r * S); }
     BD_HD float2* ptr(int row, int e) const { return p + row * PITCH + prow(L, e); }
     static BD_HD float2 ld(const float2* q) { return *q; }

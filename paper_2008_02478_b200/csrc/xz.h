@@ -203,7 +203,23 @@ struct XZArgs {
     int ny;
     int ntl;
     int cs;                // log2(cols)
+    const float2* ztw;     // exp(-2 pi i n / Pz), n < Pz   (columns longer than 64 points)
 };
+
+// Columns of more than 64 points (nz > 32) go through the registers in SP = Pz / 32 passes
+// of 32-point transforms:
+//   forward, pass p:  X[SP k + p] = sum_{z' < 32} W_32^(k z') [ W_Pz^(p z') sum_{m < SP/2} x[z' + 32 m] W_SP^(p m) ]
+//   inverse, pass p:  x[z' + 32 m] += W_SP^(-p m) W_Pz^(-p z') sum_k Y[SP k + p] W_32^(-k z')      (m < SP/2)
+// with the unit roots read from the table ztw (W_SP^(p m) = W_Pz^(32 p m)).  The DC and
+// Nyquist columns of x are then kept as two separate columns (the Nyquist one in the
+// spare slot after each row), because a pass does not hold both members of a mirror pair.
+template <int NZ>
+struct ZSplit {
+    static constexpr bool ON = NZ > 32;
+    static constexpr int SUB = ON ? 32 : NZ, PZ = 2 * NZ, SP = PZ / SUB;
+};
+BD_HD float2 pk_cmul2(float2 a, float2 w) { return pk_cmul(a, make_tw(w)); }
+BD_HD float2 pk_cmulc2(float2 a, float2 w) { return pk_cmulc(a, make_tw(w)); }
 
 // shared position of X[kx] (kx < LX) inside a row, from the xpost table
 BD_HD int xz_pos(const float4* __restrict__ xpost, int LX, int kx) {
@@ -221,6 +237,27 @@ struct XZFwd {
     static constexpr int PZ = 2 * NZ;
     static constexpr int PITCH = SRows<LX>::PITCH;
     static BD_HD long smem_elems(const Args&) { return (long)NZ * PITCH; }
+
+    // pass p of one column (nz > 32, ZSplit): frequencies kz = SP k + p
+    static BD_HD void zpass(const float2* col, float2* out, long kzs, int p, const float2* __restrict__ ztw) {
+        constexpr int SUB = ZSplit<NZ>::SUB, SP = ZSplit<NZ>::SP;
+        float2 v[SUB];
+        BD_UNROLL
+        for (int z = 0; z < SUB; ++z) v[z] = col[z * PITCH];
+        for (int m = 1; m < SP / 2; ++m) {
+            const Tw w = make_tw(BD_LDG(&ztw[(p * m * SUB) & (PZ - 1)]));
+            BD_UNROLL
+            for (int z = 0; z < SUB; ++z) v[z] = pk_add(v[z], pk_cmul(col[(z + SUB * m) * PITCH], w));
+        }
+        if (p != 0) {
+            BD_UNROLL
+            for (int z = 1; z < SUB; ++z) v[z] = pk_cmul2(v[z], BD_LDG(&ztw[p * z]));
+        }
+        PkDft<SUB, -1>::run(v);
+        out += p * kzs;
+        BD_UNROLL
+        for (int k = 0; k < SUB; ++k) { BD_STCG(out, v[k]); out += SP * kzs; }
+    }
 
     // frequencies kz = 2k + PAR of one column; column 0 carries P = X[0] + i X[LX]
     template <int PAR>
@@ -283,7 +320,12 @@ struct XZFwd {
                         const float2 Xk = pk_add(A, T), Xm = bd_f2(A.x - T.x, T.y - A.y);
                         float2* zr = sm + row * PITCH;
                         if (kp == 0) {
-                            zr[bd_float_as_int(xp[u].z)] = bd_f2(Xk.x, Xm.x);
+                            if constexpr (ZSplit<NZ>::ON) {
+                                zr[bd_float_as_int(xp[u].z)] = Xk;
+                                zr[prow(LX, LX)] = Xm;
+                            } else {
+                                zr[bd_float_as_int(xp[u].z)] = bd_f2(Xk.x, Xm.x);
+                            }
                         } else {
                             zr[bd_float_as_int(xp[u].z)] = Xk;
                             if (2 * kp != LX) zr[bd_float_as_int(xp[u].w)] = Xm;
@@ -295,12 +337,22 @@ struct XZFwd {
             const int cols = 1 << a.cs;
             const long kzs = (long)a.ntl * a.ny * cols;                 // elements between kz planes
             float2* vc = a.V + (long)c * PZ * kzs;
-            for (int kx = tid; kx < LX; kx += NT) {
-                const float2* col = sm + xz_pos(a.xpost, LX, kx);
-                float2* out = vc + ((long)((kx >> a.cs) * a.ny + y) << a.cs) + (kx & (cols - 1));
-                float2* outn = vc + ((long)((LX >> a.cs) * a.ny + y) << a.cs) + (LX & (cols - 1));
-                zhalf<0>(col, out, outn, kzs, kx);
-                zhalf<1>(col, out, outn, kzs, kx);
+            if constexpr (ZSplit<NZ>::ON) {
+                constexpr int SP = ZSplit<NZ>::SP;
+                for (int w = tid; w < (LX + 1) * SP; w += NT) {       // one (column, pass) per trip
+                    const int kx = w / SP, p = w - kx * SP;
+                    const float2* col = sm + (kx == LX ? prow(LX, LX) : xz_pos(a.xpost, LX, kx));
+                    float2* out = vc + ((long)((kx >> a.cs) * a.ny + y) << a.cs) + (kx & (cols - 1));
+                    zpass(col, out, kzs, p, a.ztw);
+                }
+            } else {
+                for (int kx = tid; kx < LX; kx += NT) {
+                    const float2* col = sm + xz_pos(a.xpost, LX, kx);
+                    float2* out = vc + ((long)((kx >> a.cs) * a.ny + y) << a.cs) + (kx & (cols - 1));
+                    float2* outn = vc + ((long)((LX >> a.cs) * a.ny + y) << a.cs) + (LX & (cols - 1));
+                    zhalf<0>(col, out, outn, kzs, kx);
+                    zhalf<1>(col, out, outn, kzs, kx);
+                }
             }
         }
     }
@@ -317,6 +369,36 @@ struct ZXInv {
     static constexpr int PZ = 2 * NZ;
     static constexpr int PITCH = SRows<LX>::PITCH;
     static BD_HD long smem_elems(const Args&) { return (long)NZ * PITCH; }
+
+    // all passes of one column (nz > 32, ZSplit)
+    static BD_HD void zcolumn(const float2* in, float2* col, long kzs, const float2* __restrict__ ztw) {
+        constexpr int SUB = ZSplit<NZ>::SUB, SP = ZSplit<NZ>::SP;
+        for (int p = 0; p < SP; ++p) {
+            float2 v[SUB];
+            const float2* ip = in + p * kzs;
+            for (int k = 0; k < SUB; ++k) { v[k] = BD_LDCG(ip); ip += SP * kzs; }
+            PkDft<SUB, +1>::run(v);
+            if (p != 0) {
+                BD_UNROLL
+                for (int z = 1; z < SUB; ++z) v[z] = pk_cmulc2(v[z], BD_LDG(&ztw[p * z]));
+            }
+            if (p == 0) {
+                for (int m = 0; m < SP / 2; ++m) {
+                    BD_UNROLL
+                    for (int z = 0; z < SUB; ++z) col[(z + SUB * m) * PITCH] = v[z];
+                }
+            } else {
+                for (int m = 0; m < SP / 2; ++m) {
+                    const Tw w = make_tw(BD_LDG(&ztw[(p * m * SUB) & (PZ - 1)]));
+                    BD_UNROLL
+                    for (int z = 0; z < SUB; ++z) {
+                        float2* q = col + (z + SUB * m) * PITCH;
+                        *q = pk_add(*q, pk_cmulc(v[z], w));
+                    }
+                }
+            }
+        }
+    }
 
     // frequencies kz = 2k + PAR of one column -> their part of x[z]; the odd half adds to
     // what the even half left in shared memory.  Column 0 carries P^ = Y0^ + i YN^.
@@ -352,12 +434,20 @@ struct ZXInv {
             const int cols = 1 << a.cs;
             const long kzs = (long)a.ntl * a.ny * cols;
             const float2* vc = a.V + (long)c * PZ * kzs;
-            for (int kx = tid; kx < LX; kx += NT) {
-                const float2* in = vc + ((long)((kx >> a.cs) * a.ny + y) << a.cs) + (kx & (cols - 1));
-                const float2* inn = vc + ((long)((LX >> a.cs) * a.ny + y) << a.cs) + (LX & (cols - 1));
-                float2* col = sm + xz_pos(a.xpost, LX, kx);
-                zhalf<0>(in, inn, col, kzs, kx);
-                zhalf<1>(in, inn, col, kzs, kx);
+            if constexpr (ZSplit<NZ>::ON) {
+                for (int kx = tid; kx <= LX; kx += NT) {
+                    const float2* in = vc + ((long)((kx >> a.cs) * a.ny + y) << a.cs) + (kx & (cols - 1));
+                    float2* col = sm + (kx == LX ? prow(LX, LX) : xz_pos(a.xpost, LX, kx));
+                    zcolumn(in, col, kzs, a.ztw);
+                }
+            } else {
+                for (int kx = tid; kx < LX; kx += NT) {
+                    const float2* in = vc + ((long)((kx >> a.cs) * a.ny + y) << a.cs) + (kx & (cols - 1));
+                    const float2* inn = vc + ((long)((LX >> a.cs) * a.ny + y) << a.cs) + (LX & (cols - 1));
+                    float2* col = sm + xz_pos(a.xpost, LX, kx);
+                    zhalf<0>(in, inn, col, kzs, kx);
+                    zhalf<1>(in, inn, col, kzs, kx);
+                }
             }
         } else if constexpr (PH == 1) {
             constexpr int items = (LX / 2 + 1) * NZ;
@@ -380,7 +470,15 @@ struct ZXInv {
                     const int w = w0 + u * NT;
                     if (w < items) {
                         const int kp = w / NZ, row = w % NZ;
-                        if (kp == 0) { Ym[u] = bd_f2(Yk[u].y, 0.f); Yk[u].y = 0.f; }   // P = (Y[0], Y[LX]), both real
+                        if (kp == 0) {
+                            if constexpr (ZSplit<NZ>::ON) {               // Y[0], Y[LX] separate, both real
+                                Ym[u] = bd_f2((sm + row * PITCH)[prow(LX, LX)].x, 0.f);
+                                Yk[u].y = 0.f;
+                            } else {                                      // P = (Y[0], Y[LX]), both real
+                                Ym[u] = bd_f2(Yk[u].y, 0.f);
+                                Yk[u].y = 0.f;
+                            }
+                        }
                         const float2 E = bd_f2(Yk[u].x + Ym[u].x, Yk[u].y - Ym[u].y);
                         const float2 D = bd_f2(Yk[u].x - Ym[u].x, Yk[u].y + Ym[u].y);
                         const float2 O = pk_cmulc(D, make_tw(bd_f2(xp[u].x, xp[u].y)));
