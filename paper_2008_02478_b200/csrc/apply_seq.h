@@ -133,63 +133,72 @@ int enqueue_tiled_2d(Launcher& run, const PlanView& p, const float* M, float* H)
     return dispatch_len(nx, [&](auto ic) { return run.template run<XInvT<decltype(ic)::value, COLS>>(gx, xa); });
 }
 
-// tiled path, nz = 2..32: XZFwd -> YFused -> ZXInv
 template <class Launcher>
-int enqueue_tiled_3d(Launcher& run, const PlanView& p, const float* M, float* H) {
-    const int nx = p.nx, ny = p.ny, nz = p.nz, Py = 2 * ny, Pz = 2 * nz, cols = p.cfg.cols;
+int dispatch_tiled_2d(Launcher& run, const PlanView& p, const float* M, float* H) {
+    switch (p.cfg.cols) {
+        case 2: return enqueue_tiled_2d<2>(run, p, M, H);
+        case 4: return enqueue_tiled_2d<4>(run, p, M, H);
+        case 8: return enqueue_tiled_2d<8>(run, p, M, H);
+        default: return -1;
+    }
+}
+
+// tiled path, nz = 2..256: XZFwd -> YFused -> ZXInv.  The pieces are separate templates so
+// that the CUDA build can put them into translation units of their own (launcher.cuh).
+// x + z transforms of the meshes with NZLO <= nz <= NZHI
+template <int NZLO, int NZHI, class Launcher>
+int enqueue_xz(Launcher& run, const PlanView& p, const float* M, float* H, bool fwd) {
+    const int nx = p.nx, ny = p.ny, nz = p.nz, cols = p.cfg.cols;
     const int ntl = (nx + 1 + cols - 1) / cols;
     XZArgs xa{M, H, p.V, p.ptw_x, p.xpost, ny, ntl, ilog2c(cols), p.tw_z};
     const Grid gx{(unsigned)(3 * ny), 1};
-    auto xz = [&](auto fwd) {
-        return dispatch_len(nx, [&](auto ic) {
-            constexpr int LX = decltype(ic)::value;
-            auto go = [&](auto nzc) {
-                constexpr int NZ = decltype(nzc)::value;
-                if constexpr ((long)NZ * SRows<LX>::PITCH * (long)sizeof(float2) <= kMaxDynSmem && LX <= 1024) {
-                    if constexpr (decltype(fwd)::value) return run.template run<XZFwd<LX, NZ>>(gx, xa);
-                    else return run.template run<ZXInv<LX, NZ>>(gx, xa);
-                } else {
-                    return -1;
-                }
-            };
-            switch (nz) {
-                case 2: return go(IC<2>{});
-                case 4: return go(IC<4>{});
-                case 8: return go(IC<8>{});
-                case 16: return go(IC<16>{});
-                case 32: return go(IC<32>{});
-                case 64: return go(IC<64>{});
-                case 128: return go(IC<128>{});
-                case 256: return go(IC<256>{});
-                default: return -1;
+    return dispatch_len(nx, [&](auto ic) {
+        constexpr int LX = decltype(ic)::value;
+        auto go = [&](auto nzc) {
+            constexpr int NZ = decltype(nzc)::value;
+            if constexpr (NZ >= NZLO && NZ <= NZHI && LX <= 1024 &&
+                          (long)NZ * SRows<LX>::PITCH * (long)sizeof(float2) <= kMaxDynSmem) {
+                if (fwd) return run.template run<XZFwd<LX, NZ>>(gx, xa);
+                return run.template run<ZXInv<LX, NZ>>(gx, xa);
+            } else {
+                return -1;
             }
-        });
-    };
-    int rc = xz(IC<1>{});
-    if (rc) return rc;
+        };
+        switch (nz) {
+            case 2: return go(IC<2>{});
+            case 4: return go(IC<4>{});
+            case 8: return go(IC<8>{});
+            case 16: return go(IC<16>{});
+            case 32: return go(IC<32>{});
+            case 64: return go(IC<64>{});
+            case 128: return go(IC<128>{});
+            case 256: return go(IC<256>{});
+            default: return -1;
+        }
+    });
+}
+
+template <class Launcher>
+int enqueue_yfused3(Launcher& run, const PlanView& p) {
+    const int cols = p.cfg.cols, ntl = (p.nx + 1 + cols - 1) / cols, Py = 2 * p.ny, Pz = 2 * p.nz;
     YFArgs ya{p.V, p.Kst, p.ptw_y, ntl, Pz};
     const Grid gy{(unsigned)(ntl * Pz), 1};
-    rc = dispatch_len(Py, [&](auto ic) {
+    return dispatch_len(Py, [&](auto ic) {
         constexpr int L = decltype(ic)::value;
         return run.template run<YFused<L, 6, cols_for3d(L)>>(gy, ya);
     });
-    if (rc) return rc;
-    return xz(IC<0>{});
 }
 
-// Launcher::run<K>(Grid, const K::Args&) -> 0 on success.
+// Launcher::run<K>(Grid, const K::Args&) -> 0 on success; Launcher::tiled_2d / xz / yfused3
+// forward to dispatch_tiled_2d / enqueue_xz / enqueue_yfused3.
 template <class Launcher>
 int enqueue_apply(Launcher& run, const PlanView& p, const float* M, float* H) {
     if (p.cfg.tiled) {
-        if (p.nz == 1) {
-            switch (p.cfg.cols) {
-                case 2: return enqueue_tiled_2d<2>(run, p, M, H);
-                case 4: return enqueue_tiled_2d<4>(run, p, M, H);
-                case 8: return enqueue_tiled_2d<8>(run, p, M, H);
-                default: return -1;
-            }
-        }
-        return enqueue_tiled_3d(run, p, M, H);
+        if (p.nz == 1) return run.tiled_2d(p, M, H);
+        int rc = run.xz(p, M, H, true);
+        if (!rc) rc = run.yfused3(p);
+        if (!rc) rc = run.xz(p, M, H, false);
+        return rc;
     }
     const int nx = p.nx, ny = p.ny, nz = p.nz, NS = nx + 1, Py = 2 * ny, Pz = 2 * nz;
     const LaunchCfg& c = p.cfg;

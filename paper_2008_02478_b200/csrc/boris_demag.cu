@@ -16,6 +16,7 @@
 #include "../../include/boris_demag.h"
 #include "apply_seq.h"
 #include "kernels.h"
+#include "launcher.cuh"
 #include "khat_layout.h"
 #include "plan_math.h"
 
@@ -37,63 +38,6 @@ int cuda_fail(cudaError_t e, const char* what) {
     } while (0)
 
 bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
-
-// ------------------------------------------------------------------ kernel wrapper
-template <class K, int PH>
-__device__ __forceinline__ void run_phases(const typename K::Args& a, float2* sm) {
-    K::template phase<PH>(threadIdx.x, blockIdx.x, blockIdx.y, a, sm);
-    if constexpr (PH + 1 < K::NPHASES) {
-        __syncthreads();
-        run_phases<K, PH + 1>(a, sm);
-    }
-}
-
-template <class K, class = void>
-struct MinBlocks { static constexpr int value = 1; };
-template <class K>
-struct MinBlocks<K, std::void_t<decltype(K::MINB)>> { static constexpr int value = K::MINB; };
-
-template <class K>
-__global__ void __launch_bounds__(K::NT, MinBlocks<K>::value) phase_kernel(const __grid_constant__ typename K::Args a) {
-    extern __shared__ __align__(16) float2 bd_smem[];
-    run_phases<K, 0>(a, bd_smem);
-}
-
-// CUDA launcher policy of bd::enqueue_apply (apply_seq.h)
-struct TimedLaunch { int kind; cudaEvent_t t0, t1; };
-
-struct CudaLauncher {
-    cudaStream_t st;
-    cudaError_t err = cudaSuccess;
-    std::vector<TimedLaunch>* timed = nullptr;     // boris_demag_apply_timed only
-    template <class K>
-    int run(bd::Grid g, const typename K::Args& a) {
-        if (timed) {
-            TimedLaunch t{K::KIND, nullptr, nullptr};
-            if ((err = cudaEventCreate(&t.t0)) != cudaSuccess) return -2;
-            if ((err = cudaEventCreate(&t.t1)) != cudaSuccess) { cudaEventDestroy(t.t0); return -2; }
-            timed->push_back(t);
-            cudaEventRecord(t.t0, st);
-            const int rc = launch<K>(g, a);
-            cudaEventRecord(t.t1, st);
-            return rc;
-        }
-        return launch<K>(g, a);
-    }
-    template <class K>
-    int launch(bd::Grid g, const typename K::Args& a) {
-        const size_t smem = (size_t)K::smem_elems(a) * sizeof(float2);
-        static size_t opted = 48 * 1024;           // per kernel instantiation
-        if (smem > opted) {
-            err = cudaFuncSetAttribute(phase_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (err != cudaSuccess) return -2;
-            opted = smem;
-        }
-        phase_kernel<K><<<dim3(g.x, g.y), K::NT, smem, st>>>(a);
-        err = cudaGetLastError();
-        return err == cudaSuccess ? 0 : -2;
-    }
-};
 
 // ------------------------------------------------------------------ plan-time kernels (fp64)
 __global__ void k_tensor(double* N, int ncomp, int nx, int ny, int nz, double hx, double hy, double hz) {

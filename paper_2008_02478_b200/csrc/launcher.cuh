@@ -1,0 +1,86 @@
+// launcher.cuh — the __global__ wrapper that runs a kernel struct's phases, and the CUDA
+// launch policy of bd::enqueue_apply (apply_seq.h).  Included by every translation unit of
+// libborisdemag.so; the tiled paths are compiled in units of their own (tu_*.cu) so that
+// the library builds in parallel.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <type_traits>
+#include <vector>
+
+#include "apply_seq.h"
+
+namespace bd {
+
+template <class K, int PH>
+__device__ __forceinline__ void run_phases(const typename K::Args& a, float2* sm) {
+    K::template phase<PH>(threadIdx.x, blockIdx.x, blockIdx.y, a, sm);
+    if constexpr (PH + 1 < K::NPHASES) {
+        __syncthreads();
+        run_phases<K, PH + 1>(a, sm);
+    }
+}
+
+template <class K, class = void>
+struct MinBlocks { static constexpr int value = 1; };
+template <class K>
+struct MinBlocks<K, std::void_t<decltype(K::MINB)>> { static constexpr int value = K::MINB; };
+
+template <class K>
+__global__ void __launch_bounds__(K::NT, MinBlocks<K>::value) phase_kernel(const __grid_constant__ typename K::Args a) {
+    extern __shared__ __align__(16) float2 bd_smem[];
+    run_phases<K, 0>(a, bd_smem);
+}
+
+struct TimedLaunch { int kind; cudaEvent_t t0, t1; };
+
+struct CudaLauncher;
+// parts of the tiled paths, each defined in its own translation unit
+int cu_tiled_2d(CudaLauncher& run, const PlanView& p, const float* M, float* H);          // tu_t2d.cu
+int cu_yfused3(CudaLauncher& run, const PlanView& p);                                     // tu_y3.cu
+int cu_xz_small(CudaLauncher& run, const PlanView& p, const float* M, float* H, bool fwd);  // tu_xz_a.cu  nz 2..16
+int cu_xz_32(CudaLauncher& run, const PlanView& p, const float* M, float* H, bool fwd);     // tu_xz_b.cu  nz 32
+int cu_xz_big(CudaLauncher& run, const PlanView& p, const float* M, float* H, bool fwd);    // tu_xz_c.cu  nz 64..256
+
+struct CudaLauncher {
+    cudaStream_t st;
+    cudaError_t err = cudaSuccess;
+    std::vector<TimedLaunch>* timed = nullptr;     // boris_demag_apply_timed only
+    template <class K>
+    int run(Grid g, const typename K::Args& a) {
+        if (timed) {
+            TimedLaunch t{K::KIND, nullptr, nullptr};
+            if ((err = cudaEventCreate(&t.t0)) != cudaSuccess) return -2;
+            if ((err = cudaEventCreate(&t.t1)) != cudaSuccess) { cudaEventDestroy(t.t0); return -2; }
+            timed->push_back(t);
+            cudaEventRecord(t.t0, st);
+            const int rc = launch<K>(g, a);
+            cudaEventRecord(t.t1, st);
+            return rc;
+        }
+        return launch<K>(g, a);
+    }
+    template <class K>
+    int launch(Grid g, const typename K::Args& a) {
+        const size_t smem = (size_t)K::smem_elems(a) * sizeof(float2);
+        static size_t opted = 48 * 1024;           // per kernel instantiation
+        if (smem > opted) {
+            err = cudaFuncSetAttribute(phase_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (err != cudaSuccess) return -2;
+            opted = smem;
+        }
+        phase_kernel<K><<<dim3(g.x, g.y), K::NT, smem, st>>>(a);
+        err = cudaGetLastError();
+        return err == cudaSuccess ? 0 : -2;
+    }
+    // hooks of enqueue_apply (apply_seq.h)
+    int tiled_2d(const PlanView& p, const float* M, float* H) { return cu_tiled_2d(*this, p, M, H); }
+    int yfused3(const PlanView& p) { return cu_yfused3(*this, p); }
+    int xz(const PlanView& p, const float* M, float* H, bool fwd) {
+        if (p.nz <= 16) return cu_xz_small(*this, p, M, H, fwd);
+        if (p.nz == 32) return cu_xz_32(*this, p, M, H, fwd);
+        return cu_xz_big(*this, p, M, H, fwd);
+    }
+};
+
+}  // namespace bd

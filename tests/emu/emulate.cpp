@@ -36,6 +36,10 @@ struct HostLauncher {
         ++launches;
         return 0;
     }
+    // hooks of enqueue_apply: the emulation keeps everything in this one translation unit
+    int tiled_2d(const bd::PlanView& p, const float* M, float* H) { return bd::dispatch_tiled_2d(*this, p, M, H); }
+    int yfused3(const bd::PlanView& p) { return bd::enqueue_yfused3(*this, p); }
+    int xz(const bd::PlanView& p, const float* M, float* H, bool fwd) { return bd::enqueue_xz<2, 256>(*this, p, M, H, fwd); }
 };
 
 }  // namespace
