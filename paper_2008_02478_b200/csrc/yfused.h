@@ -8,7 +8,7 @@
 // pencils are one contiguous piece of memory:
 //     V[c (3)][kz (Pz)][tile (NTL)][y (ny)][col (COLS)]   complex64,  kx = tile*COLS + col
 // One block = one (kz, tile): 3*COLS pencils of ny -> L = 2 ny points, held in shared
-// memory as S[c][swz(e)][col].  The pencil index e after the forward passes is in the
+// memory as S[c][p(e)][col] (p: padding, below).  The pencil index e after the forward passes is in the
 // digit-reversed order of fft_core.h; the kernel spectrum is stored in the order the
 // multiply meets it (KTile below), real and symmetry-reduced in y and z (pin P12).
 #pragma once
