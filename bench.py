@@ -178,7 +178,7 @@ def time_config(torch, binding, cfg, steps, warmup, flush, peak_gbs, profile_rep
     per_kind = {k: {"ms_per_eval": t / profile_reps, "launches_per_eval": n // profile_reps,
                     "algorithmic_bytes": kb[k], "gbs": kb[k] / (t / profile_reps) / 1e6}
                 for k, (t, n) in kinds.items()}
-    per_kind["Energy"] = {"ms_per_eval": ems / profile_reps, "launches_per_eval": 2,
+    per_kind["Energy"] = {"ms_per_eval": ems / profile_reps, "launches_per_eval": 1,
                           "algorithmic_bytes": 24 * cfg.cells, "gbs": 24 * cfg.cells / (ems / profile_reps) / 1e6}
     ms_step = ms / steps
     res = {"config": cfg.name, "mesh": [cfg.nx, cfg.ny, cfg.nz], "padded": list(info["padded"]),
@@ -186,7 +186,7 @@ def time_config(torch, binding, cfg, steps, warmup, flush, peak_gbs, profile_rep
            "compulsory_bytes": info["compulsory_bytes"], "designed_hbm_bytes": info["designed_hbm_bytes"],
            "hbm_roofline_frac": info["compulsory_bytes"] / (ms_step * 1e-3) / (peak_gbs * 1e9),
            "designed_hbm_passes": info["designed_hbm_bytes"] / info["compulsory_bytes"],
-           "launches_per_step": info["kernel_launches"] + 2, "l2": "flushed between steps" if flush else "inputs > L2",
+           "launches_per_step": info["kernel_launches"] + 1, "l2": "flushed between steps" if flush else "inputs > L2",
            "flops": path_flops(cfg), "kernels": per_kind}
     return res, plan, (M_host, M, H, E)
 

@@ -62,7 +62,8 @@ int boris_demag_apply_timed(boris_demag_plan* plan, const float* M, float* H, vo
 /* E = -(mu0/2) hx hy hz sum_cells M.H  (PAPER.md:L293 relation between field and
  * energy density, integrated; reading R13).  M, H: DEVICE pointers as in
  * apply.  E_dev: DEVICE pointer to one double, written asynchronously on `stream`.
- * Deterministic fixed-shape two-level reduction (warp shuffles, no atomics). */
+ * Deterministic fixed-shape two-level reduction in one launch (warp shuffles; the last block to
+ * finish adds the block sums in index order, so E is bit-identical across calls). */
 int boris_demag_energy(boris_demag_plan* plan, const float* M, const float* H, double* E_dev, void* stream);
 
 /* Same computation with HOST buffers: copies M host->device, applies, computes the

@@ -114,7 +114,8 @@ __device__ __forceinline__ double block_sum(double v, double* sh) {
 }
 
 __global__ void __launch_bounds__(kEnergyThreads) k_energy_partial(const float4* __restrict__ M, const float4* __restrict__ H,
-                                                                    long n4, double* partial) {
+                                                                    long n4, double* partial, unsigned* ticket,
+                                                                    double factor, double* E) {
     __shared__ double sh[32];
     double acc = 0.0;
     const long stride = (long)gridDim.x * blockDim.x;
@@ -133,16 +134,23 @@ __global__ void __launch_bounds__(kEnergyThreads) k_energy_partial(const float4*
         acc += (double)m.x * h.x + (double)m.y * h.y + (double)m.z * h.z + (double)m.w * h.w;
     }
     acc = block_sum(acc, sh);
-    if (threadIdx.x == 0) partial[blockIdx.x] = acc;
+    // second level in the same launch: the block that finishes last adds the partial sums in
+    // index order (the ticket only decides WHO adds, so E is bit-identical across calls)
+    __shared__ bool last;
+    if (threadIdx.x == 0) {
+        partial[blockIdx.x] = acc;
+        __threadfence();
+        last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    double tot = 0.0;
+    for (int i = threadIdx.x; i < (int)gridDim.x; i += blockDim.x) tot += __ldcg(&partial[i]);
+    __syncthreads();                       // sh is reused
+    tot = block_sum(tot, sh);
+    if (threadIdx.x == 0) { *E = factor * tot; *ticket = 0u; }
 }
-__global__ void __launch_bounds__(1024) k_energy_final(const double* partial, int n, double factor, double* E) {
-    __shared__ double sh[32];
-    double acc = 0.0;
-    for (int i = threadIdx.x; i < n; i += blockDim.x) acc += partial[i];
-    acc = block_sum(acc, sh);
-    if (threadIdx.x == 0) *E = factor * acc;
-}
-
 int grid_for(long total, int threads) {
     long g = (total + threads - 1) / threads;
     return (int)(g < 1 ? 1 : (g > 148L * 64 ? 148L * 64 : g));
@@ -168,7 +176,7 @@ struct boris_demag_plan {
     float2* ptw_x = nullptr;         // tiled path: per-pass twiddles of the x / y transforms
     float2* ptw_y = nullptr;
     float4* xpost = nullptr;         // tiled path: fill_xpost table
-    double* partial = nullptr;       // energy partial sums
+    double* partial = nullptr;       // energy partial sums, followed by the ticket counter
     float* stage_M = nullptr;        // apply_host staging
     float* stage_H = nullptr;
     double* stage_E = nullptr;
@@ -337,7 +345,8 @@ boris_demag_plan* boris_demag_plan_create(int nx, int ny, int nz, double hx, dou
         if (!rc) rc = dev_alloc(p, &p->W, (size_t)3 * kl.nxr() * nz * ny);
         if (!rc && nz > 1) rc = dev_alloc(p, &p->T, (size_t)3 * p->cfg.cs * nz * Py);
     }
-    if (!rc) rc = dev_alloc(p, &p->partial, (size_t)kEnergyBlocks);
+    if (!rc) rc = dev_alloc(p, &p->partial, (size_t)kEnergyBlocks + 1);
+    if (!rc && cudaMemset(p->partial, 0, ((size_t)kEnergyBlocks + 1) * sizeof(double)) != cudaSuccess) rc = fail(-2, "cudaMemset");
     if (rc) { std::string keep = g_err; boris_demag_plan_destroy(p); g_err = keep; return nullptr; }
     return p;
 }
@@ -386,9 +395,10 @@ int boris_demag_energy(boris_demag_plan* p, const float* M, const float* H, doub
     cudaStream_t st = (cudaStream_t)stream;
     const long n4 = 3L * p->nx * p->ny * p->nz / 4;
     const double factor = -0.5 * (4e-7 * bd::kPi) * p->hx * p->hy * p->hz;
-    k_energy_partial<<<kEnergyBlocks, kEnergyThreads, 0, st>>>((const float4*)M, (const float4*)H, n4, p->partial);
-    BD_CUDA(cudaGetLastError());
-    k_energy_final<<<1, 1024, 0, st>>>(p->partial, kEnergyBlocks, factor, E_dev);
+    long nblk = (n4 + 4L * kEnergyThreads - 1) / (4L * kEnergyThreads);      // fixed per plan: E stays reproducible
+    nblk = nblk < 1 ? 1 : (nblk > kEnergyBlocks ? kEnergyBlocks : nblk);
+    k_energy_partial<<<(unsigned)nblk, kEnergyThreads, 0, st>>>((const float4*)M, (const float4*)H, n4, p->partial,
+                                                               reinterpret_cast<unsigned*>(p->partial + kEnergyBlocks), factor, E_dev);
     BD_CUDA(cudaGetLastError());
     return 0;
 }

@@ -104,6 +104,8 @@ int emu_freq_of_pos(int L, int p) { return bd::freq_of_pos(L, p); }
 int emu_khat_rows(int L) { return bd::khat_rows(L); }
 int emu_khat_row_of_f(int L, int f) { return bd::khat_row_of_f(L, f); }
 int emu_khat_f_of_row(int L, int r) { return bd::khat_f_of_row(L, r); }
+int emu_slot_to_f(int L, int s) { return bd::slot_to_f(L, s); }
+int emu_f_to_slot(int L, int f) { return bd::f_to_slot(L, f); }
 int emu_dec(int L, int what) { return what < 0 ? bd::dec_np(L) : bd::dec_r(L, what); }
 
 // One forward + inverse pass chain on a single pencil, no multiply: x[0..L/2) -> X (digit

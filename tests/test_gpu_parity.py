@@ -98,6 +98,8 @@ MEDIUM = [
     ((512, 2, 4), (2e-9, 2e-9, 2e-9), "random"),          # Pz = 1024: largest fused z
     ((2, 256, 128), (5e-9, 5e-9, 3e-9), "vortex"),
     ((8, 512, 32), (2e-9, 2e-9, 1e-9), "helix"),          # Py = 1024 as in C5
+    ((256, 4, 16), (2e-9, 2e-9, 2e-9), "random"),         # z columns in 16 passes of 32 points
+    ((32, 16, 1024), (2e-9, 2e-9, 1e-9), "helix"),        # nz rows of nx = 1024 exceed shared memory: chunked fallback
 ]
 
 
@@ -119,6 +121,15 @@ def test_medium_meshes_match_the_fft_oracle(shape, h, texture):
     E_ref = demag_energy(M, H_ref, h)
     assert abs(E - E_ref) <= TOL_E * abs(E_ref)
     plan.close()
+
+
+def test_kernel_path_chosen_per_mesh():
+    expect = {(1, 32, 32): 2, (1, 1024, 1024): 2, (128, 128, 128): 3, (32, 512, 512): 3, (32, 16, 1024): 0, (512, 2, 4): 0}
+    for (nz, ny, nx), path in expect.items():
+        plan = binding.DemagPlan(nx, ny, nz, 2e-9, 2e-9, 1e-9)
+        assert plan.layout()["path"] == path
+        assert plan.info()["kernel_launches"] == (3 if path else plan.info()["kernel_launches"])
+        plan.close()
 
 
 # ----------------------------------------------------------------- the five configs at full size

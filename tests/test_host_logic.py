@@ -121,6 +121,15 @@ def test_pruned_forward_and_truncated_inverse_fft_against_numpy(emu, L):
     assert np.abs(back.view(np.complex64) / L - x).max() < 3e-6
 
 
+def test_kernel_tile_slots_are_a_bijection_onto_the_lower_half(emu):
+    for L in (2, 4, 8, 16, 32, 64, 128, 256, 512, 1024, 2048):
+        RL = emu.emu_dec(L, emu.emu_dec(L, -1) - 1)
+        F = L // RL
+        slots = [emu.emu_f_to_slot(L, f) for f in range(F // 2 + 1)]
+        assert sorted(slots) == list(range(F // 2 + 1))
+        assert all(emu.emu_slot_to_f(L, s) == f for f, s in enumerate(slots))
+
+
 CASES = [
     # (nz, ny, nx), h, texture, cs_override
     ((1, 32, 32), (5.0, 5.0, 3.0), "random", 0),          # config C1 itself
@@ -138,6 +147,10 @@ CASES = [
     ((128, 4, 4), (2.0, 2.0, 2.0), "random", 0),          # Pz = 256 as in C4
     ((512, 2, 4), (2.0, 2.0, 2.0), "random", 0),          # Pz = 1024
     ((32, 512, 4), (2.0, 2.0, 1.0), "helix", 2),          # Py = 1024, Pz = 64 as in C5
+    ((64, 4, 8), (2.0, 2.0, 1.0), "random", 0),           # z columns in 4 passes of 32 points
+    ((256, 2, 4), (2.0, 2.0, 2.0), "random", 0),          # ... in 16 passes
+    ((4, 8, 16), (5.0, 4.0, 3.0), "random", -1),          # chunked fallback kernels forced
+    ((16, 32, 32), (2.0, 2.0, 1.0), "helix", -1),
 ]
 
 
