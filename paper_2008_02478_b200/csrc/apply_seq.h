@@ -22,6 +22,8 @@ struct LaunchCfg {
     int tiled;     // 1: tiled path (xt.h / yfused.h), 0: the kernels of kernels.h
     int cols;      // kx columns per tile
     int rbt;       // rows per block of XFwdT / XInvT
+    int pf_y;      // L2 prefetch distance of YFused in blocks (= blocks resident on the device), 0: off
+    int pf_xz;     // ... of XZFwd
 };
 
 // kx columns per tile of the tiled path: 3 * L * cols complex = 96 KB of shared memory
@@ -57,6 +59,7 @@ inline LaunchCfg make_launch_cfg(int nx, int ny, int nz) {
     c.cols = nz == 1 ? cols_for(Py) : cols_for3d(Py);
     c.rbt = nx >= 512 ? 8 : 4096 / nx;
     while (c.rbt > ny) c.rbt >>= 1;
+    c.pf_y = 0; c.pf_xz = 0;       // set by the plan from the SM count
     return c;
 }
 
@@ -122,7 +125,7 @@ int enqueue_tiled_2d(Launcher& run, const PlanView& p, const float* M, float* H)
     const Grid gx{(unsigned)(3L * ny / p.cfg.rbt), 1};
     int rc = dispatch_len(nx, [&](auto ic) { return run.template run<XFwdT<decltype(ic)::value, COLS>>(gx, xa); });
     if (rc) return rc;
-    YFArgs ya{p.V, p.Kst, p.ptw_y, ntl, 1};
+    YFArgs ya{p.V, p.Kst, p.ptw_y, ntl, 1, p.cfg.pf_y};
     const Grid gy{(unsigned)ntl, 1};
     rc = dispatch_len(Py, [&](auto ic) {
         constexpr int L = decltype(ic)::value;
@@ -150,7 +153,7 @@ template <int NZLO, int NZHI, class Launcher>
 int enqueue_xz(Launcher& run, const PlanView& p, const float* M, float* H, bool fwd) {
     const int nx = p.nx, ny = p.ny, nz = p.nz, cols = p.cfg.cols;
     const int ntl = (nx + 1 + cols - 1) / cols;
-    XZArgs xa{M, H, p.V, p.ptw_x, p.xpost, ny, ntl, ilog2c(cols), p.tw_z};
+    XZArgs xa{M, H, p.V, p.ptw_x, p.xpost, ny, ntl, ilog2c(cols), p.tw_z, p.cfg.pf_xz};
     const Grid gx{(unsigned)(3 * ny), 1};
     return dispatch_len(nx, [&](auto ic) {
         constexpr int LX = decltype(ic)::value;
@@ -181,7 +184,7 @@ int enqueue_xz(Launcher& run, const PlanView& p, const float* M, float* H, bool 
 template <class Launcher>
 int enqueue_yfused3(Launcher& run, const PlanView& p) {
     const int cols = p.cfg.cols, ntl = (p.nx + 1 + cols - 1) / cols, Py = 2 * p.ny, Pz = 2 * p.nz;
-    YFArgs ya{p.V, p.Kst, p.ptw_y, ntl, Pz};
+    YFArgs ya{p.V, p.Kst, p.ptw_y, ntl, Pz, p.cfg.pf_y};
     const Grid gy{(unsigned)(ntl * Pz), 1};
     return dispatch_len(Py, [&](auto ic) {
         constexpr int L = decltype(ic)::value;

@@ -319,6 +319,12 @@ boris_demag_plan* boris_demag_plan_create(int nx, int ny, int nz, double hx, dou
     p->nx = nx; p->ny = ny; p->nz = nz; p->hx = hx; p->hy = hy; p->hz = hz; p->device = dev;
     const int Py = 2 * ny, Pz = nz > 1 ? 2 * nz : 1;
     p->cfg = bd::make_launch_cfg(nx, ny, nz);
+    {
+        int sms = 148;
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        p->cfg.pf_y = 2 * sms;         // YFused: two blocks per SM
+        p->cfg.pf_xz = sms;            // XZFwd: one
+    }
     p->kl = p->cfg.tiled ? bd::make_klayout_tiled(nx, ny, nz, p->cfg.cols) : bd::make_klayout(nx, ny, nz, p->cfg.ty);
     const bd::KLayout& kl = p->kl;
 

@@ -204,6 +204,7 @@ struct XZArgs {
     int ntl;
     int cs;                // log2(cols)
     const float2* ztw;     // exp(-2 pi i n / Pz), n < Pz   (columns longer than 64 points)
+    int pf;                // blocks ahead whose input rows are started towards L2 (0: none; XZFwd)
 };
 
 // Columns of more than 64 points (nz > 32) go through the registers in SP = Pz / 32 passes
@@ -220,6 +221,28 @@ struct ZSplit {
 };
 BD_HD float2 pk_cmul2(float2 a, float2 w) { return pk_cmul(a, make_tw(w)); }
 BD_HD float2 pk_cmulc2(float2 a, float2 w) { return pk_cmulc(a, make_tw(w)); }
+
+// body(kp, row, xp) for kp = 0..LX/2 and row < nrows: a thread keeps kp (and its xpost entry)
+// and walks over rows; kp = LX/2, its own mirror, is taken by one thread per row at the end
+template <int LX, int NT, class Body>
+BD_HD void for_kp_rows(int tid, int nrows, const float4* __restrict__ xpost, Body&& body) {
+    constexpr int HK = LX / 2;
+    if constexpr (HK <= NT) {
+        constexpr int G = NT / HK;
+        const int kp = tid % HK, rg = tid / HK;
+        if (rg < G) {
+            const float4 xp = BD_LDG(&xpost[kp]);
+            for (int row = rg; row < nrows; row += G) body(kp, row, xp);
+        }
+    } else {
+        for (int kp = tid; kp < HK; kp += NT) {
+            const float4 xp = BD_LDG(&xpost[kp]);
+            for (int row = 0; row < nrows; ++row) body(kp, row, xp);
+        }
+    }
+    const float4 xh = BD_LDG(&xpost[HK]);
+    for (int row = tid; row < nrows; row += NT) body(HK, row, xh);
+}
 
 // shared position of X[kx] (kx < LX) inside a row, from the xpost table
 BD_HD int xz_pos(const float4* __restrict__ xpost, int LX, int kx) {
@@ -289,50 +312,39 @@ struct XZFwd {
         SRows<LX> s{sm};
         if constexpr (PH == 0) {
             GRowsIn in{a.M + ((long)c * NZ * a.ny + y) * LX, (long)a.ny * LX};
+            const int nb = bx + a.pf;                      // rows of the block that follows this one on the SM
+            if (a.pf > 0 && nb < 3 * a.ny) {
+                const int cn = nb / a.ny, yn = nb - cn * a.ny;
+                const char* mn = reinterpret_cast<const char*>(a.M + ((long)cn * NZ * a.ny + yn) * LX);
+                constexpr int LPR = LX * 4 / 128 > 0 ? LX * 4 / 128 : 1;         // 128-byte lines per row
+                for (int o = tid; o < NZ * LPR; o += NT)
+                    bd_prefetch_l2(mn + (long)(o / LPR) * a.ny * LX * 4 + (o % LPR) * 128);
+            }
             x_rows_pass<LX, 0, false, NT>(tid, NZ, in, s, a.ptw);
         } else if constexpr (PH < NP) {
             x_rows_pass<LX, PH, false, NT>(tid, NZ, s, s, a.ptw);
         } else if constexpr (PH == NP) {
             // untangle in place: Z[kp], Z[LX-kp] -> X[kp], X[LX-kp]; kp = 0 -> P = (X[0], X[LX])
-            constexpr int items = (LX / 2 + 1) * NZ;
-            for (int w0 = tid; w0 < items; w0 += 4 * NT) {
-                float2 Zk[4], Zm[4];
-                float4 xp[4];
-                BD_UNROLL
-                for (int u = 0; u < 4; ++u) {
-                    const int w = w0 + u * NT;
-                    if (w < items) {
-                        const int kp = w / NZ, row = w % NZ;
-                        xp[u] = BD_LDG(&a.xpost[kp]);
-                        const float2* zr = sm + row * PITCH;
-                        Zk[u] = zr[bd_float_as_int(xp[u].z)];
-                        Zm[u] = zr[bd_float_as_int(xp[u].w)];
+            for_kp_rows<LX, NT>(tid, NZ, a.xpost, [&](int kp, int row, const float4& xp) {
+                float2* zr = sm + row * PITCH;
+                const int pk = bd_float_as_int(xp.z), pm = bd_float_as_int(xp.w);
+                const float2 Zk = zr[pk], Zm = zr[pm];
+                const float2 A = bd_f2(Zk.x + Zm.x, Zk.y - Zm.y);
+                const float2 B = bd_f2(Zk.x - Zm.x, Zk.y + Zm.y);
+                const float2 T = pk_cmul(bd_f2(B.y, -B.x), make_tw(bd_f2(xp.x, xp.y)));
+                const float2 Xk = pk_add(A, T), Xm = bd_f2(A.x - T.x, T.y - A.y);
+                if (kp == 0) {
+                    if constexpr (ZSplit<NZ>::ON) {
+                        zr[pk] = Xk;
+                        zr[prow(LX, LX)] = Xm;
+                    } else {
+                        zr[pk] = bd_f2(Xk.x, Xm.x);
                     }
+                } else {
+                    zr[pk] = Xk;
+                    if (2 * kp != LX) zr[pm] = Xm;
                 }
-                BD_UNROLL
-                for (int u = 0; u < 4; ++u) {
-                    const int w = w0 + u * NT;
-                    if (w < items) {
-                        const int kp = w / NZ, row = w % NZ;
-                        const float2 A = bd_f2(Zk[u].x + Zm[u].x, Zk[u].y - Zm[u].y);
-                        const float2 B = bd_f2(Zk[u].x - Zm[u].x, Zk[u].y + Zm[u].y);
-                        const float2 T = pk_cmul(bd_f2(B.y, -B.x), make_tw(bd_f2(xp[u].x, xp[u].y)));
-                        const float2 Xk = pk_add(A, T), Xm = bd_f2(A.x - T.x, T.y - A.y);
-                        float2* zr = sm + row * PITCH;
-                        if (kp == 0) {
-                            if constexpr (ZSplit<NZ>::ON) {
-                                zr[bd_float_as_int(xp[u].z)] = Xk;
-                                zr[prow(LX, LX)] = Xm;
-                            } else {
-                                zr[bd_float_as_int(xp[u].z)] = bd_f2(Xk.x, Xm.x);
-                            }
-                        } else {
-                            zr[bd_float_as_int(xp[u].z)] = Xk;
-                            if (2 * kp != LX) zr[bd_float_as_int(xp[u].w)] = Xm;
-                        }
-                    }
-                }
-            }
+            });
         } else {
             const int cols = 1 << a.cs;
             const long kzs = (long)a.ntl * a.ny * cols;                 // elements between kz planes
@@ -450,44 +462,25 @@ struct ZXInv {
                 }
             }
         } else if constexpr (PH == 1) {
-            constexpr int items = (LX / 2 + 1) * NZ;
-            for (int w0 = tid; w0 < items; w0 += 4 * NT) {
-                float2 Yk[4], Ym[4];
-                float4 xp[4];
-                BD_UNROLL
-                for (int u = 0; u < 4; ++u) {
-                    const int w = w0 + u * NT;
-                    if (w < items) {
-                        const int kp = w / NZ, row = w % NZ;
-                        xp[u] = BD_LDG(&a.xpost[kp]);
-                        const float2* zr = sm + row * PITCH;
-                        Yk[u] = zr[bd_float_as_int(xp[u].z)];
-                        Ym[u] = zr[bd_float_as_int(xp[u].w)];
+            for_kp_rows<LX, NT>(tid, NZ, a.xpost, [&](int kp, int row, const float4& xp) {
+                float2* zr = sm + row * PITCH;
+                const int pk = bd_float_as_int(xp.z), pm = bd_float_as_int(xp.w);
+                float2 Yk = zr[pk], Ym = zr[pm];
+                if (kp == 0) {
+                    if constexpr (ZSplit<NZ>::ON) {               // Y[0], Y[LX] separate, both real
+                        Ym = bd_f2(zr[prow(LX, LX)].x, 0.f);
+                        Yk.y = 0.f;
+                    } else {                                      // P = (Y[0], Y[LX]), both real
+                        Ym = bd_f2(Yk.y, 0.f);
+                        Yk.y = 0.f;
                     }
                 }
-                BD_UNROLL
-                for (int u = 0; u < 4; ++u) {
-                    const int w = w0 + u * NT;
-                    if (w < items) {
-                        const int kp = w / NZ, row = w % NZ;
-                        if (kp == 0) {
-                            if constexpr (ZSplit<NZ>::ON) {               // Y[0], Y[LX] separate, both real
-                                Ym[u] = bd_f2((sm + row * PITCH)[prow(LX, LX)].x, 0.f);
-                                Yk[u].y = 0.f;
-                            } else {                                      // P = (Y[0], Y[LX]), both real
-                                Ym[u] = bd_f2(Yk[u].y, 0.f);
-                                Yk[u].y = 0.f;
-                            }
-                        }
-                        const float2 E = bd_f2(Yk[u].x + Ym[u].x, Yk[u].y - Ym[u].y);
-                        const float2 D = bd_f2(Yk[u].x - Ym[u].x, Yk[u].y + Ym[u].y);
-                        const float2 O = pk_cmulc(D, make_tw(bd_f2(xp[u].x, xp[u].y)));
-                        float2* zr = sm + row * PITCH;
-                        zr[bd_float_as_int(xp[u].z)] = bd_f2(E.x - O.y, E.y + O.x);
-                        if (kp != 0 && 2 * kp != LX) zr[bd_float_as_int(xp[u].w)] = bd_f2(E.x + O.y, O.x - E.y);
-                    }
-                }
-            }
+                const float2 E = bd_f2(Yk.x + Ym.x, Yk.y - Ym.y);
+                const float2 D = bd_f2(Yk.x - Ym.x, Yk.y + Ym.y);
+                const float2 O = pk_cmulc(D, make_tw(bd_f2(xp.x, xp.y)));
+                zr[pk] = bd_f2(E.x - O.y, E.y + O.x);
+                if (kp != 0 && 2 * kp != LX) zr[pm] = bd_f2(E.x + O.y, O.x - E.y);
+            });
         } else if constexpr (PH <= NP) {
             // phases 2..NP run inverse passes NP-1..1
             x_rows_pass<LX, NP + 1 - PH, true, NT>(tid, NZ, s, s, a.ptw);

@@ -292,6 +292,7 @@ struct YFArgs {
     const float2* ptw;    // per-pass twiddles of length L
     int ntl;              // kx tiles
     int pz;               // padded z length (1 in 2-D mode)
+    int pf;               // blocks ahead whose input tile is started towards L2 (0: none)
 };
 
 // blockIdx.x = o + pz * tile; o enumerates kz so that a plane and its mirror Pz - kz,
@@ -341,6 +342,17 @@ struct YFused {
             constexpr long KB = (long)NR * COLS * NC * RL * sizeof(float);
             const char* kt = reinterpret_cast<const char*>(a.K) + ((long)b.kzr * a.ntl + b.tile) * KB;
             for (long o = (long)tid * 128; o < KB; o += NT * 128) bd_prefetch_l2(kt + o);
+            // ... and the input tile of the block that will follow this one on the SM
+            const int nb = bx + a.pf;
+            if (a.pf > 0 && nb < a.ntl * a.pz) {
+                const Blk n = decode(nb, a);
+                const GTile<COLS> g = gtile(n, 0, a);
+                constexpr long TB = (long)NY * COLS * sizeof(float2);
+                for (long o = (long)tid * 128; o < 3 * TB; o += NT * 128) {
+                    const long c = o / TB;
+                    bd_prefetch_l2(reinterpret_cast<const char*>(g.p + c * g.cstride) + (o - c * TB));
+                }
+            }
         }
         for (int w = tid; w < ITEMS; w += NT) {
             const int col = w % COLS, it = w / COLS;
