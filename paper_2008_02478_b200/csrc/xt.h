@@ -80,6 +80,8 @@ inline void fill_xpost(float4* h, int LX) {
     }
 }
 
+constexpr int XB = 4;     // independent items per trip of the post / pre loops
+
 // all rows of a block through pass P; a thread keeps its butterfly index (and twiddles)
 // and walks over rows
 template <int LX, int P, bool INV, int NT, class In, class Out>
@@ -122,11 +124,11 @@ struct XFwdT {
             const int c = (int)(g0 / a.ny), y0 = (int)(g0 - (long)c * a.ny);
             const int items = (LX / 2 + 1) * a.rb;
             float2* vc = a.V + (long)c * a.ntl * a.ny * COLS;
-            // four independent items per trip: loads first, then arithmetic and stores
-            for (int w0 = tid; w0 < items; w0 += 4 * NT) {
-                float2 Zk[4], Zm[4], tw[4];
+            // XB independent items per trip: loads first, then arithmetic and stores
+            for (int w0 = tid; w0 < items; w0 += XB * NT) {
+                float2 Zk[XB], Zm[XB], tw[XB];
                 BD_UNROLL
-                for (int u = 0; u < 4; ++u) {
+                for (int u = 0; u < XB; ++u) {
                     const int w = w0 + u * NT;
                     if (w < items) {
                         const int kp = w >> a.rbs, row = w & (a.rb - 1);
@@ -138,7 +140,7 @@ struct XFwdT {
                     }
                 }
                 BD_UNROLL
-                for (int u = 0; u < 4; ++u) {
+                for (int u = 0; u < XB; ++u) {
                     const int w = w0 + u * NT;
                     if (w < items) {
                         const int kp = w >> a.rbs, row = w & (a.rb - 1);
@@ -175,11 +177,11 @@ struct XInvT {
             const int c = (int)(g0 / a.ny), y0 = (int)(g0 - (long)c * a.ny);
             const int items = (LX / 2 + 1) * a.rb;
             const float2* vc = a.V + (long)c * a.ntl * a.ny * COLS;
-            for (int w0 = tid; w0 < items; w0 += 4 * NT) {
-                float2 Yk[4], Ym[4];
-                float4 xp[4];
+            for (int w0 = tid; w0 < items; w0 += XB * NT) {
+                float2 Yk[XB], Ym[XB];
+                float4 xp[XB];
                 BD_UNROLL
-                for (int u = 0; u < 4; ++u) {
+                for (int u = 0; u < XB; ++u) {
                     const int w = w0 + u * NT;
                     if (w < items) {
                         const int kp = w >> a.rbs, row = w & (a.rb - 1);
@@ -190,7 +192,7 @@ struct XInvT {
                     }
                 }
                 BD_UNROLL
-                for (int u = 0; u < 4; ++u) {
+                for (int u = 0; u < XB; ++u) {
                     const int w = w0 + u * NT;
                     if (w < items) {
                         const int kp = w >> a.rbs, row = w & (a.rb - 1);
