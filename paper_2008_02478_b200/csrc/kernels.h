@@ -1,5 +1,6 @@
-// kernels.h — the kernels of boris_demag_apply as sequences of barrier-separated
-// phases.  Each kernel is a struct K with
+// kernels.h — the chunked FALLBACK kernels of boris_demag_apply (3-D meshes the tiled
+// path of xt.h / xz.h / yfused.h does not cover: DESIGN.md section 8), as sequences of
+// barrier-separated phases.  Each kernel is a struct K with
 //     K::NT                       threads per block
 //     K::NPHASES                  phases; a __syncthreads() separates consecutive phases
 //     K::smem_elems(args)         float2 elements of dynamic shared memory
@@ -11,7 +12,6 @@
 // Path:            workspace W[3][NS][nz][ny] complex
 //   XFwd   S1  x: zero-pad + real->complex FFT (pruned, half-length complex trick),
 //              written transposed (y fastest) so that y pencils are contiguous
-//   Y2D    S2+S4+S6 (nz = 1): y FFT, tensor multiply, inverse y FFT in one launch
 //   YFwd   S2  (nz > 1) y FFT of a slab of kx slots into the L2-resident scratch T
 //   ZFused S3+S4+S5: z FFT, tensor multiply, inverse z FFT in one launch (the paper's
 //              pipelined kernel), in place on T
@@ -23,7 +23,7 @@
 namespace bd {
 
 // K::KIND numbers the kernels for the per-kernel timing of boris_demag_apply_timed
-constexpr int kNumKinds = 6;   // XFwd, Y2D, YFwd, ZFused, YInv, XInv
+constexpr int kNumKinds = 6;   // timing slots: x forward, fused y (tiled path), YFwd, ZFused, YInv, x inverse
 
 // ------------------------------------------------------------------ accessors
 struct SmemPencil {            // contiguous padded pencils, one buffer per component
@@ -186,83 +186,20 @@ struct XInv {
 };
 
 // ------------------------------------------------------------------ fused kernels (S2+S4+S6 / S3+S4+S5)
-struct KAcc2D {                 // K[slot][c(4)][q(RL)][row]
-    const float* p; int nrows; int rl;
-    BD_HD float get(int c, int q, int row) const { return BD_LDG(&p[((long)c * rl + q) * nrows + row]); }
-};
 struct KAcc3D {                 // K[slot][ytile][c(6)][q(RL)][row][t]
     const float* p; int nrows; int rl; int ty;
     BD_HD float get(int c, int q, int row) const { return BD_LDG(&p[(((long)c * rl + q) * nrows + row) * ty]); }
 };
 
 struct FusedArgs {
-    float2* D;             // Y2D: W [3][NS][ny];  ZFused: T [3][CS][nz][Py]
+    float2* D;             // T [3][CS][nz][Py]
     const float* K;        // kernel spectrum in fused-pass order
     const float2* tw;      // exp(-2 pi i k / L)
-    int npencils;          // Y2D: NS
-    int nb;                // Y2D: pencils (kx slots) per block
+    int npencils;          // unused
+    int nb;                // unused
     int py;                // ZFused: padded y length (pencil stride)
     int cs, s0;            // ZFused: slots in this chunk, first global slot
     int ty;                // ZFused: pencils per block (power of two, divides py)
-};
-
-// nz = 1: one block = nb kx slots x 3 components, pencils along y are contiguous.
-template <int L>
-struct Y2D {
-    using Args = FusedArgs;
-    static constexpr int KIND = 1;
-    static constexpr int NT = 128;
-    static constexpr int NP = dec_np(L);
-    static constexpr int NPHASES = 2 * NP - 1;
-    static constexpr int RL = dec_rlast(L);
-    static constexpr int PL = padlen(L);
-    static BD_HD long smem_elems(const Args& a) { return NP == 1 ? 0 : (long)a.nb * 3 * PL; }
-
-    template <int P, bool INV>
-    static BD_HD void pass(int tid, int bx, const Args& a, float2* sm) {
-        constexpr int IPP = L / dec_r(L, P);
-        const int items = a.nb * 3 * IPP;
-        const long cstride = (long)a.npencils * (L / 2);
-        for (int w = tid; w < items; w += NT) {
-            const int pc = w / IPP, it = w - pc * IPP;
-            const int pb = pc / 3, c = pc - pb * 3;
-            const int slot = bx * a.nb + pb;
-            if (slot >= a.npencils) continue;
-            SmemPencil s{sm + (long)pb * 3 * PL, PL};
-            GlobalPencil g{a.D + (long)slot * (L / 2), cstride, 1};
-            if constexpr (P == 0 && !INV) fwd_pass<L, 0>(c, it, g, s, a.tw);
-            else if constexpr (P == 0) inv_pass<L, 0>(c, it, s, g, a.tw);
-            else if constexpr (!INV) fwd_pass<L, P>(c, it, s, s, a.tw);
-            else inv_pass<L, P>(c, it, s, s, a.tw);
-        }
-    }
-
-    static BD_HD void mid(int tid, int bx, const Args& a, float2* sm) {
-        constexpr int F = dec_items(L);
-        const int items = a.nb * F;
-        const int nrows = khat_rows(L);
-        const long cstride = (long)a.npencils * (L / 2);
-        for (int w = tid; w < items; w += NT) {
-            const int pb = w / F, i = w - pb * F;
-            const int slot = bx * a.nb + pb;
-            if (slot >= a.npencils) continue;
-            KAcc2D K{a.K + (long)slot * 4 * RL * nrows, nrows, RL};
-            if constexpr (NP == 1) {
-                GlobalPencil g{a.D + (long)slot * (L / 2), cstride, 1};
-                fused_mid<L, 4>(i, g, g, K);
-            } else {
-                SmemPencil s{sm + (long)pb * 3 * PL, PL};
-                fused_mid<L, 4>(i, s, s, K);
-            }
-        }
-    }
-
-    template <int PH>
-    static BD_HD void phase(int tid, int bx, int by, const Args& a, float2* sm) {
-        if constexpr (PH < NP - 1) pass<PH, false>(tid, bx, a, sm);
-        else if constexpr (PH == NP - 1) mid(tid, bx, a, sm);
-        else pass<2 * NP - 2 - PH, true>(tid, bx, a, sm);
-    }
 };
 
 // nz > 1: one block = ty adjacent y positions x 3 components of one kx slot; pencils

@@ -5,10 +5,11 @@
 // with the value at a mirrored frequency Py - ky (Pz - kz) equal to the stored one
 // times -1 for the components odd in y (z).  kx needs no mirror (real -> complex in x).
 //
-// Device storage (fp32), in the order the fused kernels meet it (fft_core.h khat_*):
-//   nz == 1 (Y2D, fused dimension y):
-//       K[slot = kx][c (4)][q (RL)][row]                       row = canonical y item
-//   nz  > 1 (ZFused, fused dimension z; y is a plain tile coordinate and keeps all Py
+// Device storage (fp32), in the order the fused kernels meet it:
+//   tiled path (YFused, fused dimension y; yfused.h "kernel-spectrum tile"):
+//       K[kzr][tile][c][chunk][slot][col][CH]
+//   chunked fallback, nz > 1 (ZFused, fused dimension z, fft_core.h khat_*; y is a plain
+//            tile coordinate and keeps all Py
 //            positions of the in-place y FFT, in its digit-reversed order):
 //       K[slot = kx][ytile][c (6)][q (RL)][row][t]             py = ytile*ty + t
 // The entry (q, row) of the fused dimension holds frequency k = f'(row) + F*q; if
@@ -27,7 +28,7 @@ struct KLayout {
     int Lf;                // fused FFT length: Py (nz = 1) or Pz
     int RL, nrows;         // last radix and canonical rows of the fused dimension
     int ty, ntiles;        // y tile of ZFused (ty = ntiles = 1... for nz = 1: ty = 1, ntiles = 1)
-    // tiled path (yfused.h): K[kzr][tile][row (NR)][col][c][q (RLy)], fused dimension y
+    // tiled path (yfused.h): K[kzr][tile][c][chunk][slot (NRy)][col][CH], fused dimension y
     int tiled;             // 1: tiled layout below, 0: the layouts above
     int cols, ntl;         // kx columns per tile, tiles
     int RLy, Fy, NRy;      // last radix of the y transform, its items, stored rows Fy/2 + 1

@@ -10,7 +10,7 @@
 // One block = one (kz, tile): 3*COLS pencils of ny -> L = 2 ny points, held in shared
 // memory as S[c][p(e)][col] (p: padding, below).  The pencil index e after the forward passes is in the
 // digit-reversed order of fft_core.h; the kernel spectrum is stored in the order the
-// multiply meets it (KTile below), real and symmetry-reduced in y and z (pin P12).
+// multiply meets it (kernel-spectrum tile below), real and symmetry-reduced in y and z (pin P12).
 #pragma once
 #include <cmath>
 
@@ -274,15 +274,6 @@ BD_HD void mid3(int i, const float* __restrict__ kslot, int cstride, const In& i
             for (int q = 0; q < RL; ++q) out.ptr(c, i * RL)[Out::off(1, q)] = v[c][q];
         }
     }
-}
-
-// item of the last pass whose frequency offset is f (inverse of item_partial_freq)
-BD_HD int item_of_partial_freq(int L, int f) {
-    const int np = dec_np(L);
-    if (np == 1) return 0;
-    if (np == 2) return f;
-    const int r0 = dec_r(L, 0), r1 = dec_r(L, 1);
-    return (f % r0) * r1 + f / r0;
 }
 
 // ------------------------------------------------------------------ YFused (S2+S4+S6)
