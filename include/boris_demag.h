@@ -66,6 +66,14 @@ int boris_demag_apply_timed(boris_demag_plan* plan, const float* M, float* H, vo
  * finish adds the block sums in index order, so E is bit-identical across calls). */
 int boris_demag_energy(boris_demag_plan* plan, const float* M, const float* H, double* E_dev, void* stream);
 
+/* boris_demag_apply followed by boris_demag_energy in one enqueue: H = -N * M and
+ * E = -(mu0/2) hx hy hz sum(M.H) (north_star).  On the tiled kernel paths the
+ * sum is gathered by the kernel that writes H (fp64 per-block sums, added in block order by the
+ * block that finishes last: bit-identical across calls), so M and H are not read again; other
+ * meshes run the two calls back to back.  Arguments, layout, aliasing and error codes as for
+ * boris_demag_apply and boris_demag_energy; E_dev is a DEVICE double. */
+int boris_demag_apply_energy(boris_demag_plan* plan, const float* M, float* H, double* E_dev, void* stream);
+
 /* Same computation with HOST buffers: copies M host->device, applies, computes the
  * energy, copies H (and E if E_host != NULL) device->host and synchronises `stream`.
  * M_host, H_host: host pointers, fp32 [3][nz][ny][nx] (pinned memory makes the

@@ -40,6 +40,8 @@ def lib():
                                               ctypes.POINTER(c_int)]
         L.boris_demag_energy.restype = c_int
         L.boris_demag_energy.argtypes = [c_vp, c_vp, c_vp, c_vp, c_vp]
+        L.boris_demag_apply_energy.restype = c_int
+        L.boris_demag_apply_energy.argtypes = [c_vp, c_vp, c_vp, c_vp, c_vp]
         L.boris_demag_apply_host.restype = c_int
         L.boris_demag_apply_host.argtypes = [c_vp, c_vp, c_vp, c_vp, c_vp]
         L.boris_demag_last_error.restype = ctypes.c_char_p
@@ -167,6 +169,15 @@ class DemagPlan:
             E = torch.empty(1, dtype=torch.float64, device=M.device)
         _check(lib().boris_demag_energy(self._h, self._ptr(M, "M"), self._ptr(H, "H"), E.data_ptr(),
                                         self._stream(stream)), "boris_demag_energy")
+        return E
+
+    def apply_energy(self, M, H, E=None, stream=None):
+        """boris_demag_apply_energy: H <- -N * M and E <- -(mu0/2) dV sum M.H in one enqueue.  Asynchronous."""
+        import torch
+        if E is None:
+            E = torch.empty(1, dtype=torch.float64, device=M.device)
+        _check(lib().boris_demag_apply_energy(self._h, self._ptr(M, "M"), self._ptr(H, "H"), E.data_ptr(),
+                                              self._stream(stream)), "boris_demag_apply_energy")
         return E
 
     def apply_host(self, M_host, H_host, want_energy=True, stream=None):

@@ -88,6 +88,7 @@ struct PlanView {
     const float2 *ptw_x = nullptr, *ptw_y = nullptr;   // per-pass twiddles (tiled path)
     float2* V = nullptr;                               // tiled spectrum (tiled path)
     const float4* xpost = nullptr;                     // fill_xpost table (tiled path)
+    EnergyArgs en = {nullptr, nullptr, nullptr, nullptr, 0.0};   // energy fused into the last kernel (tiled path)
 };
 
 template <int L> struct IC { static constexpr int value = L; };
@@ -121,7 +122,7 @@ template <int COLS, class Launcher>
 int enqueue_tiled_2d(Launcher& run, const PlanView& p, const float* M, float* H) {
     const int nx = p.nx, ny = p.ny, Py = 2 * ny;
     const int ntl = (nx + 1 + COLS - 1) / COLS;
-    XTArgs xa{M, H, p.V, p.ptw_x, p.xpost, ny, ntl, p.cfg.rbt, ilog2c(p.cfg.rbt)};
+    XTArgs xa{M, H, p.V, p.ptw_x, p.xpost, ny, ntl, p.cfg.rbt, ilog2c(p.cfg.rbt), p.en};
     const Grid gx{(unsigned)(3L * ny / p.cfg.rbt), 1};
     int rc = dispatch_len(nx, [&](auto ic) { return run.template run<XFwdT<decltype(ic)::value, COLS>>(gx, xa); });
     if (rc) return rc;
@@ -153,7 +154,7 @@ template <int NZLO, int NZHI, class Launcher>
 int enqueue_xz(Launcher& run, const PlanView& p, const float* M, float* H, bool fwd) {
     const int nx = p.nx, ny = p.ny, nz = p.nz, cols = p.cfg.cols;
     const int ntl = (nx + 1 + cols - 1) / cols;
-    XZArgs xa{M, H, p.V, p.ptw_x, p.xpost, ny, ntl, ilog2c(cols), p.tw_z, p.cfg.pf_xz};
+    XZArgs xa{M, H, p.V, p.ptw_x, p.xpost, ny, ntl, ilog2c(cols), p.tw_z, p.cfg.pf_xz, p.en};
     const Grid gx{(unsigned)(3 * ny), 1};
     return dispatch_len(nx, [&](auto ic) {
         constexpr int LX = decltype(ic)::value;

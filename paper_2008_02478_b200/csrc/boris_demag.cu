@@ -97,6 +97,7 @@ __global__ void k_gather_natural(const float* Kst, KLayout kl, float* out) {
 
 // ------------------------------------------------------------------ energy (S8)
 constexpr int kEnergyBlocks = 592, kEnergyThreads = 256;
+constexpr int kFusedEnergySlots = 3 * 1024;      // blocks of XInvT (3 ny / rb) or ZXInv (3 ny), ny <= 1024
 
 __device__ __forceinline__ double warp_sum(double v) {
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -177,6 +178,7 @@ struct boris_demag_plan {
     float2* ptw_y = nullptr;
     float4* xpost = nullptr;         // tiled path: fill_xpost table
     double* partial = nullptr;       // energy partial sums, followed by the ticket counter
+    double* partial_f = nullptr;     // fused energy (apply_energy): one slot per block of the last kernel + ticket
     float* stage_M = nullptr;        // apply_host staging
     float* stage_H = nullptr;
     double* stage_E = nullptr;
@@ -302,7 +304,7 @@ const char* boris_demag_last_error(void) { return g_err.c_str(); }
 void boris_demag_plan_destroy(boris_demag_plan* p) {
     if (!p) return;
     cudaFree(p->Kst); cudaFree(p->tw_x); cudaFree(p->tw_xpost); cudaFree(p->tw_y); cudaFree(p->tw_z);
-    cudaFree(p->W); cudaFree(p->T); cudaFree(p->partial);
+    cudaFree(p->W); cudaFree(p->T); cudaFree(p->partial); cudaFree(p->partial_f);
     cudaFree(p->V); cudaFree(p->ptw_x); cudaFree(p->ptw_y); cudaFree(p->xpost);
     cudaFree(p->stage_M); cudaFree(p->stage_H); cudaFree(p->stage_E);
     delete p;
@@ -353,6 +355,8 @@ boris_demag_plan* boris_demag_plan_create(int nx, int ny, int nz, double hx, dou
     }
     if (!rc) rc = dev_alloc(p, &p->partial, (size_t)kEnergyBlocks + 1);
     if (!rc && cudaMemset(p->partial, 0, ((size_t)kEnergyBlocks + 1) * sizeof(double)) != cudaSuccess) rc = fail(-2, "cudaMemset");
+    if (!rc) rc = dev_alloc(p, &p->partial_f, (size_t)kFusedEnergySlots + 1);
+    if (!rc && cudaMemset(p->partial_f, 0, ((size_t)kFusedEnergySlots + 1) * sizeof(double)) != cudaSuccess) rc = fail(-2, "cudaMemset");
     if (rc) { std::string keep = g_err; boris_demag_plan_destroy(p); g_err = keep; return nullptr; }
     return p;
 }
@@ -363,6 +367,24 @@ int boris_demag_apply(boris_demag_plan* p, const float* M, float* H, void* strea
     if (((uintptr_t)M | (uintptr_t)H) & 15) return fail(-1, "M and H must be 16-byte aligned");
     CudaLauncher run{(cudaStream_t)stream};
     const bd::PlanView pv = plan_view(p);
+    const int rc = bd::enqueue_apply(run, pv, M, H);
+    if (rc == -2) return cuda_fail(run.err, "kernel launch");
+    if (rc) return fail(rc, "unsupported size");
+    return 0;
+}
+
+int boris_demag_apply_energy(boris_demag_plan* p, const float* M, float* H, double* E_dev, void* stream) {
+    if (!p || !M || !H || !E_dev) return fail(-1, "null argument");
+    if (M == H) return fail(-1, "M and H must not alias");
+    if (((uintptr_t)M | (uintptr_t)H) & 15) return fail(-1, "M and H must be 16-byte aligned");
+    if (!p->cfg.tiled) {
+        if (int rc = boris_demag_apply(p, M, H, stream)) return rc;
+        return boris_demag_energy(p, M, H, E_dev, stream);
+    }
+    CudaLauncher run{(cudaStream_t)stream};
+    bd::PlanView pv = plan_view(p);
+    pv.en = bd::EnergyArgs{M, p->partial_f, reinterpret_cast<unsigned*>(p->partial_f + kFusedEnergySlots), E_dev,
+                           -0.5 * (4e-7 * bd::kPi) * p->hx * p->hy * p->hz};
     const int rc = bd::enqueue_apply(run, pv, M, H);
     if (rc == -2) return cuda_fail(run.err, "kernel launch");
     if (rc) return fail(rc, "unsupported size");
@@ -419,10 +441,11 @@ int boris_demag_apply_host(boris_demag_plan* p, const float* M_host, float* H_ho
         if (int rc = dev_alloc(p, &p->stage_E, 1)) return rc;
     }
     BD_CUDA(cudaMemcpyAsync(p->stage_M, M_host, n * sizeof(float), cudaMemcpyHostToDevice, st));
-    if (int rc = boris_demag_apply(p, p->stage_M, p->stage_H, stream)) return rc;
     if (E_host) {
-        if (int rc = boris_demag_energy(p, p->stage_M, p->stage_H, p->stage_E, stream)) return rc;
+        if (int rc = boris_demag_apply_energy(p, p->stage_M, p->stage_H, p->stage_E, stream)) return rc;
         BD_CUDA(cudaMemcpyAsync(E_host, p->stage_E, sizeof(double), cudaMemcpyDeviceToHost, st));
+    } else {
+        if (int rc = boris_demag_apply(p, p->stage_M, p->stage_H, stream)) return rc;
     }
     BD_CUDA(cudaMemcpyAsync(H_host, p->stage_H, n * sizeof(float), cudaMemcpyDeviceToHost, st));
     BD_CUDA(cudaStreamSynchronize(st));

@@ -33,6 +33,7 @@ struct SRows {
     static BD_HD constexpr int off(int S, int r) { return prow(L, r * S); }
     BD_HD float2* ptr(int row, int e) const { return p + row * PITCH + prow(L, e); }
     static BD_HD float2 ld(const float2* q) { return *q; }
+    BD_HD void st(float2* q, float2 v) const { *q = v; }
 };
 struct GRowsIn {               // rows of a real array read as (x[2m], x[2m+1]) pairs
     const float* p; long pitch;
@@ -44,7 +45,66 @@ struct GRowsOut {
     float* p; long pitch;
     static BD_HD constexpr int off(int S, int r) { return r * S; }
     BD_HD float2* ptr(int row, int e) const { return reinterpret_cast<float2*>(p + row * pitch) + e; }
+    BD_HD void st(float2* q, float2 v) const { *q = v; }
 };
+// H rows written, and sum M.H gathered on the way (S8 fused into S7): M has H's layout, so
+// the matching M pair sits at a fixed byte distance from the H pair
+struct GRowsOutE {
+    float* p; long pitch; long m_minus_h; double* acc;
+    static BD_HD constexpr int off(int S, int r) { return r * S; }
+    BD_HD float2* ptr(int row, int e) const { return reinterpret_cast<float2*>(p + row * pitch) + e; }
+    BD_HD void st(float2* q, float2 v) const {
+        *q = v;
+        const float2 m = BD_LDCG(reinterpret_cast<const float2*>(reinterpret_cast<const char*>(q) + m_minus_h));
+        *acc += (double)m.x * v.x + (double)m.y * v.y;
+    }
+};
+
+// Energy fused into the last kernel of an evaluation (boris_demag_apply_energy): every block
+// leaves sum M.H of its rows in partial[block]; the block that finishes last adds them in
+// index order (the ticket decides who adds, not what: E is bit-identical across calls).
+struct EnergyArgs {
+    const float* M;        // nullptr: no energy
+    double* partial;       // one slot per block
+    unsigned* ticket;
+    double* E;             // device scalar
+    double factor;         // -(mu0/2) hx hy hz
+};
+BD_HD void energy_finish(double acc, const EnergyArgs& en) {
+#if defined(__CUDA_ARCH__)
+    __shared__ double sh[32];
+    __shared__ bool last;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) sh[wid] = acc;
+    __syncthreads();
+    if (wid == 0) {
+        double v = lane < nw ? sh[lane] : 0.0;
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) {
+            en.partial[blockIdx.x] = v;
+            __threadfence();
+            last = atomicAdd(en.ticket, 1u) == gridDim.x - 1;
+        }
+    }
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    double tot = 0.0;
+    for (int i = threadIdx.x; i < (int)gridDim.x; i += blockDim.x) tot += __ldcg(&en.partial[i]);
+    for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
+    __syncthreads();
+    if (lane == 0) sh[wid] = tot;
+    __syncthreads();
+    if (wid == 0) {
+        double v = lane < nw ? sh[lane] : 0.0;
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) { *en.E = en.factor * v; *en.ticket = 0u; }
+    }
+#else
+    (void)acc; (void)en;       // the host emulation checks H only
+#endif
+}
 
 struct XTArgs {
     const float* M;        // [3][ny][nx]
@@ -57,6 +117,7 @@ struct XTArgs {
     int ntl;
     int rb;                // rows (consecutive y of one component) per block; a power of two dividing ny
     int rbs;               // log2(rb)
+    EnergyArgs en;         // XInvT: energy gathered while H is written (en.M == nullptr: off)
 };
 
 BD_HD int bd_float_as_int(float f) {
@@ -210,8 +271,15 @@ struct XInvT {
         } else if constexpr (PH < NP) {
             x_rows_pass<LX, NP - PH, true, NT>(tid, a.rb, s, s, a.ptw);
         } else {
-            GRowsOut out{a.H + g0 * LX, LX};
-            x_rows_pass<LX, 0, true, NT>(tid, a.rb, s, out, a.ptw);
+            if (a.en.M) {
+                double acc = 0.0;
+                GRowsOutE out{a.H + g0 * LX, LX, (long)((const char*)a.en.M - (const char*)a.H), &acc};
+                x_rows_pass<LX, 0, true, NT>(tid, a.rb, s, out, a.ptw);
+                energy_finish(acc, a.en);
+            } else {
+                GRowsOut out{a.H + g0 * LX, LX};
+                x_rows_pass<LX, 0, true, NT>(tid, a.rb, s, out, a.ptw);
+            }
         }
     }
 };

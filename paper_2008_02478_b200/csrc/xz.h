@@ -205,6 +205,7 @@ struct XZArgs {
     int cs;                // log2(cols)
     const float2* ztw;     // exp(-2 pi i n / Pz), n < Pz   (columns longer than 64 points)
     int pf;                // blocks ahead whose input rows are started towards L2 (0: none; XZFwd)
+    EnergyArgs en;         // ZXInv: energy gathered while H is written (en.M == nullptr: off)
 };
 
 // Columns of more than 64 points (nz > 32) go through the registers in SP = Pz / 32 passes
@@ -485,8 +486,16 @@ struct ZXInv {
             // phases 2..NP run inverse passes NP-1..1
             x_rows_pass<LX, NP + 1 - PH, true, NT>(tid, NZ, s, s, a.ptw);
         } else {
-            GRowsOut out{a.H + ((long)c * NZ * a.ny + y) * LX, (long)a.ny * LX};
-            x_rows_pass<LX, 0, true, NT>(tid, NZ, s, out, a.ptw);
+            if (a.en.M) {
+                double acc = 0.0;
+                GRowsOutE out{a.H + ((long)c * NZ * a.ny + y) * LX, (long)a.ny * LX,
+                              (long)((const char*)a.en.M - (const char*)a.H), &acc};
+                x_rows_pass<LX, 0, true, NT>(tid, NZ, s, out, a.ptw);
+                energy_finish(acc, a.en);
+            } else {
+                GRowsOut out{a.H + ((long)c * NZ * a.ny + y) * LX, (long)a.ny * LX};
+                x_rows_pass<LX, 0, true, NT>(tid, NZ, s, out, a.ptw);
+            }
         }
     }
 };

@@ -75,6 +75,7 @@ struct STile {                 // shared: S[c][p(e)][col]
     static BD_HD constexpr int off(int S, int r) { return r * pstep(S) * COLS; }
     BD_HD float2* ptr(int c, int e) const { return p + c * CP + pidx(e) * COLS; }
     static BD_HD float2 ld(const float2* q) { return *q; }
+    BD_HD void st(float2* q, float2 v) const { *q = v; }
 };
 template <int COLS>
 struct GTile {                 // global: V tile [y][col], component stride cstride
@@ -82,6 +83,7 @@ struct GTile {                 // global: V tile [y][col], component stride cstr
     static BD_HD constexpr int off(int S, int r) { return r * S * COLS; }
     BD_HD float2* ptr(int c, int e) const { return p + c * cstride + (long)e * COLS; }
     static BD_HD float2 ld(const float2* q) { return BD_LDCG(q); }     // streamed once: keep it out of L1
+    BD_HD void st(float2* q, float2 v) const { *q = v; }
 };
 
 // ------------------------------------------------------------------ passes
@@ -122,7 +124,7 @@ BD_HD void fwd_passM(int it, int c0, int cstep, int cend, const In& in, const Ou
         }
         float2* po = out.ptr(c, base);
         BD_UNROLL
-        for (int q = 0; q < R; ++q) po[Out::off(S, q)] = v[q];
+        for (int q = 0; q < R; ++q) out.st(po + Out::off(S, q), v[q]);
     }
 }
 
@@ -159,11 +161,11 @@ BD_HD void inv_passM(int it, int c0, int cstep, int cend, const In& in, const Ou
         if constexpr (P == 0) {
             PkDftTrunc<R, +1>::run(v);
             BD_UNROLL
-            for (int r = 0; r < R / 2; ++r) po[Out::off(S, r)] = v[r];
+            for (int r = 0; r < R / 2; ++r) out.st(po + Out::off(S, r), v[r]);
         } else {
             PkDft<R, +1>::run(v);
             BD_UNROLL
-            for (int r = 0; r < R; ++r) po[Out::off(S, r)] = v[r];
+            for (int r = 0; r < R; ++r) out.st(po + Out::off(S, r), v[r]);
         }
     }
 }

@@ -123,6 +123,27 @@ def test_medium_meshes_match_the_fft_oracle(shape, h, texture):
     plan.close()
 
 
+@pytest.mark.parametrize("shape", [(1, 64, 128), (1, 1024, 16), (8, 32, 64), (64, 16, 32), (512, 2, 4)])
+def test_fused_apply_energy_matches_the_two_calls_and_is_reproducible(shape):
+    nz, ny, nx = shape
+    h = (2e-9, 3e-9, 1e-9)
+    M_host = W.make_texture("random", shape, 8e5, seed=31)
+    plan = binding.DemagPlan(nx, ny, nz, *h)
+    M = torch.from_numpy(M_host).cuda()
+    H1, H2 = torch.empty_like(M), torch.full_like(M, float("nan"))
+    plan.apply(M, H1)
+    E1 = plan.energy(M, H1)
+    E2 = plan.apply_energy(M, H2)
+    E3 = plan.apply_energy(M, H2).clone()
+    torch.cuda.synchronize()
+    assert torch.equal(H1, H2)                                   # same kernels, same bits
+    assert E2.item() == E3.item()                                # fixed summation order
+    assert abs(E2.item() - E1.item()) <= 1e-12 * abs(E1.item())  # both fp64 sums of the same products
+    E_ref = demag_energy(M_host, demag_fft(M_host, h), h)
+    assert abs(E2.item() - E_ref) <= TOL_E * abs(E_ref)
+    plan.close()
+
+
 def test_kernel_path_chosen_per_mesh():
     expect = {(1, 32, 32): 2, (1, 1024, 1024): 2, (128, 128, 128): 3, (32, 512, 512): 3, (32, 16, 1024): 0, (512, 2, 4): 0}
     for (nz, ny, nx), path in expect.items():
