@@ -34,6 +34,8 @@ struct SRows {
     BD_HD float2* ptr(int row, int e) const { return p + row * PITCH + prow(L, e); }
     static BD_HD float2 ld(const float2* q) { return *q; }
     BD_HD void st(float2* q, float2 v) const { *q = v; }
+    BD_HD void pre(const float2*, int) const {}
+    BD_HD void stq(float2* q, float2 v, int) const { *q = v; }
 };
 struct GRowsIn {               // rows of a real array read as (x[2m], x[2m+1]) pairs
     const float* p; long pitch;
@@ -46,6 +48,8 @@ struct GRowsOut {
     static BD_HD constexpr int off(int S, int r) { return r * S; }
     BD_HD float2* ptr(int row, int e) const { return reinterpret_cast<float2*>(p + row * pitch) + e; }
     BD_HD void st(float2* q, float2 v) const { *q = v; }
+    BD_HD void pre(const float2*, int) const {}
+    BD_HD void stq(float2* q, float2 v, int) const { *q = v; }
 };
 // H rows written, and sum M.H gathered on the way (S8 fused into S7): M has H's layout, so
 // the matching M pair sits at a fixed byte distance from the H pair
@@ -53,11 +57,15 @@ struct GRowsOutE {
     float* p; long pitch; long m_minus_h; double* acc;
     static BD_HD constexpr int off(int S, int r) { return r * S; }
     BD_HD float2* ptr(int row, int e) const { return reinterpret_cast<float2*>(p + row * pitch) + e; }
-    BD_HD void st(float2* q, float2 v) const {
-        *q = v;
-        const float2 m = BD_LDCG(reinterpret_cast<const float2*>(reinterpret_cast<const char*>(q) + m_minus_h));
-        *acc += (double)m.x * v.x + (double)m.y * v.y;
+    mutable float2 mbuf[8];        // M pairs of the outputs of one butterfly, loaded before it is computed
+    BD_HD void pre(const float2* q, int r) const {
+        mbuf[r] = BD_LDCG(reinterpret_cast<const float2*>(reinterpret_cast<const char*>(q) + m_minus_h));
     }
+    BD_HD void stq(float2* q, float2 v, int r) const {
+        *q = v;
+        *acc += (double)mbuf[r].x * v.x + (double)mbuf[r].y * v.y;
+    }
+    BD_HD void st(float2* q, float2 v) const { *q = v; }
 };
 
 // Energy fused into the last kernel of an evaluation (boris_demag_apply_energy): every block

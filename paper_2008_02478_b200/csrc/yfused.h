@@ -76,6 +76,8 @@ struct STile {                 // shared: S[c][p(e)][col]
     BD_HD float2* ptr(int c, int e) const { return p + c * CP + pidx(e) * COLS; }
     static BD_HD float2 ld(const float2* q) { return *q; }
     BD_HD void st(float2* q, float2 v) const { *q = v; }
+    BD_HD void pre(const float2*, int) const {}
+    BD_HD void stq(float2* q, float2 v, int) const { *q = v; }
 };
 template <int COLS>
 struct GTile {                 // global: V tile [y][col], component stride cstride
@@ -84,6 +86,8 @@ struct GTile {                 // global: V tile [y][col], component stride cstr
     BD_HD float2* ptr(int c, int e) const { return p + c * cstride + (long)e * COLS; }
     static BD_HD float2 ld(const float2* q) { return BD_LDCG(q); }     // streamed once: keep it out of L1
     BD_HD void st(float2* q, float2 v) const { *q = v; }
+    BD_HD void pre(const float2*, int) const {}
+    BD_HD void stq(float2* q, float2 v, int) const { *q = v; }
 };
 
 // ------------------------------------------------------------------ passes
@@ -159,9 +163,12 @@ BD_HD void inv_passM(int it, int c0, int cstep, int cend, const In& in, const Ou
         }
         float2* po = out.ptr(c, base);
         if constexpr (P == 0) {
+            // an accessor that needs something from memory per output (the fused energy) asks for it now
+            BD_UNROLL
+            for (int r = 0; r < R / 2; ++r) out.pre(po + Out::off(S, r), r);
             PkDftTrunc<R, +1>::run(v);
             BD_UNROLL
-            for (int r = 0; r < R / 2; ++r) out.st(po + Out::off(S, r), v[r]);
+            for (int r = 0; r < R / 2; ++r) out.stq(po + Out::off(S, r), v[r], r);
         } else {
             PkDft<R, +1>::run(v);
             BD_UNROLL
