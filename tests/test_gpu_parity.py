@@ -181,7 +181,9 @@ def test_config_at_full_size(name):
     H2 = np.empty_like(M)
     E2 = plan.apply_host(M, H2)
     assert np.array_equal(H2, H)
-    assert E2 == E
+    # apply_host gathers E inside the last kernel (boris_demag_apply_energy): another fp64 summation order
+    assert abs(E2 - E) <= 1e-12 * abs(E)
+    assert plan.apply_host(M, H2) == E2
     plan.close()
 
 
