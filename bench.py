@@ -379,7 +379,7 @@ def main():
 
     # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the ncu --set full
     # captures summarised in profiles/r01_tiled.md (one capture per workload; None where none was taken)
-    ncu_traffic = {("C5", "YFused"): 618432768 + 356407296, ("C3", "YFused"): 42230784 + 26368}
+    ncu_traffic = {("C5", "YFused"): 648591360 + 357802240, ("C3", "YFused"): 42233088 + 1280}
     kernels = res["kernels"]
     dom = max((k for k in kernels if k != "Energy"), key=lambda k: kernels[k]["ms_per_eval"])
     dk = kernels[dom]
