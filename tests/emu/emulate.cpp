@@ -15,9 +15,21 @@
 
 namespace {
 
+// Thread order inside a phase: 0 ascending, 1 descending, 2 odd threads then even ones.  The threads of
+// a phase must not depend on each other (only barriers order them), so every order has to give
+// the same bits: a cheap stand-in for a race checker.
+int g_thread_order = 0;
+
 template <class K, int PH>
 void run_phases(int bx, int by, const typename K::Args& a, float2* sm) {
-    for (int tid = 0; tid < K::NT; ++tid) K::template phase<PH>(tid, bx, by, a, sm);
+    if (g_thread_order == 1) {
+        for (int tid = K::NT - 1; tid >= 0; --tid) K::template phase<PH>(tid, bx, by, a, sm);
+    } else if (g_thread_order == 2) {
+        for (int tid = 1; tid < K::NT; tid += 2) K::template phase<PH>(tid, bx, by, a, sm);
+        for (int tid = 0; tid < K::NT; tid += 2) K::template phase<PH>(tid, bx, by, a, sm);
+    } else {
+        for (int tid = 0; tid < K::NT; ++tid) K::template phase<PH>(tid, bx, by, a, sm);
+    }
     if constexpr (PH + 1 < K::NPHASES) run_phases<K, PH + 1>(bx, by, a, sm);
 }
 
@@ -99,6 +111,7 @@ int emu_storage_roundtrip(int nx, int ny, int nz, const double* Kred, double* ou
     return 0;
 }
 
+void emu_set_thread_order(int order) { g_thread_order = order; }
 int emu_pos_of_freq(int L, int k) { return bd::pos_of_freq(L, k); }
 int emu_freq_of_pos(int L, int p) { return bd::freq_of_pos(L, p); }
 int emu_khat_rows(int L) { return bd::khat_rows(L); }

@@ -166,3 +166,24 @@ def test_emulated_kernels_match_the_oracle(emu, shape, h, texture, cs):
     err = np.abs(H - H_ref)
     assert err.max() <= 1e-5 * Ms                                   # north_star tolerance
     assert np.sqrt((err ** 2).sum() / (H_ref ** 2).sum()) <= 2e-6
+
+
+@pytest.mark.parametrize("shape,cs", [((1, 16, 64), 0), ((1, 128, 8), 0), ((4, 8, 16), 0), ((32, 4, 32), 0),
+                                      ((64, 4, 8), 0), ((8, 16, 8), -1)])
+def test_phases_do_not_depend_on_the_order_of_their_threads(emu, shape, cs):
+    """Threads of one phase may only meet at barriers: running them in another order must give the same bits."""
+    nz, ny, nx = shape
+    h = (2.0, 3.0, 1.0)
+    M = W.make_texture("random", shape, 8e5, seed=17)
+    K = binding.spectrum_host(nx, ny, nz, *h)
+    out = []
+    try:
+        for order in (0, 1, 2):
+            emu.emu_set_thread_order(order)
+            H = np.full(M.shape, np.nan, np.float32)
+            assert emu.emu_apply(nx, ny, nz, vp(K), vp(M), vp(H), cs) == 0
+            out.append(H)
+    finally:
+        emu.emu_set_thread_order(0)
+    assert np.isfinite(out[0]).all()
+    assert np.array_equal(out[0], out[1]) and np.array_equal(out[0], out[2])
