@@ -324,8 +324,8 @@ boris_demag_plan* boris_demag_plan_create(int nx, int ny, int nz, double hx, dou
     {
         int sms = 148;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        p->cfg.pf_y = 2 * sms;         // YFused: two blocks per SM
-        p->cfg.pf_xz = sms;            // XZFwd: one
+        p->cfg.pf_y = sms / 2;          // measured: 8..148 blocks ahead are within 1 %, longer distances lose (profiles/r01_tiled.md)
+        p->cfg.pf_xz = sms / 4;         // measured best of 0 / 8 / 32 / 74 / 110 / 148 / 296
     }
     p->kl = p->cfg.tiled ? bd::make_klayout_tiled(nx, ny, nz, p->cfg.cols) : bd::make_klayout(nx, ny, nz, p->cfg.ty);
     const bd::KLayout& kl = p->kl;
