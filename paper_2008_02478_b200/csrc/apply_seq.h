@@ -22,7 +22,7 @@ struct LaunchCfg {
     int tiled;     // 1: tiled path (xt.h / yfused.h), 0: the kernels of kernels.h
     int cols;      // kx columns per tile
     int rbt;       // rows per block of XFwdT / XInvT
-    int pf_y;      // L2 prefetch distance of YFused in blocks (= blocks resident on the device), 0: off
+    int pf_y;      // L2 prefetch distance of YFused in blocks, 0: off (set by the plan)
     int pf_xz;     // ... of XZFwd
 };
 
