@@ -15,7 +15,6 @@ namespace bd {
 
 struct LaunchCfg {
     int rb;        // rows per block of XFwd / XInv
-    int nb_y2d;    // kx slots per block of Y2D
     int nb_y;      // rows per block of YFwd / YInv
     int cs;        // kx slots per chunk of the 3-D path
     int ty;        // y positions per block of ZFused
@@ -45,7 +44,6 @@ inline LaunchCfg make_launch_cfg(int nx, int ny, int nz) {
     const int Py = 2 * ny, Pz = nz > 1 ? 2 * nz : 1;
     c.rb = nx <= 512 ? 16 : 8;
     while (c.rb > ny) c.rb >>= 1;
-    c.nb_y2d = Py >= 256 ? 1 : 256 / Py;
     c.nb_y = Py >= 1024 ? 2 : 2048 / Py;
     c.ty = Pz <= 128 ? 16 : (Pz <= 256 ? 8 : (Pz <= 512 ? 4 : 2));
     while (c.ty > Py) c.ty >>= 1;
