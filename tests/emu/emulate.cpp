@@ -56,6 +56,27 @@ struct HostLauncher {
 
 }  // namespace
 
+namespace {
+struct PlainPencil {           // one unpadded pencil in plain memory
+    float2* p;
+    static constexpr int off(int S, int r) { return r * S; }
+    float2* ptr(int, int e) const { return p + e; }
+    static float2 ld(const float2* q) { return *q; }
+    void st(float2* q, float2 v) const { *q = v; }
+    void pre(const float2*, int) const {}
+    void stq(float2* q, float2 v, int) const { *q = v; }
+};
+template <int L, int P, bool INV>
+void pk_pass_all(PlainPencil a, const float2* ptw) {
+    constexpr int items = L / bd::dec_r(L, P);
+    for (int it = 0; it < items; ++it) {
+        if constexpr (!INV) bd::fwd_passM<L, P>(it, 0, 1, 1, a, a, ptw);
+        else bd::inv_passM<L, P>(it, 0, 1, 1, a, a, ptw);
+    }
+}
+}  // namespace
+
+
 extern "C" {
 
 // Kred: natural reduced spectrum [ncomp][nzr][nyr][nxr] in fp64 including the folded
@@ -135,6 +156,31 @@ int emu_fft_roundtrip(int L, const float* in_ri, float* spec_ri, float* out_ri) 
     if (rc) return rc;
     for (int i = 0; i < L; ++i) { spec_ri[2 * i] = b[i].x; spec_ri[2 * i + 1] = b[i].y; }
     rc = dispatch_len(L, [&](auto ic) { return run.template run<YPass<decltype(ic)::value, true>>(Grid{1, 1}, g); });
+    if (rc) return rc;
+    for (int i = 0; i < L / 2; ++i) { out_ri[2 * i] = a[i].x; out_ri[2 * i + 1] = a[i].y; }
+    return 0;
+}
+
+// The packed-arithmetic passes of the tiled path (pk.h, yfused.h) on one pencil: x[0..L/2) -> X (digit
+// reversed, length L) -> back to x[0..L/2) scaled by L, with the per-pass twiddle tables of fill_pass_twiddles.
+int emu_fft_roundtrip_pk(int L, const float* in_ri, float* spec_ri, float* out_ri) {
+    using namespace bd;
+    std::vector<float2> ptw((size_t)ptw_total(L)), a((size_t)L, bd_f2(0.f, 0.f));
+    fill_pass_twiddles(ptw.data(), L);
+    for (int i = 0; i < L / 2; ++i) { a[i].x = in_ri[2 * i]; a[i].y = in_ri[2 * i + 1]; }
+    const int rc = dispatch_len(L, [&](auto ic) {
+        constexpr int LL = decltype(ic)::value;
+        constexpr int NP = dec_np(LL);
+        PlainPencil pp{a.data()};
+        pk_pass_all<LL, 0, false>(pp, ptw.data());
+        if constexpr (NP >= 2) pk_pass_all<LL, 1, false>(pp, ptw.data());
+        if constexpr (NP >= 3) pk_pass_all<LL, 2, false>(pp, ptw.data());
+        for (int i = 0; i < LL; ++i) { spec_ri[2 * i] = a[i].x; spec_ri[2 * i + 1] = a[i].y; }
+        if constexpr (NP >= 3) pk_pass_all<LL, 2, true>(pp, ptw.data());
+        if constexpr (NP >= 2) pk_pass_all<LL, 1, true>(pp, ptw.data());
+        pk_pass_all<LL, 0, true>(pp, ptw.data());
+        return 0;
+    });
     if (rc) return rc;
     for (int i = 0; i < L / 2; ++i) { out_ri[2 * i] = a[i].x; out_ri[2 * i + 1] = a[i].y; }
     return 0;

@@ -106,14 +106,15 @@ def test_index_maps_are_bijections_and_rows_cover_the_half_spectrum(emu):
         assert covered == set(range(L // 2 + 1))
 
 
+@pytest.mark.parametrize("core", ["emu_fft_roundtrip", "emu_fft_roundtrip_pk"])      # chunked kernels' core, packed core
 @pytest.mark.parametrize("L", [4, 8, 16, 32, 64, 128, 256, 512, 1024, 2048])
-def test_pruned_forward_and_truncated_inverse_fft_against_numpy(emu, L):
+def test_pruned_forward_and_truncated_inverse_fft_against_numpy(emu, L, core):
     rng = np.random.default_rng(L)
     x = (rng.standard_normal(L // 2) + 1j * rng.standard_normal(L // 2)).astype(np.complex64)
     xin = np.ascontiguousarray(x.view(np.float32))
     spec = np.zeros(2 * L, np.float32)
     back = np.zeros(L, np.float32)
-    assert emu.emu_fft_roundtrip(L, vp(xin), vp(spec), vp(back)) == 0
+    assert getattr(emu, core)(L, vp(xin), vp(spec), vp(back)) == 0
     ref = np.fft.fft(np.concatenate([x.astype(np.complex128), np.zeros(L // 2)]))
     got = spec.view(np.complex64)
     pos = [emu.emu_pos_of_freq(L, k) for k in range(L)]
