@@ -415,13 +415,32 @@ struct ZXInv {
 
     // frequencies kz = 2k + PAR of one column -> their part of x[z]; the odd half adds to
     // what the even half left in shared memory.  Column 0 carries P^ = Y0^ + i YN^.
-    template <int PAR>
-    static BD_HD void zhalf(const float2* in, const float2* inn, float2* col, long kzs, int kx) {
+    // nq: the Nyquist column, spread over the lanes of warp 0 (lane l holds kz = l and l + 32); only
+    // that warp's first trip (kx = lane) carries column 0 and calls with WARP0 = true
+    static constexpr int NQ = (PZ + 31) / 32;
+    static constexpr bool COOP = LX >= 32;                  // all 32 lanes of warp 0 are in the first trip
+    template <int PAR, bool WARP0>
+    static BD_HD void zhalf(const float2* in, const float2* inn, const float2* nq, float2* col, long kzs, int kx) {
         float2 v[NZ];
+        in += PAR * kzs;
         BD_UNROLL
-        in += PAR * kzs; inn += PAR * kzs;
         for (int k = 0; k < NZ; ++k) { v[k] = BD_LDCG(in); in += 2 * kzs; }
+#if defined(__CUDA_ARCH__)
+        if constexpr (WARP0 && COOP) {
+            // every lane hands its share of the Nyquist column to lane 0 (kx = 0)
+            BD_UNROLL
+            for (int k = 0; k < NZ; ++k) {
+                const int kz = 2 * k + PAR;
+                float2 n;
+                n.x = __shfl_sync(0xffffffffu, nq[kz >> 5].x, kz & 31);
+                n.y = __shfl_sync(0xffffffffu, nq[kz >> 5].y, kz & 31);
+                if (kx == 0) v[k] = bd_f2(v[k].x - n.y, v[k].y + n.x);
+            }
+        } else
+#endif
         if (kx == 0) {
+            (void)nq;
+            inn += PAR * kzs;
             BD_UNROLL
             for (int k = 0; k < NZ; ++k) {
                 const float2 n = BD_LDCG(inn);
@@ -454,12 +473,29 @@ struct ZXInv {
                     zcolumn(in, col, kzs, a.ztw);
                 }
             } else {
+                const float2* inn = vc + ((long)((LX >> a.cs) * a.ny + y) << a.cs) + (LX & (cols - 1));
+                float2 nq[NQ];
+                BD_UNROLL
+                for (int q = 0; q < NQ; ++q) nq[q] = bd_f2(0.f, 0.f);
+#if defined(__CUDA_ARCH__)
+                if (COOP && tid < 32) {
+                    // the Nyquist column (column 0 needs it: P^ = Y0^ + i YN^) is fetched by the 32 lanes of
+                    // warp 0 together, in flight with their own columns, instead of by lane 0 alone afterwards
+                    BD_UNROLL
+                    for (int q = 0; q < NQ; ++q)
+                        if (tid + 32 * q < PZ) nq[q] = BD_LDCG(inn + (long)(tid + 32 * q) * kzs);
+                }
+#endif
                 for (int kx = tid; kx < LX; kx += NT) {
                     const float2* in = vc + ((long)((kx >> a.cs) * a.ny + y) << a.cs) + (kx & (cols - 1));
-                    const float2* inn = vc + ((long)((LX >> a.cs) * a.ny + y) << a.cs) + (LX & (cols - 1));
                     float2* col = sm + xz_pos(a.xpost, LX, kx);
-                    zhalf<0>(in, inn, col, kzs, kx);
-                    zhalf<1>(in, inn, col, kzs, kx);
+                    if (kx < 32) {                 // warp 0, first trip
+                        zhalf<0, true>(in, inn, nq, col, kzs, kx);
+                        zhalf<1, true>(in, inn, nq, col, kzs, kx);
+                    } else {
+                        zhalf<0, false>(in, inn, nq, col, kzs, kx);
+                        zhalf<1, false>(in, inn, nq, col, kzs, kx);
+                    }
                 }
             }
         } else if constexpr (PH == 1) {
