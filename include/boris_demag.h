@@ -16,8 +16,12 @@
  *   - SI units: M, H in A/m; cell sides in metres; energy in joules; mu0 = 4 pi 1e-7.
  *   - M and H are fp32, planar, [3][nz][ny][nx], x fastest: element (c, k, j, i) of
  *     a component c in {x, y, z} at cell (i, j, k) is at ((c*nz + k)*ny + j)*nx + i.
- *   - Supported sizes: nx, ny in {2, 4, ..., 1024} with nx >= 4; nz = 1 (2-D mode,
- *     Nxz and Nyz dropped) or nz in {2, 4, ..., 512}.  Anything else: error -1.
+ *   - Supported sizes: 1 <= nx, ny <= 1024, 1 <= nz <= 512 (nz = 1: 2-D mode, Nxz and Nyz
+ *     dropped); anything else: error -1.  The kernels work on power-of-two meshes (nx >= 4,
+ *     ny >= 2, nz = 1 or >= 2): any other mesh is evaluated exactly as the corner of the next
+ *     power-of-two mesh whose remaining cells hold M = 0 (linear convolution only needs a
+ *     padded length >= 2n - 1), staged through plan-owned buffers by two copy
+ *     kernels per call; M and H then only need 4-byte alignment.
  *   - All fp32 arithmetic on the device; fp64 only at plan time and in the energy sum.
  *   - A plan owns the kernel spectrum, twiddle tables and workspace on the device
  *     that was current when it was created.  It may be used from one stream at a

@@ -201,7 +201,8 @@ class DemagPlan:
     def kernel_spectrum(self):
         """Natural reduced fp32 spectrum [ncomp][nzr][nyr][nxr] read back from the device."""
         ncomp = 6 if self.nz > 1 else 4
-        out = np.empty((ncomp, self.nz + 1 if self.nz > 1 else 1, self.ny + 1, self.nx + 1), np.float32)
+        Px, Py, Pz = self.info()["padded"]          # of the power-of-two mesh the kernels work on
+        out = np.empty((ncomp, Pz // 2 + 1 if self.nz > 1 else 1, Py // 2 + 1, Px // 2 + 1), np.float32)
         _check(lib().boris_demag_plan_kernel_spectrum(self._h, out.ctypes.data), "boris_demag_plan_kernel_spectrum")
         return out
 

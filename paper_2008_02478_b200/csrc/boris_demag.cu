@@ -161,6 +161,13 @@ int grid_for(long total, int threads) {
 
 // ------------------------------------------------------------------ plan
 struct boris_demag_plan {
+    // nx, ny, nz: the mesh the kernels work on (powers of two).  ux, uy, uz: the caller's mesh; where it is
+    // not one the kernels take, it sits in the corner of the next power-of-two mesh whose other cells
+    // hold M = 0 (exact: empty cells add nothing to the sum of PAPER.md:L323), staged through Mp / Hp.
+    int ux, uy, uz;
+    bool padmode = false;
+    float* Mp = nullptr;             // [3][nz][ny][nx], zero outside the caller's cells
+    float* Hp = nullptr;
     int nx, ny, nz;
     double hx, hy, hz;
     bd::KLayout kl;
@@ -288,10 +295,35 @@ int build_spectrum(boris_demag_plan* p) {
 int check_sizes(int nx, int ny, int nz, double hx, double hy, double hz) {
     if (!(hx > 0.0) || !(hy > 0.0) || !(hz > 0.0) || !std::isfinite(hx) || !std::isfinite(hy) || !std::isfinite(hz))
         return fail(-1, "cell sides must be positive and finite");
-    if (!is_pow2(nx) || nx < 4 || nx > 1024) return fail(-1, "nx must be a power of two in [4, 1024]");
-    if (!is_pow2(ny) || ny < 2 || ny > 1024) return fail(-1, "ny must be a power of two in [2, 1024]");
-    if (!(nz == 1 || (is_pow2(nz) && nz >= 2 && nz <= 512))) return fail(-1, "nz must be 1 or a power of two in [2, 512]");
+    if (nx < 1 || nx > 1024) return fail(-1, "nx must be in [1, 1024]");
+    if (ny < 1 || ny > 1024) return fail(-1, "ny must be in [1, 1024]");
+    if (nz < 1 || nz > 512) return fail(-1, "nz must be in [1, 512]");
     return 0;
+}
+
+int next_pow2(int n) { int p = 1; while (p < n) p <<= 1; return p; }
+
+// (used by the entry points below)
+// caller's mesh [3][uz][uy][ux] <-> its corner of the kernels' mesh [3][nz][ny][nx]
+__global__ void k_pad(const float* __restrict__ src, float* __restrict__ dst, int ux, int uy, int uz, int nx, int ny, int nz) {
+    const long total = 3L * ux * uy * uz;
+    for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total; idx += (long)gridDim.x * blockDim.x) {
+        long r = idx;
+        const int x = (int)(r % ux); r /= ux;
+        const int y = (int)(r % uy); r /= uy;
+        const int z = (int)(r % uz); const int c = (int)(r / uz);
+        dst[(((long)c * nz + z) * ny + y) * nx + x] = src[idx];
+    }
+}
+__global__ void k_crop(const float* __restrict__ src, float* __restrict__ dst, int ux, int uy, int uz, int nx, int ny, int nz) {
+    const long total = 3L * ux * uy * uz;
+    for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total; idx += (long)gridDim.x * blockDim.x) {
+        long r = idx;
+        const int x = (int)(r % ux); r /= ux;
+        const int y = (int)(r % uy); r /= uy;
+        const int z = (int)(r % uz); const int c = (int)(r / uz);
+        dst[idx] = src[(((long)c * nz + z) * ny + y) * nx + x];
+    }
 }
 
 }  // namespace
@@ -305,20 +337,24 @@ void boris_demag_plan_destroy(boris_demag_plan* p) {
     if (!p) return;
     cudaFree(p->Kst); cudaFree(p->tw_x); cudaFree(p->tw_xpost); cudaFree(p->tw_y); cudaFree(p->tw_z);
     cudaFree(p->W); cudaFree(p->T); cudaFree(p->partial); cudaFree(p->partial_f);
-    cudaFree(p->V); cudaFree(p->ptw_x); cudaFree(p->ptw_y); cudaFree(p->xpost);
+    cudaFree(p->V); cudaFree(p->ptw_x); cudaFree(p->ptw_y); cudaFree(p->xpost); cudaFree(p->Mp); cudaFree(p->Hp);
     cudaFree(p->stage_M); cudaFree(p->stage_H); cudaFree(p->stage_E);
     delete p;
 }
 
-boris_demag_plan* boris_demag_plan_create(int nx, int ny, int nz, double hx, double hy, double hz) {
+boris_demag_plan* boris_demag_plan_create(int ux, int uy, int uz, double hx, double hy, double hz) {
     g_err.clear();
-    if (check_sizes(nx, ny, nz, hx, hy, hz)) return nullptr;
+    if (check_sizes(ux, uy, uz, hx, hy, hz)) return nullptr;
+    // the kernels take power-of-two meshes: nx >= 4, ny >= 2, nz = 1 or >= 2
+    const int nx = next_pow2(ux < 4 ? 4 : ux), ny = next_pow2(uy < 2 ? 2 : uy), nz = uz == 1 ? 1 : next_pow2(uz);
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) { cuda_fail(e, "cudaGetDevice (no CUDA device: this library has no CPU fallback)"); return nullptr; }
     boris_demag_plan* p = new (std::nothrow) boris_demag_plan();
     if (!p) { fail(-3, "out of host memory"); return nullptr; }
     p->nx = nx; p->ny = ny; p->nz = nz; p->hx = hx; p->hy = hy; p->hz = hz; p->device = dev;
+    p->ux = ux; p->uy = uy; p->uz = uz;
+    p->padmode = nx != ux || ny != uy || nz != uz;
     const int Py = 2 * ny, Pz = nz > 1 ? 2 * nz : 1;
     p->cfg = bd::make_launch_cfg(nx, ny, nz);
     {
@@ -353,6 +389,13 @@ boris_demag_plan* boris_demag_plan_create(int nx, int ny, int nz, double hx, dou
         if (!rc) rc = dev_alloc(p, &p->W, (size_t)3 * kl.nxr() * nz * ny);
         if (!rc && nz > 1) rc = dev_alloc(p, &p->T, (size_t)3 * p->cfg.cs * nz * Py);
     }
+    if (p->padmode) {
+        const size_t np = (size_t)3 * nx * ny * nz;
+        if (!rc) rc = dev_alloc(p, &p->Mp, np);
+        if (!rc) rc = dev_alloc(p, &p->Hp, np);
+        if (!rc && cudaMemset(p->Mp, 0, np * sizeof(float)) != cudaSuccess) rc = fail(-2, "cudaMemset");
+        if (!rc && cudaMemset(p->Hp, 0, np * sizeof(float)) != cudaSuccess) rc = fail(-2, "cudaMemset");
+    }
     if (!rc) rc = dev_alloc(p, &p->partial, (size_t)kEnergyBlocks + 1);
     if (!rc && cudaMemset(p->partial, 0, ((size_t)kEnergyBlocks + 1) * sizeof(double)) != cudaSuccess) rc = fail(-2, "cudaMemset");
     if (!rc) rc = dev_alloc(p, &p->partial_f, (size_t)kFusedEnergySlots + 1);
@@ -361,25 +404,52 @@ boris_demag_plan* boris_demag_plan_create(int nx, int ny, int nz, double hx, dou
     return p;
 }
 
-int boris_demag_apply(boris_demag_plan* p, const float* M, float* H, void* stream) {
+namespace {
+int check_fields(const boris_demag_plan* p, const void* M, const void* H, bool alias_ok) {
     if (!p || !M || !H) return fail(-1, "null argument");
-    if (M == H) return fail(-1, "M and H must not alias");
-    if (((uintptr_t)M | (uintptr_t)H) & 15) return fail(-1, "M and H must be 16-byte aligned");
+    if (!alias_ok && M == H) return fail(-1, "M and H must not alias");
+    // the kernels read rows as 16-byte vectors; a mesh staged through Mp / Hp is copied element by element
+    if ((((uintptr_t)M | (uintptr_t)H) & (p->padmode ? 3 : 15)) != 0)
+        return fail(-1, p->padmode ? "M and H must be 4-byte aligned" : "M and H must be 16-byte aligned");
+    return 0;
+}
+int stage(const boris_demag_plan* p, bool in, const float* src, float* dst, cudaStream_t st) {
+    const long total = 3L * p->ux * p->uy * p->uz;
+    if (in) k_pad<<<grid_for(total, 256), 256, 0, st>>>(src, dst, p->ux, p->uy, p->uz, p->nx, p->ny, p->nz);
+    else k_crop<<<grid_for(total, 256), 256, 0, st>>>(src, dst, p->ux, p->uy, p->uz, p->nx, p->ny, p->nz);
+    BD_CUDA(cudaGetLastError());
+    return 0;
+}
+}  // namespace
+
+int boris_demag_apply(boris_demag_plan* p, const float* M, float* H, void* stream) {
+    if (int rc = check_fields(p, M, H, false)) return rc;
+    if (p->padmode) {
+        if (int rc = stage(p, true, M, p->Mp, (cudaStream_t)stream)) return rc;
+        M = p->Mp;
+    }
+    float* Hu = H;
+    if (p->padmode) H = p->Hp;
     CudaLauncher run{(cudaStream_t)stream};
     const bd::PlanView pv = plan_view(p);
     const int rc = bd::enqueue_apply(run, pv, M, H);
     if (rc == -2) return cuda_fail(run.err, "kernel launch");
     if (rc) return fail(rc, "unsupported size");
+    if (p->padmode) return stage(p, false, p->Hp, Hu, (cudaStream_t)stream);
     return 0;
 }
 
 int boris_demag_apply_energy(boris_demag_plan* p, const float* M, float* H, double* E_dev, void* stream) {
-    if (!p || !M || !H || !E_dev) return fail(-1, "null argument");
-    if (M == H) return fail(-1, "M and H must not alias");
-    if (((uintptr_t)M | (uintptr_t)H) & 15) return fail(-1, "M and H must be 16-byte aligned");
+    if (!E_dev) return fail(-1, "null argument");
+    if (int rc = check_fields(p, M, H, false)) return rc;
     if (!p->cfg.tiled) {
         if (int rc = boris_demag_apply(p, M, H, stream)) return rc;
         return boris_demag_energy(p, M, H, E_dev, stream);
+    }
+    float* Hu = H;
+    if (p->padmode) {            // the empty cells of Mp add nothing to sum M.H
+        if (int rc = stage(p, true, M, p->Mp, (cudaStream_t)stream)) return rc;
+        M = p->Mp; H = p->Hp;
     }
     CudaLauncher run{(cudaStream_t)stream};
     bd::PlanView pv = plan_view(p);
@@ -388,14 +458,19 @@ int boris_demag_apply_energy(boris_demag_plan* p, const float* M, float* H, doub
     const int rc = bd::enqueue_apply(run, pv, M, H);
     if (rc == -2) return cuda_fail(run.err, "kernel launch");
     if (rc) return fail(rc, "unsupported size");
+    if (p->padmode) return stage(p, false, p->Hp, Hu, (cudaStream_t)stream);
     return 0;
 }
 
 int boris_demag_apply_timed(boris_demag_plan* p, const float* M, float* H, void* stream, float ms_by_kind[6],
                             int launches_by_kind[6]) {
-    if (!p || !M || !H || !ms_by_kind || !launches_by_kind) return fail(-1, "null argument");
-    if (M == H) return fail(-1, "M and H must not alias");
-    if (((uintptr_t)M | (uintptr_t)H) & 15) return fail(-1, "M and H must be 16-byte aligned");
+    if (!ms_by_kind || !launches_by_kind) return fail(-1, "null argument");
+    if (int rc = check_fields(p, M, H, false)) return rc;
+    float* Hu = H;
+    if (p->padmode) {            // the staging copies are not among the timed kinds
+        if (int rc = stage(p, true, M, p->Mp, (cudaStream_t)stream)) return rc;
+        M = p->Mp; H = p->Hp;
+    }
     std::vector<TimedLaunch> timed;
     CudaLauncher run{(cudaStream_t)stream};
     run.timed = &timed;
@@ -414,13 +489,19 @@ int boris_demag_apply_timed(boris_demag_plan* p, const float* M, float* H, void*
     if (rc == -2) return cuda_fail(run.err, "kernel launch");
     if (rc) return fail(rc, "unsupported size");
     if (e != cudaSuccess) return cuda_fail(e, "cudaStreamSynchronize");
+    if (p->padmode) return stage(p, false, p->Hp, Hu, (cudaStream_t)stream);
     return 0;
 }
 
 int boris_demag_energy(boris_demag_plan* p, const float* M, const float* H, double* E_dev, void* stream) {
-    if (!p || !M || !H || !E_dev) return fail(-1, "null argument");
-    if (((uintptr_t)M | (uintptr_t)H) & 15) return fail(-1, "M and H must be 16-byte aligned");
+    if (!E_dev) return fail(-1, "null argument");
+    if (int rc = check_fields(p, M, H, true)) return rc;
     cudaStream_t st = (cudaStream_t)stream;
+    if (p->padmode) {            // sum over the staged copies: the empty cells of Mp add nothing
+        if (int rc = stage(p, true, M, p->Mp, st)) return rc;
+        if (int rc = stage(p, true, H, p->Hp, st)) return rc;
+        M = p->Mp; H = p->Hp;
+    }
     const long n4 = 3L * p->nx * p->ny * p->nz / 4;
     const double factor = -0.5 * (4e-7 * bd::kPi) * p->hx * p->hy * p->hz;
     long nblk = (n4 + 4L * kEnergyThreads - 1) / (4L * kEnergyThreads);      // fixed per plan: E stays reproducible
@@ -434,7 +515,7 @@ int boris_demag_energy(boris_demag_plan* p, const float* M, const float* H, doub
 int boris_demag_apply_host(boris_demag_plan* p, const float* M_host, float* H_host, double* E_host, void* stream) {
     if (!p || !M_host || !H_host) return fail(-1, "null argument");
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t n = (size_t)3 * p->nx * p->ny * p->nz;
+    const size_t n = (size_t)3 * p->ux * p->uy * p->uz;
     if (!p->stage_M) {
         if (int rc = dev_alloc(p, &p->stage_M, n)) return rc;
         if (int rc = dev_alloc(p, &p->stage_H, n)) return rc;
@@ -460,6 +541,9 @@ int boris_demag_plan_info(const boris_demag_plan* p, long long* compulsory_bytes
     const long long kred = 4LL * kl.ncomp * kl.nxr() * kl.nyr() * kl.nzr();
     const long long wbytes = 3LL * kl.nxr() * p->nz * p->ny * (long long)sizeof(float2);
     if (compulsory_bytes) *compulsory_bytes = 24 * N + kred;
+    if (compulsory_bytes && p->padmode)      // of the caller's mesh: its cells and the reduced spectrum of its own 2n padding
+        *compulsory_bytes = 24LL * p->ux * p->uy * p->uz +
+                            4LL * kl.ncomp * (p->ux + 1) * (p->uy + 1) * (p->uz > 1 ? p->uz + 1 : 1);
     // M in, W out | W in, stored spectrum in, W out | W in, H out.  The scratch T of the
     // 3-D path is sized to stay in L2 and is not counted.
     if (designed_hbm_bytes) *designed_hbm_bytes = 24 * N + 4 * wbytes + 4LL * kl.storage_elems();
@@ -468,9 +552,10 @@ int boris_demag_plan_info(const boris_demag_plan* p, long long* compulsory_bytes
         const long long vbytes = 3LL * kl.Pz * kl.ntl * p->ny * kl.cols * (long long)sizeof(float2);
         *designed_hbm_bytes = 24 * N + 4 * vbytes + 4LL * kl.storage_elems();
     }
+    if (designed_hbm_bytes && p->padmode) *designed_hbm_bytes += 48LL * p->ux * p->uy * p->uz;   // staging in and out
     if (workspace_bytes) *workspace_bytes = p->bytes;
     if (padded) { padded[0] = kl.Px; padded[1] = kl.Py; padded[2] = kl.Pz; }
-    if (kernel_launches) *kernel_launches = bd::apply_launch_count(p->nx, p->nz, p->cfg);
+    if (kernel_launches) *kernel_launches = bd::apply_launch_count(p->nx, p->nz, p->cfg) + (p->padmode ? 2 : 0);
     return 0;
 }
 

@@ -144,6 +144,37 @@ def test_fused_apply_energy_matches_the_two_calls_and_is_reproducible(shape):
     plan.close()
 
 
+@pytest.mark.parametrize("shape", [(1, 1, 1), (1, 7, 9), (3, 5, 6), (1, 100, 60), (5, 33, 17), (2, 1, 3), (40, 3, 2)])
+def test_meshes_that_are_not_powers_of_two_match_the_plain_double_sum(shape):
+    """Any mesh is the corner of the next power-of-two mesh with M = 0 elsewhere (include/boris_demag.h)."""
+    nz, ny, nx = shape
+    h = (3e-9, 2e-9, 4e-9)
+    Ms = 8e5
+    M_host = W.make_texture("random", shape, Ms, seed=41)
+    plan = binding.DemagPlan(nx, ny, nz, *h)
+    H, E = gpu_apply(plan, M_host, want_energy=True)
+    H_ref = demag_direct(M_host, h)
+    assert_parity(H, H_ref, Ms)
+    E_ref = demag_energy(M_host, H_ref, h)
+    assert abs(E - E_ref) <= TOL_E * abs(E_ref)
+    M = torch.from_numpy(M_host).cuda()
+    H2 = torch.full_like(M, float("nan"))
+    E2 = plan.apply_energy(M, H2)
+    torch.cuda.synchronize()
+    assert np.array_equal(H2.cpu().numpy(), H)
+    assert abs(E2.item() - E_ref) <= TOL_E * abs(E_ref)
+    H3 = np.empty_like(M_host)
+    E3 = plan.apply_host(M_host, H3)
+    assert np.array_equal(H3, H) and E3 == E2.item()
+    info = plan.info()
+    assert info["kernel_launches"] >= 5 and info["compulsory_bytes"] >= 24 * nx * ny * nz
+    plan.close()
+    with pytest.raises(binding.DemagError):
+        binding.DemagPlan(1025, 4, 1, *h)
+    with pytest.raises(binding.DemagError):
+        binding.DemagPlan(4, 4, 0, *h)
+
+
 def test_kernel_path_chosen_per_mesh():
     expect = {(1, 32, 32): 2, (1, 1024, 1024): 2, (128, 128, 128): 3, (32, 512, 512): 3, (32, 16, 1024): 0, (512, 2, 4): 0}
     for (nz, ny, nx), path in expect.items():
