@@ -54,6 +54,18 @@ void boris_demag_plan_destroy(boris_demag_plan* plan);
  * never allocates, never synchronises; bit-identical across calls. */
 int boris_demag_apply(boris_demag_plan* plan, const float* M, float* H, void* stream);
 
+/* Variants of boris_demag_apply selected by `flags` (0 = boris_demag_apply itself):
+ *   BORIS_DEMAG_AOS         M and H hold one float3 per cell, [nz][ny][nx][3], the layout of a vector-field
+ *                           library instead of planar components;
+ *   BORIS_DEMAG_ACCUMULATE  H += -N * M instead of H = -N * M: the demag term added to an effective field
+ *                           that already holds other contributions ("additive field contributions").
+ * Both go through plan-owned planar staging buffers and two copy kernels (M in, H out); on a power-of-two
+ * mesh the buffers are allocated by the FIRST such call (24 bytes per cell), which is the one case in which an
+ * apply allocates.  M, H: DEVICE pointers, 4-byte aligned, must not alias.  Error codes as boris_demag_apply. */
+#define BORIS_DEMAG_AOS 1u
+#define BORIS_DEMAG_ACCUMULATE 2u
+int boris_demag_apply_ex(boris_demag_plan* plan, const float* M, float* H, unsigned flags, void* stream);
+
 /* boris_demag_apply, instrumented for the measurement harness: a CUDA event pair is
  * recorded on `stream` around every kernel launch, the stream is synchronised, and the
  * device time is returned summed per kernel kind, in the order

@@ -35,6 +35,8 @@ def lib():
         L.boris_demag_plan_destroy.argtypes = [c_vp]
         L.boris_demag_apply.restype = c_int
         L.boris_demag_apply.argtypes = [c_vp, c_vp, c_vp, c_vp]
+        L.boris_demag_apply_ex.restype = c_int
+        L.boris_demag_apply_ex.argtypes = [c_vp, c_vp, c_vp, ctypes.c_uint, c_vp]
         L.boris_demag_apply_timed.restype = c_int
         L.boris_demag_apply_timed.argtypes = [c_vp, c_vp, c_vp, c_vp, ctypes.POINTER(ctypes.c_float),
                                               ctypes.POINTER(c_int)]
@@ -139,6 +141,20 @@ class DemagPlan:
         """H <- -N * M on `stream` (default: torch's current stream).  Asynchronous."""
         _check(lib().boris_demag_apply(self._h, self._ptr(M, "M"), self._ptr(H, "H"), self._stream(stream)),
                "boris_demag_apply")
+        return H
+
+    AOS, ACCUMULATE = 1, 2
+
+    def apply_ex(self, M, H, flags, stream=None):
+        """boris_demag_apply_ex: AOS -> M, H are [nz][ny][nx][3]; ACCUMULATE -> H += -N * M.  Asynchronous."""
+        import torch
+        shape = (self.nz, self.ny, self.nx, 3) if flags & self.AOS else self.shape
+        for t, name in ((M, "M"), (H, "H")):
+            if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()
+                    and tuple(t.shape) == tuple(shape)):
+                raise DemagError(f"{name} must be a contiguous CUDA float32 tensor of shape {shape}")
+        _check(lib().boris_demag_apply_ex(self._h, M.data_ptr(), H.data_ptr(), int(flags), self._stream(stream)),
+               "boris_demag_apply_ex")
         return H
 
     # timing slots of boris_demag_apply_timed, named per kernel path (boris_demag_plan_layout)

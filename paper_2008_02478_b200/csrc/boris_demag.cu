@@ -305,24 +305,32 @@ int next_pow2(int n) { int p = 1; while (p < n) p <<= 1; return p; }
 
 // (used by the entry points below)
 // caller's mesh [3][uz][uy][ux] <-> its corner of the kernels' mesh [3][nz][ny][nx]
-__global__ void k_pad(const float* __restrict__ src, float* __restrict__ dst, int ux, int uy, int uz, int nx, int ny, int nz) {
-    const long total = 3L * ux * uy * uz;
+// aos: the caller's array is [uz][uy][ux][3] (one float3 per cell) instead of planar [3][uz][uy][ux]
+__global__ void k_pad(const float* __restrict__ src, float* __restrict__ dst, int ux, int uy, int uz, int nx, int ny, int nz,
+                      bool aos) {
+    const long cells = (long)ux * uy * uz, total = 3L * cells;
     for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total; idx += (long)gridDim.x * blockDim.x) {
         long r = idx;
         const int x = (int)(r % ux); r /= ux;
         const int y = (int)(r % uy); r /= uy;
         const int z = (int)(r % uz); const int c = (int)(r / uz);
-        dst[(((long)c * nz + z) * ny + y) * nx + x] = src[idx];
+        const long cell = ((long)z * uy + y) * ux + x;
+        dst[(((long)c * nz + z) * ny + y) * nx + x] = src[aos ? 3 * cell + c : idx];
     }
 }
-__global__ void k_crop(const float* __restrict__ src, float* __restrict__ dst, int ux, int uy, int uz, int nx, int ny, int nz) {
-    const long total = 3L * ux * uy * uz;
+// accumulate: dst += the staged field instead of dst = it (additive effective-field contributions)
+__global__ void k_crop(const float* __restrict__ src, float* __restrict__ dst, int ux, int uy, int uz, int nx, int ny, int nz,
+                       bool aos, bool accumulate) {
+    const long cells = (long)ux * uy * uz, total = 3L * cells;
     for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total; idx += (long)gridDim.x * blockDim.x) {
         long r = idx;
         const int x = (int)(r % ux); r /= ux;
         const int y = (int)(r % uy); r /= uy;
         const int z = (int)(r % uz); const int c = (int)(r / uz);
-        dst[idx] = src[(((long)c * nz + z) * ny + y) * nx + x];
+        const long cell = ((long)z * uy + y) * ux + x;
+        const long o = aos ? 3 * cell + c : idx;
+        const float v = src[(((long)c * nz + z) * ny + y) * nx + x];
+        dst[o] = accumulate ? dst[o] + v : v;
     }
 }
 
@@ -413,10 +421,11 @@ int check_fields(const boris_demag_plan* p, const void* M, const void* H, bool a
         return fail(-1, p->padmode ? "M and H must be 4-byte aligned" : "M and H must be 16-byte aligned");
     return 0;
 }
-int stage(const boris_demag_plan* p, bool in, const float* src, float* dst, cudaStream_t st) {
+int stage(const boris_demag_plan* p, bool in, const float* src, float* dst, cudaStream_t st, bool aos = false,
+          bool accumulate = false) {
     const long total = 3L * p->ux * p->uy * p->uz;
-    if (in) k_pad<<<grid_for(total, 256), 256, 0, st>>>(src, dst, p->ux, p->uy, p->uz, p->nx, p->ny, p->nz);
-    else k_crop<<<grid_for(total, 256), 256, 0, st>>>(src, dst, p->ux, p->uy, p->uz, p->nx, p->ny, p->nz);
+    if (in) k_pad<<<grid_for(total, 256), 256, 0, st>>>(src, dst, p->ux, p->uy, p->uz, p->nx, p->ny, p->nz, aos);
+    else k_crop<<<grid_for(total, 256), 256, 0, st>>>(src, dst, p->ux, p->uy, p->uz, p->nx, p->ny, p->nz, aos, accumulate);
     BD_CUDA(cudaGetLastError());
     return 0;
 }
@@ -460,6 +469,29 @@ int boris_demag_apply_energy(boris_demag_plan* p, const float* M, float* H, doub
     if (rc) return fail(rc, "unsupported size");
     if (p->padmode) return stage(p, false, p->Hp, Hu, (cudaStream_t)stream);
     return 0;
+}
+
+int boris_demag_apply_ex(boris_demag_plan* p, const float* M, float* H, unsigned flags, void* stream) {
+    if (!p || !M || !H) return fail(-1, "null argument");
+    if (M == H) return fail(-1, "M and H must not alias");
+    if (flags & ~(unsigned)(BORIS_DEMAG_AOS | BORIS_DEMAG_ACCUMULATE)) return fail(-1, "unknown flag");
+    if (flags == 0) return boris_demag_apply(p, M, H, stream);
+    if (((uintptr_t)M | (uintptr_t)H) & 3) return fail(-1, "M and H must be 4-byte aligned");
+    if (!p->Mp) {                // first use of a staged variant on a power-of-two mesh
+        const size_t np = (size_t)3 * p->nx * p->ny * p->nz;
+        if (int rc = dev_alloc(p, &p->Mp, np)) return rc;
+        if (int rc = dev_alloc(p, &p->Hp, np)) return rc;
+        BD_CUDA(cudaMemsetAsync(p->Mp, 0, np * sizeof(float), (cudaStream_t)stream));
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool aos = (flags & BORIS_DEMAG_AOS) != 0, acc = (flags & BORIS_DEMAG_ACCUMULATE) != 0;
+    if (int rc = stage(p, true, M, p->Mp, st, aos)) return rc;
+    CudaLauncher run{st};
+    const bd::PlanView pv = plan_view(p);
+    const int rc = bd::enqueue_apply(run, pv, p->Mp, p->Hp);
+    if (rc == -2) return cuda_fail(run.err, "kernel launch");
+    if (rc) return fail(rc, "unsupported size");
+    return stage(p, false, p->Hp, H, st, aos, acc);
 }
 
 int boris_demag_apply_timed(boris_demag_plan* p, const float* M, float* H, void* stream, float ms_by_kind[6],

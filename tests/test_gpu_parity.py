@@ -175,6 +175,29 @@ def test_meshes_that_are_not_powers_of_two_match_the_plain_double_sum(shape):
         binding.DemagPlan(4, 4, 0, *h)
 
 
+@pytest.mark.parametrize("shape", [(1, 64, 32), (8, 16, 32), (3, 10, 6)])
+def test_float3_layout_and_accumulate_variants_give_the_same_field(shape):
+    nz, ny, nx = shape
+    M_host = W.make_texture("random", shape, 8e5, seed=51)
+    plan = binding.DemagPlan(nx, ny, nz, 2e-9, 2e-9, 1e-9)
+    M = torch.from_numpy(M_host).cuda()
+    H = torch.empty_like(M)
+    plan.apply(M, H)
+    M3 = M.permute(1, 2, 3, 0).contiguous()                    # [nz][ny][nx][3]
+    H3 = torch.full_like(M3, float("nan"))
+    plan.apply_ex(M3, H3, plan.AOS)
+    assert torch.equal(H3.permute(3, 0, 1, 2), H)              # same kernels on the same planar copy: same bits
+    H0 = torch.randn_like(M) * 1e4
+    Hacc = H0.clone()
+    plan.apply_ex(M, Hacc, plan.ACCUMULATE)
+    assert torch.equal(Hacc, H0 + H)
+    H0a = H0.permute(1, 2, 3, 0).contiguous()
+    plan.apply_ex(M3, H0a, plan.AOS | plan.ACCUMULATE)
+    assert torch.equal(H0a.permute(3, 0, 1, 2), H0 + H)
+    assert binding.lib().boris_demag_apply_ex(plan._h, M.data_ptr(), H.data_ptr(), 8, None) == -1
+    plan.close()
+
+
 def test_kernel_path_chosen_per_mesh():
     expect = {(1, 32, 32): 2, (1, 1024, 1024): 2, (128, 128, 128): 3, (32, 512, 512): 3, (32, 16, 1024): 0, (512, 2, 4): 0}
     for (nz, ny, nx), path in expect.items():
