@@ -62,6 +62,16 @@ def lib():
         L.boris_demag_spectrum_host.argtypes = [c_int, c_int, c_int, c_dbl, c_dbl, c_dbl, c_vp]
         L.boris_demag_version.restype = ctypes.c_char_p
         L.boris_demag_version.argtypes = []
+        L.boris_llg_create.restype = c_vp
+        L.boris_llg_create.argtypes = [c_vp, c_int, c_int, c_int] + [c_dbl] * 7
+        L.boris_llg_destroy.restype = None
+        L.boris_llg_destroy.argtypes = [c_vp]
+        L.boris_llg_set_applied_field.restype = c_int
+        L.boris_llg_set_applied_field.argtypes = [c_vp, c_dbl, c_dbl, c_dbl]
+        L.boris_llg_effective_field.restype = c_int
+        L.boris_llg_effective_field.argtypes = [c_vp, c_vp, c_vp, c_vp]
+        L.boris_llg_rk4.restype = c_int
+        L.boris_llg_rk4.argtypes = [c_vp, c_vp, c_dbl, c_int, c_vp]
         _lib = L
     return _lib
 
@@ -235,3 +245,40 @@ def _host_ptr(a, shape):
     if not (isinstance(a, np.ndarray) and a.dtype == np.float32 and a.flags.c_contiguous and a.shape == tuple(shape)):
         raise DemagError(f"host array must be C-contiguous float32 of shape {shape}")
     return a.ctypes.data
+
+
+class LLG:
+    """include/boris_llg.h: effective field (demag + exchange + applied field) and RK4 steps of the LLG equation
+    on CUDA float32 unit fields [3][nz][ny][nx].  Argument marshalling only."""
+
+    GAMMA = 2.212761569e5          # mu0 |gamma_e|, m / (A s)
+
+    def __init__(self, plan, Ms, A, alpha, gamma=GAMMA, Hext=(0.0, 0.0, 0.0)):
+        self.plan = plan
+        self._h = lib().boris_llg_create(plan._h, plan.nx, plan.ny, plan.nz, *plan.h, Ms, A, alpha, gamma)
+        if not self._h:
+            raise DemagError("boris_llg_create failed: " + last_error())
+        self.set_applied_field(*Hext)
+
+    def set_applied_field(self, Hx, Hy, Hz):
+        _check(lib().boris_llg_set_applied_field(self._h, Hx, Hy, Hz), "boris_llg_set_applied_field")
+
+    def effective_field(self, m, Heff, stream=None):
+        _check(lib().boris_llg_effective_field(self._h, self.plan._ptr(m, "m"), self.plan._ptr(Heff, "Heff"),
+                                               self.plan._stream(stream)), "boris_llg_effective_field")
+        return Heff
+
+    def rk4(self, m, dt, nsteps=1, stream=None):
+        _check(lib().boris_llg_rk4(self._h, self.plan._ptr(m, "m"), dt, nsteps, self.plan._stream(stream)), "boris_llg_rk4")
+        return m
+
+    def close(self):
+        if self._h:
+            lib().boris_llg_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,155 @@
+// boris_llg.cu — C ABI of include/boris_llg.h: the LLG evaluation around the demag path
+// (SURVEY.md section 8(f), NEXT-1).  The demagnetizing field comes from boris_demag_apply; the
+// kernels here are the cheap local terms of one evaluation (Eq. (1) at L33)
+// and the RK4 bookkeeping.  All of them stream planar fp32 fields once: HBM-bound.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <new>
+#include <string>
+
+#include "../../include/boris_llg.h"
+
+namespace {
+
+constexpr double kMu0 = 4e-7 * 3.14159265358979323846264338327950288;
+
+struct Dims { int nx, ny, nz; };
+
+// M = Ms m  (the demag kernels take A/m)
+__global__ void k_scale(const float* __restrict__ m, float* __restrict__ M, float Ms, long n) {
+    for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) M[i] = Ms * m[i];
+}
+
+// Heff += cx (m[x+1] - 2 m + m[x-1]) + cy (...) + cz (...) + Hext, a missing neighbour contributing nothing
+// (homogeneous Neumann condition); c* = 2A / (mu0 Ms h*^2)
+__global__ void k_exchange_zeeman(const float* __restrict__ m, float* __restrict__ H, Dims d, float cx, float cy, float cz,
+                                  float hx, float hy, float hz) {
+    const long cells = (long)d.nx * d.ny * d.nz, total = 3 * cells;
+    for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total; idx += (long)gridDim.x * blockDim.x) {
+        long r = idx;
+        const int x = (int)(r % d.nx); r /= d.nx;
+        const int y = (int)(r % d.ny); r /= d.ny;
+        const int z = (int)(r % d.nz); const int c = (int)(r / d.nz);
+        const float v = m[idx];
+        float lap = 0.f;
+        if (x + 1 < d.nx) lap += cx * (m[idx + 1] - v);
+        if (x > 0) lap += cx * (m[idx - 1] - v);
+        if (y + 1 < d.ny) lap += cy * (m[idx + d.nx] - v);
+        if (y > 0) lap += cy * (m[idx - d.nx] - v);
+        if (z + 1 < d.nz) lap += cz * (m[idx + (long)d.nx * d.ny] - v);
+        if (z > 0) lap += cz * (m[idx - (long)d.nx * d.ny] - v);
+        H[idx] += lap + (c == 0 ? hx : (c == 1 ? hy : hz));
+    }
+}
+
+// One RK4 stage per cell: k = -g [u x H + alpha u x (u x H)]  (Eq. (1) solved for dm/dt, g = gamma / (1 + alpha^2));
+// acc = (first ? 0 : acc) + w k;  then either the next stage state u_next = m0 + a k, or (last) the step
+// m0 <- normalise(m0 + dt/6 acc).
+// (u and unext, m0 and mout may be the same arrays: a thread reads its cell before it writes it)
+__global__ void k_rk4_stage(const float* m0, const float* u, const float* __restrict__ H,
+                            float* __restrict__ acc, float* unext, float* mout, long cells,
+                            float g, float alpha, float w, float a, float dt6, int first, int last) {
+    for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < cells; i += (long)gridDim.x * blockDim.x) {
+        const float ux = u[i], uy = u[i + cells], uz = u[i + 2 * cells];
+        const float Hx = H[i], Hy = H[i + cells], Hz = H[i + 2 * cells];
+        const float tx = uy * Hz - uz * Hy, ty = uz * Hx - ux * Hz, tz = ux * Hy - uy * Hx;          // u x H
+        const float dx = uy * tz - uz * ty, dy = uz * tx - ux * tz, dz = ux * ty - uy * tx;          // u x (u x H)
+        const float kx = -g * (tx + alpha * dx), ky = -g * (ty + alpha * dy), kz = -g * (tz + alpha * dz);
+        float ax = w * kx, ay = w * ky, az = w * kz;
+        if (!first) { ax += acc[i]; ay += acc[i + cells]; az += acc[i + 2 * cells]; }
+        const float px = m0[i], py = m0[i + cells], pz = m0[i + 2 * cells];
+        if (!last) {
+            acc[i] = ax; acc[i + cells] = ay; acc[i + 2 * cells] = az;
+            unext[i] = px + a * kx; unext[i + cells] = py + a * ky; unext[i + 2 * cells] = pz + a * kz;
+        } else {
+            const float nx = px + dt6 * ax, ny = py + dt6 * ay, nz = pz + dt6 * az;
+            const float inv = rsqrtf(nx * nx + ny * ny + nz * nz);
+            mout[i] = nx * inv; mout[i + cells] = ny * inv; mout[i + 2 * cells] = nz * inv;
+        }
+    }
+}
+
+int grid_for(long total) {
+    long g = (total + 255) / 256;
+    return (int)(g < 1 ? 1 : (g > 148L * 16 ? 148L * 16 : g));
+}
+
+}  // namespace
+
+struct boris_llg {
+    boris_demag_plan* plan;
+    Dims d;
+    double hx, hy, hz, Ms, A, alpha, gamma;
+    double Hext[3] = {0.0, 0.0, 0.0};
+    float *M = nullptr, *H = nullptr, *u = nullptr, *acc = nullptr;     // [3][nz][ny][nx] each
+};
+
+extern "C" {
+
+void boris_llg_destroy(boris_llg* s) {
+    if (!s) return;
+    cudaFree(s->M); cudaFree(s->H); cudaFree(s->u); cudaFree(s->acc);
+    delete s;
+}
+
+boris_llg* boris_llg_create(boris_demag_plan* plan, int nx, int ny, int nz, double hx, double hy, double hz,
+                            double Ms, double A, double alpha, double gamma) {
+    if (!plan || nx < 1 || ny < 1 || nz < 1 || !(hx > 0) || !(hy > 0) || !(hz > 0) || !(Ms > 0) || !(A >= 0) ||
+        !(alpha >= 0) || !(gamma > 0))
+        return nullptr;
+    int padded[3];
+    long long comp = 0;
+    if (boris_demag_plan_info(plan, &comp, nullptr, nullptr, padded, nullptr)) return nullptr;
+    boris_llg* s = new (std::nothrow) boris_llg();
+    if (!s) return nullptr;
+    s->plan = plan; s->d = Dims{nx, ny, nz};
+    s->hx = hx; s->hy = hy; s->hz = hz; s->Ms = Ms; s->A = A; s->alpha = alpha; s->gamma = gamma;
+    const size_t bytes = (size_t)3 * nx * ny * nz * sizeof(float);
+    if (cudaMalloc((void**)&s->M, bytes) != cudaSuccess || cudaMalloc((void**)&s->H, bytes) != cudaSuccess ||
+        cudaMalloc((void**)&s->u, bytes) != cudaSuccess || cudaMalloc((void**)&s->acc, bytes) != cudaSuccess) {
+        boris_llg_destroy(s);
+        return nullptr;
+    }
+    return s;
+}
+
+int boris_llg_set_applied_field(boris_llg* s, double Hx, double Hy, double Hz) {
+    if (!s || !std::isfinite(Hx) || !std::isfinite(Hy) || !std::isfinite(Hz)) return -1;
+    s->Hext[0] = Hx; s->Hext[1] = Hy; s->Hext[2] = Hz;
+    return 0;
+}
+
+int boris_llg_effective_field(boris_llg* s, const float* m, float* Heff, void* stream) {
+    if (!s || !m || !Heff || m == Heff) return -1;
+    cudaStream_t st = (cudaStream_t)stream;
+    const long cells = (long)s->d.nx * s->d.ny * s->d.nz, n = 3 * cells;
+    k_scale<<<grid_for(n), 256, 0, st>>>(m, s->M, (float)s->Ms, n);
+    if (int rc = boris_demag_apply(s->plan, s->M, Heff, stream)) return rc;
+    const double c = 2.0 * s->A / (kMu0 * s->Ms);
+    k_exchange_zeeman<<<grid_for(n), 256, 0, st>>>(m, Heff, s->d, (float)(c / (s->hx * s->hx)), (float)(c / (s->hy * s->hy)),
+                                                   (float)(c / (s->hz * s->hz)), (float)s->Hext[0], (float)s->Hext[1],
+                                                   (float)s->Hext[2]);
+    return cudaGetLastError() == cudaSuccess ? 0 : -2;
+}
+
+int boris_llg_rk4(boris_llg* s, float* m, double dt, int nsteps, void* stream) {
+    if (!s || !m || !(dt > 0) || nsteps < 0) return -1;
+    cudaStream_t st = (cudaStream_t)stream;
+    const long cells = (long)s->d.nx * s->d.ny * s->d.nz;
+    const float g = (float)(s->gamma / (1.0 + s->alpha * s->alpha)), al = (float)s->alpha;
+    const float w[4] = {1.f, 2.f, 2.f, 1.f};
+    const float a[4] = {(float)(0.5 * dt), (float)(0.5 * dt), (float)dt, 0.f};
+    for (int step = 0; step < nsteps; ++step) {
+        const float* u = m;                                      // stage state: m0, then the work array
+        for (int k = 0; k < 4; ++k) {
+            if (int rc = boris_llg_effective_field(s, u, s->H, stream)) return rc;
+            k_rk4_stage<<<grid_for(cells), 256, 0, st>>>(m, u, s->H, s->acc, s->u, m, cells, g, al, w[k], a[k],
+                                                         (float)(dt / 6.0), k == 0, k == 3);
+            u = s->u;
+        }
+    }
+    return cudaGetLastError() == cudaSuccess ? 0 : -2;
+}
+
+}  // extern "C"

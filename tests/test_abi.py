@@ -9,6 +9,7 @@ from paper_2008_02478_b200 import binding, build
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 HEADER = os.path.join(ROOT, "include", "boris_demag.h")
+HEADER_LLG = os.path.join(ROOT, "include", "boris_llg.h")
 
 
 @pytest.fixture(scope="session", autouse=True)
@@ -17,9 +18,9 @@ def built_library():
 
 
 def declared_symbols():
-    text = open(HEADER).read()
+    text = open(HEADER).read() + open(HEADER_LLG).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(boris_demag_\w+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(boris_(?:demag|llg)_\w+)\s*\(", text)))
 
 
 def test_header_declares_the_entry_points_the_north_star_names():
