@@ -16,30 +16,32 @@ constexpr double kMu0 = 4e-7 * 3.14159265358979323846264338327950288;
 
 struct Dims { int nx, ny, nz; };
 
-// M = Ms m  (the demag kernels take A/m)
-__global__ void k_scale(const float* __restrict__ m, float* __restrict__ M, float Ms, long n) {
-    for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) M[i] = Ms * m[i];
-}
-
-// Heff += cx (m[x+1] - 2 m + m[x-1]) + cy (...) + cz (...) + Hext, a missing neighbour contributing nothing
-// (homogeneous Neumann condition); c* = 2A / (mu0 Ms h*^2)
-__global__ void k_exchange_zeeman(const float* __restrict__ m, float* __restrict__ H, Dims d, float cx, float cy, float cz,
-                                  float hx, float hy, float hz) {
-    const long cells = (long)d.nx * d.ny * d.nz, total = 3 * cells;
-    for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total; idx += (long)gridDim.x * blockDim.x) {
-        long r = idx;
-        const int x = (int)(r % d.nx); r /= d.nx;
-        const int y = (int)(r % d.ny); r /= d.ny;
-        const int z = (int)(r % d.nz); const int c = (int)(r / d.nz);
-        const float v = m[idx];
-        float lap = 0.f;
-        if (x + 1 < d.nx) lap += cx * (m[idx + 1] - v);
-        if (x > 0) lap += cx * (m[idx - 1] - v);
-        if (y + 1 < d.ny) lap += cy * (m[idx + d.nx] - v);
-        if (y > 0) lap += cy * (m[idx - d.nx] - v);
-        if (z + 1 < d.nz) lap += cz * (m[idx + (long)d.nx * d.ny] - v);
-        if (z > 0) lap += cz * (m[idx - (long)d.nx * d.ny] - v);
-        H[idx] += lap + (c == 0 ? hx : (c == 1 ? hy : hz));
+// Heff = Ms Hd + cx (m[x+1] - 2 m + m[x-1]) + cy (...) + cz (...) + Hext on input Hd = H_demag(m) (the demag
+// operator is linear: H_demag(Ms m) = Ms H_demag(m), so the unit field goes through boris_demag_apply as it is);
+// a missing neighbour contributes nothing (homogeneous Neumann condition); c* = 2A / (mu0 Ms h*^2).
+// One block walks over rows (c, z, y); its threads over x.
+__global__ void k_exchange_zeeman(const float* __restrict__ m, float* __restrict__ H, Dims d, float Ms, float cx, float cy,
+                                  float cz, float hx, float hy, float hz) {
+    const long rows = 3L * d.nz * d.ny, plane = (long)d.nx * d.ny;
+    for (long row = blockIdx.x; row < rows; row += gridDim.x) {
+        const int y = (int)(row % d.ny);
+        const int z = (int)((row / d.ny) % d.nz);
+        const int c = (int)(row / ((long)d.ny * d.nz));
+        const float hext = c == 0 ? hx : (c == 1 ? hy : hz);
+        const float* mr = m + row * d.nx;
+        float* hr = H + row * d.nx;
+        const bool yp = y + 1 < d.ny, ym = y > 0, zp = z + 1 < d.nz, zm = z > 0;
+        for (int x = threadIdx.x; x < d.nx; x += blockDim.x) {
+            const float v = mr[x];
+            float lap = 0.f;
+            if (x + 1 < d.nx) lap += cx * (mr[x + 1] - v);
+            if (x > 0) lap += cx * (mr[x - 1] - v);
+            if (yp) lap += cy * (mr[x + d.nx] - v);
+            if (ym) lap += cy * (mr[x - d.nx] - v);
+            if (zp) lap += cz * (mr[x + plane] - v);
+            if (zm) lap += cz * (mr[x - plane] - v);
+            hr[x] = Ms * hr[x] + lap + hext;
+        }
     }
 }
 
@@ -82,14 +84,14 @@ struct boris_llg {
     Dims d;
     double hx, hy, hz, Ms, A, alpha, gamma;
     double Hext[3] = {0.0, 0.0, 0.0};
-    float *M = nullptr, *H = nullptr, *u = nullptr, *acc = nullptr;     // [3][nz][ny][nx] each
+    float *H = nullptr, *u = nullptr, *acc = nullptr;     // [3][nz][ny][nx] each
 };
 
 extern "C" {
 
 void boris_llg_destroy(boris_llg* s) {
     if (!s) return;
-    cudaFree(s->M); cudaFree(s->H); cudaFree(s->u); cudaFree(s->acc);
+    cudaFree(s->H); cudaFree(s->u); cudaFree(s->acc);
     delete s;
 }
 
@@ -106,8 +108,7 @@ boris_llg* boris_llg_create(boris_demag_plan* plan, int nx, int ny, int nz, doub
     s->plan = plan; s->d = Dims{nx, ny, nz};
     s->hx = hx; s->hy = hy; s->hz = hz; s->Ms = Ms; s->A = A; s->alpha = alpha; s->gamma = gamma;
     const size_t bytes = (size_t)3 * nx * ny * nz * sizeof(float);
-    if (cudaMalloc((void**)&s->M, bytes) != cudaSuccess || cudaMalloc((void**)&s->H, bytes) != cudaSuccess ||
-        cudaMalloc((void**)&s->u, bytes) != cudaSuccess || cudaMalloc((void**)&s->acc, bytes) != cudaSuccess) {
+    if (cudaMalloc((void**)&s->H, bytes) != cudaSuccess || cudaMalloc((void**)&s->u, bytes) != cudaSuccess || cudaMalloc((void**)&s->acc, bytes) != cudaSuccess) {
         boris_llg_destroy(s);
         return nullptr;
     }
@@ -123,13 +124,13 @@ int boris_llg_set_applied_field(boris_llg* s, double Hx, double Hy, double Hz) {
 int boris_llg_effective_field(boris_llg* s, const float* m, float* Heff, void* stream) {
     if (!s || !m || !Heff || m == Heff) return -1;
     cudaStream_t st = (cudaStream_t)stream;
-    const long cells = (long)s->d.nx * s->d.ny * s->d.nz, n = 3 * cells;
-    k_scale<<<grid_for(n), 256, 0, st>>>(m, s->M, (float)s->Ms, n);
-    if (int rc = boris_demag_apply(s->plan, s->M, Heff, stream)) return rc;
+    if (int rc = boris_demag_apply(s->plan, m, Heff, stream)) return rc;          // H_demag of the unit field
     const double c = 2.0 * s->A / (kMu0 * s->Ms);
-    k_exchange_zeeman<<<grid_for(n), 256, 0, st>>>(m, Heff, s->d, (float)(c / (s->hx * s->hx)), (float)(c / (s->hy * s->hy)),
-                                                   (float)(c / (s->hz * s->hz)), (float)s->Hext[0], (float)s->Hext[1],
-                                                   (float)s->Hext[2]);
+    const long rows = 3L * s->d.nz * s->d.ny;
+    const int threads = s->d.nx >= 256 ? 256 : (s->d.nx >= 64 ? 64 : 32);
+    k_exchange_zeeman<<<(unsigned)(rows < 148L * 32 ? rows : 148L * 32), threads, 0, st>>>(
+        m, Heff, s->d, (float)s->Ms, (float)(c / (s->hx * s->hx)), (float)(c / (s->hy * s->hy)), (float)(c / (s->hz * s->hz)),
+        (float)s->Hext[0], (float)s->Hext[1], (float)s->Hext[2]);
     return cudaGetLastError() == cudaSuccess ? 0 : -2;
 }
 
