@@ -128,7 +128,7 @@ int boris_llg_effective_field(boris_llg* s, const float* m, float* Heff, void* s
     const double c = 2.0 * s->A / (kMu0 * s->Ms);
     const long rows = 3L * s->d.nz * s->d.ny;
     const int threads = s->d.nx >= 256 ? 256 : (s->d.nx >= 64 ? 64 : 32);
-    k_exchange_zeeman<<<(unsigned)(rows < 148L * 32 ? rows : 148L * 32), threads, 0, st>>>(
+    k_exchange_zeeman<<<(unsigned)(rows < (1L << 20) ? rows : (1L << 20)), threads, 0, st>>>(
         m, Heff, s->d, (float)s->Ms, (float)(c / (s->hx * s->hx)), (float)(c / (s->hy * s->hy)), (float)(c / (s->hz * s->hz)),
         (float)s->Hext[0], (float)s->Hext[1], (float)s->Hext[2]);
     return cudaGetLastError() == cudaSuccess ? 0 : -2;
