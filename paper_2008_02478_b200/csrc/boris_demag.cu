@@ -37,7 +37,6 @@ int cuda_fail(cudaError_t e, const char* what) {
         if (e_ != cudaSuccess) return cuda_fail(e_, #call);       \
     } while (0)
 
-bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
 
 // ------------------------------------------------------------------ plan-time kernels (fp64)
 __global__ void k_tensor(double* N, int ncomp, int nx, int ny, int nz, double hx, double hy, double hz) {

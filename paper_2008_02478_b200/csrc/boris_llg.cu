@@ -47,34 +47,51 @@ __global__ void k_exchange_zeeman(const float* __restrict__ m, float* __restrict
 
 // One RK4 stage per cell: k = -g [u x H + alpha u x (u x H)]  (Eq. (1) solved for dm/dt, g = gamma / (1 + alpha^2));
 // acc = (first ? 0 : acc) + w k;  then either the next stage state u_next = m0 + a k, or (last) the step
-// m0 <- normalise(m0 + dt/6 acc).
-// (u and unext, m0 and mout may be the same arrays: a thread reads its cell before it writes it)
-__global__ void k_rk4_stage(const float* m0, const float* u, const float* __restrict__ H,
-                            float* __restrict__ acc, float* unext, float* mout, long cells,
-                            float g, float alpha, float w, float a, float dt6, int first, int last) {
-    for (long i = blockIdx.x * (long)blockDim.x + threadIdx.x; i < cells; i += (long)gridDim.x * blockDim.x) {
-        const float ux = u[i], uy = u[i + cells], uz = u[i + 2 * cells];
-        const float Hx = H[i], Hy = H[i + cells], Hz = H[i + 2 * cells];
-        const float tx = uy * Hz - uz * Hy, ty = uz * Hx - ux * Hz, tz = ux * Hy - uy * Hx;          // u x H
-        const float dx = uy * tz - uz * ty, dy = uz * tx - ux * tz, dz = ux * ty - uy * tx;          // u x (u x H)
-        const float kx = -g * (tx + alpha * dx), ky = -g * (ty + alpha * dy), kz = -g * (tz + alpha * dz);
-        float ax = w * kx, ay = w * ky, az = w * kz;
-        if (!first) { ax += acc[i]; ay += acc[i + cells]; az += acc[i + 2 * cells]; }
-        const float px = m0[i], py = m0[i + cells], pz = m0[i + 2 * cells];
-        if (!last) {
-            acc[i] = ax; acc[i + cells] = ay; acc[i + 2 * cells] = az;
-            unext[i] = px + a * kx; unext[i + cells] = py + a * ky; unext[i + 2 * cells] = pz + a * kz;
-        } else {
-            const float nx = px + dt6 * ax, ny = py + dt6 * ay, nz = pz + dt6 * az;
-            const float inv = rsqrtf(nx * nx + ny * ny + nz * nz);
-            mout[i] = nx * inv; mout[i + cells] = ny * inv; mout[i + 2 * cells] = nz * inv;
+// m0 <- normalise(m0 + dt/6 acc) (m0 and mout may be the same array: a thread reads its cell before it writes it).
+// The local field terms are gathered on the way (no separate pass over H): Hd is H_demag of the unit stage state
+// u, and H_eff = Ms Hd + exchange stencil of u + H_applied is formed per cell.  u and unext must be different
+// arrays (neighbours of u are read).  One block walks over rows (z, y); threads over x.
+__global__ void k_rk4_stage_fused(const float* m0, const float* __restrict__ u, const float* __restrict__ Hd,
+                                  float* __restrict__ acc, float* __restrict__ unext, float* mout, Dims d, float Ms, float cx,
+                                  float cy, float cz, float hx, float hy, float hz, float g, float alpha, float w, float a,
+                                  float dt6, int first, int last) {
+    const long rows = (long)d.nz * d.ny, plane = (long)d.nx * d.ny, cells = plane * d.nz;
+    for (long row = blockIdx.x; row < rows; row += gridDim.x) {
+        const int y = (int)(row % d.ny), z = (int)(row / d.ny);
+        const bool yp = y + 1 < d.ny, ym = y > 0, zp = z + 1 < d.nz, zm = z > 0;
+        for (int x = threadIdx.x; x < d.nx; x += blockDim.x) {
+            const long i = row * d.nx + x;
+            float uv[3], H[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const float* uc = u + c * cells + i;
+                const float v = uc[0];
+                float lap = 0.f;
+                if (x + 1 < d.nx) lap += cx * (uc[1] - v);
+                if (x > 0) lap += cx * (uc[-1] - v);
+                if (yp) lap += cy * (uc[d.nx] - v);
+                if (ym) lap += cy * (uc[-d.nx] - v);
+                if (zp) lap += cz * (uc[plane] - v);
+                if (zm) lap += cz * (uc[-plane] - v);
+                uv[c] = v;
+                H[c] = Ms * Hd[c * cells + i] + lap + (c == 0 ? hx : (c == 1 ? hy : hz));
+            }
+            const float tx = uv[1] * H[2] - uv[2] * H[1], ty = uv[2] * H[0] - uv[0] * H[2], tz = uv[0] * H[1] - uv[1] * H[0];
+            const float dx = uv[1] * tz - uv[2] * ty, dy = uv[2] * tx - uv[0] * tz, dz = uv[0] * ty - uv[1] * tx;
+            const float kx = -g * (tx + alpha * dx), ky = -g * (ty + alpha * dy), kz = -g * (tz + alpha * dz);
+            float ax = w * kx, ay = w * ky, az = w * kz;
+            if (!first) { ax += acc[i]; ay += acc[i + cells]; az += acc[i + 2 * cells]; }
+            const float px = m0[i], py = m0[i + cells], pz = m0[i + 2 * cells];
+            if (!last) {
+                acc[i] = ax; acc[i + cells] = ay; acc[i + 2 * cells] = az;
+                unext[i] = px + a * kx; unext[i + cells] = py + a * ky; unext[i + 2 * cells] = pz + a * kz;
+            } else {
+                const float nx = px + dt6 * ax, ny = py + dt6 * ay, nz = pz + dt6 * az;
+                const float inv = rsqrtf(nx * nx + ny * ny + nz * nz);
+                mout[i] = nx * inv; mout[i + cells] = ny * inv; mout[i + 2 * cells] = nz * inv;
+            }
         }
     }
-}
-
-int grid_for(long total) {
-    long g = (total + 255) / 256;
-    return (int)(g < 1 ? 1 : (g > 148L * 16 ? 148L * 16 : g));
 }
 
 }  // namespace
@@ -84,14 +101,14 @@ struct boris_llg {
     Dims d;
     double hx, hy, hz, Ms, A, alpha, gamma;
     double Hext[3] = {0.0, 0.0, 0.0};
-    float *H = nullptr, *u = nullptr, *acc = nullptr;     // [3][nz][ny][nx] each
+    float *H = nullptr, *u = nullptr, *u2 = nullptr, *acc = nullptr;     // [3][nz][ny][nx] each; u, u2: stage states
 };
 
 extern "C" {
 
 void boris_llg_destroy(boris_llg* s) {
     if (!s) return;
-    cudaFree(s->H); cudaFree(s->u); cudaFree(s->acc);
+    cudaFree(s->H); cudaFree(s->u); cudaFree(s->u2); cudaFree(s->acc);
     delete s;
 }
 
@@ -108,7 +125,8 @@ boris_llg* boris_llg_create(boris_demag_plan* plan, int nx, int ny, int nz, doub
     s->plan = plan; s->d = Dims{nx, ny, nz};
     s->hx = hx; s->hy = hy; s->hz = hz; s->Ms = Ms; s->A = A; s->alpha = alpha; s->gamma = gamma;
     const size_t bytes = (size_t)3 * nx * ny * nz * sizeof(float);
-    if (cudaMalloc((void**)&s->H, bytes) != cudaSuccess || cudaMalloc((void**)&s->u, bytes) != cudaSuccess || cudaMalloc((void**)&s->acc, bytes) != cudaSuccess) {
+    if (cudaMalloc((void**)&s->H, bytes) != cudaSuccess || cudaMalloc((void**)&s->u, bytes) != cudaSuccess ||
+        cudaMalloc((void**)&s->u2, bytes) != cudaSuccess || cudaMalloc((void**)&s->acc, bytes) != cudaSuccess) {
         boris_llg_destroy(s);
         return nullptr;
     }
@@ -141,13 +159,21 @@ int boris_llg_rk4(boris_llg* s, float* m, double dt, int nsteps, void* stream) {
     const float g = (float)(s->gamma / (1.0 + s->alpha * s->alpha)), al = (float)s->alpha;
     const float w[4] = {1.f, 2.f, 2.f, 1.f};
     const float a[4] = {(float)(0.5 * dt), (float)(0.5 * dt), (float)dt, 0.f};
+    const double c = 2.0 * s->A / (kMu0 * s->Ms);
+    const float cx = (float)(c / (s->hx * s->hx)), cy = (float)(c / (s->hy * s->hy)), cz = (float)(c / (s->hz * s->hz));
+    const long rows = (long)s->d.nz * s->d.ny;
+    const int threads = s->d.nx >= 256 ? 256 : (s->d.nx >= 64 ? 64 : 32);
+    const unsigned blocks = (unsigned)(rows < (1L << 20) ? rows : (1L << 20));
+    (void)cells;
     for (int step = 0; step < nsteps; ++step) {
-        const float* u = m;                                      // stage state: m0, then the work array
+        const float* u = m;                                      // stage state: m0, then the two work arrays in turn
         for (int k = 0; k < 4; ++k) {
-            if (int rc = boris_llg_effective_field(s, u, s->H, stream)) return rc;
-            k_rk4_stage<<<grid_for(cells), 256, 0, st>>>(m, u, s->H, s->acc, s->u, m, cells, g, al, w[k], a[k],
-                                                         (float)(dt / 6.0), k == 0, k == 3);
-            u = s->u;
+            float* un = (k & 1) ? s->u2 : s->u;
+            if (int rc = boris_demag_apply(s->plan, u, s->H, stream)) return rc;      // H_demag of the unit stage state
+            k_rk4_stage_fused<<<blocks, threads, 0, st>>>(m, u, s->H, s->acc, un, m, s->d, (float)s->Ms, cx, cy, cz,
+                                                          (float)s->Hext[0], (float)s->Hext[1], (float)s->Hext[2], g, al,
+                                                          w[k], a[k], (float)(dt / 6.0), k == 0, k == 3);
+            u = un;
         }
     }
     return cudaGetLastError() == cudaSuccess ? 0 : -2;

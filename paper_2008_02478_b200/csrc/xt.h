@@ -265,7 +265,6 @@ struct XInvT {
                     const int w = w0 + u * NT;
                     if (w < items) {
                         const int kp = w >> a.rbs, row = w & (a.rb - 1);
-                        const int km = LX - kp;
                         if (kp == 0) { Yk[u].y = 0.f; Ym[u].y = 0.f; }    // DC and Nyquist of a real row are real
                         const float2 E = bd_f2(Yk[u].x + Ym[u].x, Yk[u].y - Ym[u].y);
                         const float2 D = bd_f2(Yk[u].x - Ym[u].x, Yk[u].y + Ym[u].y);
