@@ -60,6 +60,9 @@ def kind_bytes(cfg, info):
         return {"XFwdT": 12 * N + sp, "YFused": 2 * sp + kst, "XInvT": sp + 12 * N}
     if info["path"] == 3:
         return {"XZFwd": 12 * N + sp, "YFused": 2 * sp + kst, "ZXInv": sp + 12 * N}
+    if info["path"] == 4:                    # plane path: X (unpadded) in, partial planes out (cols = ky residues)
+        pp = sp * (2 if info["cols"] > 1 else 1)
+        return {"XFwdT": 12 * N + sp, "YZFused": sp + kst + pp, "XInvP": pp + 12 * N}
     t = 8 * 3 * (nx + 1) * nz * 2 * ny       # y-padded scratch T over all chunks
     return {"XFwd": 12 * N + sp, "Y2D": 2 * sp + kst, "YFwd": sp + t, "ZFused": 2 * t + kst, "YInv": t + sp,
             "XInv": sp + 12 * N}

@@ -115,10 +115,12 @@ int boris_demag_plan_info(const boris_demag_plan* plan, long long* compulsory_by
 /* Which kernel path the plan uses and how much it stores (harness bookkeeping).
  * Any out pointer may be NULL.
  *   path                 = 2: tiled 2-D (XFwdT, YFused, XInvT), 3: tiled 3-D (XZFwd, YFused, ZXInv),
+ *                          4: plane path of nz = 32 slabs (XFwdT, YZFused, XInvP; csrc/plane.h),
  *                          0: chunked fallback (XFwd, [Y2D | YFwd, ZFused, YInv per chunk], XInv)
- *   spectrum_bytes       = bytes of the intermediate spectrum array in HBM (V or W)
+ *   spectrum_bytes       = bytes of the intermediate spectrum array in HBM (V, W or the plane path's X)
  *   kernel_storage_bytes = bytes of the stored fp32 kernel spectrum (with layout padding)
- *   cols                 = kx columns per tile of the tiled paths (0 otherwise) */
+ *   cols                 = kx columns per tile of the tiled paths, ky residues (partial planes) of the
+ *                          plane path (0 otherwise) */
 int boris_demag_plan_layout(const boris_demag_plan* plan, int* path, long long* spectrum_bytes,
                             long long* kernel_storage_bytes, int* cols);
 

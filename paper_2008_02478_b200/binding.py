@@ -170,7 +170,8 @@ class DemagPlan:
     # timing slots of boris_demag_apply_timed, named per kernel path (boris_demag_plan_layout)
     KINDS = {0: ("XFwd", "Y2D", "YFwd", "ZFused", "YInv", "XInv"),
              2: ("XFwdT", "YFused", "-", "-", "-", "XInvT"),
-             3: ("XZFwd", "YFused", "-", "-", "-", "ZXInv")}
+             3: ("XZFwd", "YFused", "-", "-", "-", "ZXInv"),
+             4: ("XFwdT", "YZFused", "-", "-", "-", "XInvP")}
 
     def apply_timed(self, M, H, stream=None):
         """boris_demag_apply_timed: {kind: (ms, launches)} of one evaluation.  Synchronous."""

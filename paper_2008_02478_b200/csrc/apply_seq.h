@@ -7,6 +7,7 @@
 
 #include "kernels.h"
 #include "khat_layout.h"
+#include "plane.h"
 #include "xt.h"
 #include "xz.h"
 #include "yfused.h"
@@ -23,6 +24,7 @@ struct LaunchCfg {
     int rbt;       // rows per block of XFwdT / XInvT
     int pf_y;      // L2 prefetch distance of YFused in blocks, 0: off (set by the plan)
     int pf_xz;     // ... of XZFwd
+    PlaneGeom plane;   // plane path (plane.h): thin slabs, takes precedence over the tiled path
 };
 
 // kx columns per tile of the tiled path: 3 * L * cols complex = 96 KB of shared memory
@@ -58,6 +60,7 @@ inline LaunchCfg make_launch_cfg(int nx, int ny, int nz) {
     c.rbt = nx >= 512 ? 8 : 4096 / nx;
     while (c.rbt > ny) c.rbt >>= 1;
     c.pf_y = 0; c.pf_xz = 0;       // set by the plan from the SM count
+    c.plane = plane_geom(nx, ny, nz);
     return c;
 }
 
@@ -87,6 +90,11 @@ struct PlanView {
     float2* V = nullptr;                               // tiled spectrum (tiled path)
     const float4* xpost = nullptr;                     // fill_xpost table (tiled path)
     EnergyArgs en = {nullptr, nullptr, nullptr, nullptr, 0.0};   // energy fused into the last kernel (tiled path)
+    // plane path (plane.h)
+    float2 *X = nullptr, *P = nullptr;
+    const float* KP = nullptr;
+    const int* kidx = nullptr;
+    const float2 *pl_tw = nullptr, *pl_zt = nullptr;
 };
 
 template <int L> struct IC { static constexpr int value = L; };
@@ -111,7 +119,7 @@ struct Grid { unsigned x, y; };
 
 inline int apply_launch_count(int nx, int nz, const LaunchCfg& c) {
     const int NS = nx + 1;
-    if (c.tiled) return 3;
+    if (c.plane.on || c.tiled) return 3;
     return nz == 1 ? 3 : 2 + 3 * ((NS + c.cs - 1) / c.cs);
 }
 
@@ -191,10 +199,60 @@ int enqueue_yfused3(Launcher& run, const PlanView& p) {
     });
 }
 
+// plane path (plane.h), nz = 32: XFwdT<LX,1> -> YZFused -> XInvP
+template <class Launcher>
+int enqueue_plane_x(Launcher& run, const PlanView& p, const float* M, float* H, bool fwd) {
+    const int nx = p.nx, ny = p.ny, nz = p.nz;
+    const PlaneGeom& g = p.cfg.plane;
+    if (fwd) {
+        XTArgs xa{M, H, p.X, p.ptw_x, p.xpost, ny, nx + 1, 16, 4, p.en};
+        const Grid gx{(unsigned)(3L * nz * ny / 16), 1};
+        return dispatch_len(nx, [&](auto ic) { return run.template run<XFwdT<decltype(ic)::value, 1>>(gx, xa); });
+    }
+    XPArgs ia{p.P, H, p.ptw_x, p.xpost, ny, nx + 1, g.lsp, 3L * nz * (nx + 1) * g.lsp, p.en};
+    const Grid gi{(unsigned)(3L * nz * ny / 16), 1};
+    return dispatch_len(nx, [&](auto ic) {
+        constexpr int LX = decltype(ic)::value;
+        switch (g.nq) {
+            case 1: return run.template run<XInvP<LX, 1>>(gi, ia);
+            case 2: return run.template run<XInvP<LX, 2>>(gi, ia);
+            case 4: return run.template run<XInvP<LX, 4>>(gi, ia);
+            default: return -1;
+        }
+    });
+}
+template <class Launcher>
+int enqueue_plane_yz(Launcher& run, const PlanView& p) {
+    const PlaneGeom& g = p.cfg.plane;
+    YZArgs ya{p.X, p.P, p.KP, p.kidx, p.pl_tw, p.pl_zt, p.nx + 1, p.ny};
+    const Grid gy{(unsigned)((p.nx + 1) * g.nq), 1};
+    auto go = [&](auto lsc) {
+        constexpr int LS = decltype(lsc)::value;
+        switch (g.nq) {
+            case 1: return run.template run<YZFused<LS, 1>>(gy, ya);
+            case 2: return run.template run<YZFused<LS, 2>>(gy, ya);
+            case 4: return run.template run<YZFused<LS, 4>>(gy, ya);
+            default: return -1;
+        }
+    };
+    switch (g.ls) {
+        case 64: return go(IC<64>{});
+        case 128: return go(IC<128>{});
+        case 256: return go(IC<256>{});
+        default: return -1;
+    }
+}
+
 // Launcher::run<K>(Grid, const K::Args&) -> 0 on success; Launcher::tiled_2d / xz / yfused3
 // forward to dispatch_tiled_2d / enqueue_xz / enqueue_yfused3.
 template <class Launcher>
 int enqueue_apply(Launcher& run, const PlanView& p, const float* M, float* H) {
+    if (p.cfg.plane.on) {
+        int rc = run.plane_x(p, M, H, true);
+        if (!rc) rc = run.plane_yz(p);
+        if (!rc) rc = run.plane_x(p, M, H, false);
+        return rc;
+    }
     if (p.cfg.tiled) {
         if (p.nz == 1) return run.tiled_2d(p, M, H);
         int rc = run.xz(p, M, H, true);

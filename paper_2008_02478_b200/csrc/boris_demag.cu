@@ -81,6 +81,22 @@ __global__ void k_fill_storage(float* Kst, KLayout kl, const double* Kred) {
         Kst[idx] = (float)storage_value(kl, idx, Kred);
 }
 
+__global__ void k_fill_plane(float* KP, PlaneK pk, const int* slot_ky, const double* Kred) {
+    const long total = pk.storage_elems();
+    for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total; idx += (long)gridDim.x * blockDim.x)
+        KP[idx] = (float)plane_storage_value(pk, idx, slot_ky, Kred);
+}
+__global__ void k_gather_plane(const float* KP, PlaneK pk, const int* kidx, float* out) {
+    const long total = 6L * (pk.nz + 1) * (pk.ny + 1) * (pk.nx + 1);
+    for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total; idx += (long)gridDim.x * blockDim.x) {
+        long r = idx;
+        const int kx = (int)(r % (pk.nx + 1)); r /= (pk.nx + 1);
+        const int ky = (int)(r % (pk.ny + 1)); r /= (pk.ny + 1);
+        const int kz = (int)(r % (pk.nz + 1)); const int c = (int)(r / (pk.nz + 1));
+        out[idx] = KP[plane_storage_index_of(pk, kidx, c, kz, ky, kx)];
+    }
+}
+
 __global__ void k_gather_natural(const float* Kst, KLayout kl, float* out) {
     const long total = kl.reduced_elems();
     for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total; idx += (long)gridDim.x * blockDim.x) {
@@ -96,7 +112,7 @@ __global__ void k_gather_natural(const float* Kst, KLayout kl, float* out) {
 
 // ------------------------------------------------------------------ energy (S8)
 constexpr int kEnergyBlocks = 592, kEnergyThreads = 256;
-constexpr int kFusedEnergySlots = 3 * 1024;      // blocks of XInvT (3 ny / rb) or ZXInv (3 ny), ny <= 1024
+constexpr int kFusedEnergySlots = 8192;          // blocks of XInvT (3 ny / rb), ZXInv (3 ny) or XInvP (3 nz ny / 16)
 
 __device__ __forceinline__ double warp_sum(double v) {
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -183,6 +199,13 @@ struct boris_demag_plan {
     float2* ptw_x = nullptr;         // tiled path: per-pass twiddles of the x / y transforms
     float2* ptw_y = nullptr;
     float4* xpost = nullptr;         // tiled path: fill_xpost table
+    // plane path (plane.h)
+    float2* X = nullptr;             // [3 nz][nx+1][ny]
+    float2* P = nullptr;             // [NQ][3 nz][nx+1][LSP]
+    float* KP = nullptr;             // kernel spectrum, plane order
+    int* kidx = nullptr;             // [NQ][LS]
+    float2* pl_tw = nullptr;
+    float2* pl_zt = nullptr;
     double* partial = nullptr;       // energy partial sums, followed by the ticket counter
     double* partial_f = nullptr;     // fused energy (apply_energy): one slot per block of the last kernel + ticket
     float* stage_M = nullptr;        // apply_host staging
@@ -222,6 +245,7 @@ int upload_pass_twiddles(boris_demag_plan* p, float2** dst, int L) {
 bd::PlanView plan_view(const boris_demag_plan* p) {
     bd::PlanView pv{p->nx, p->ny, p->nz, p->cfg, p->Kst, p->tw_x, p->tw_xpost, p->tw_y, p->tw_z, p->W, p->T};
     pv.ptw_x = p->ptw_x; pv.ptw_y = p->ptw_y; pv.V = p->V; pv.xpost = p->xpost;
+    pv.X = p->X; pv.P = p->P; pv.KP = p->KP; pv.kidx = p->kidx; pv.pl_tw = p->pl_tw; pv.pl_zt = p->pl_zt;
     return pv;
 }
 
@@ -282,10 +306,28 @@ int build_spectrum(boris_demag_plan* p) {
     const double scale = -1.0 / (2.0 * (double)kl.Px * (double)kl.Py * (double)kl.Pz);
     k_scale_sign<<<grid_for(nC, 256), 256>>>(dC, kl, scale);
     BD_TRY(cudaGetLastError());
-    if ((rc = dev_alloc(p, &p->Kst, (size_t)kl.storage_elems()))) { cleanup(); return rc; }
-    k_fill_storage<<<grid_for(kl.storage_elems(), 256), 256>>>(p->Kst, kl, dC);
-    BD_TRY(cudaGetLastError());
-    BD_TRY(cudaDeviceSynchronize());
+    if (p->cfg.plane.on) {
+        const bd::PlaneGeom& g = p->cfg.plane;
+        const bd::PlaneK pk = bd::make_plane_k(nx, ny, nz, g);
+        std::vector<int> kidx((size_t)g.nq * g.ls), slotky((size_t)g.nq * g.nsl);
+        bd::plane_fill_tables(ny, g, kidx.data(), slotky.data());
+        int* dslot = nullptr;
+        if ((rc = dev_alloc(p, &p->kidx, kidx.size()))) { cleanup(); return rc; }
+        if ((rc = dev_alloc(p, &p->KP, (size_t)pk.storage_elems()))) { cleanup(); return rc; }
+        BD_TRY(cudaMalloc((void**)&dslot, slotky.size() * sizeof(int)));
+        cudaMemcpy(dslot, slotky.data(), slotky.size() * sizeof(int), cudaMemcpyHostToDevice);
+        cudaMemcpy(p->kidx, kidx.data(), kidx.size() * sizeof(int), cudaMemcpyHostToDevice);
+        k_fill_plane<<<grid_for(pk.storage_elems(), 256), 256>>>(p->KP, pk, dslot, dC);
+        cudaError_t e1 = cudaGetLastError();
+        if (e1 == cudaSuccess) e1 = cudaDeviceSynchronize();
+        cudaFree(dslot);
+        BD_TRY(e1);
+    } else {
+        if ((rc = dev_alloc(p, &p->Kst, (size_t)kl.storage_elems()))) { cleanup(); return rc; }
+        k_fill_storage<<<grid_for(kl.storage_elems(), 256), 256>>>(p->Kst, kl, dC);
+        BD_TRY(cudaGetLastError());
+        BD_TRY(cudaDeviceSynchronize());
+    }
 #undef BD_TRY
     cleanup();
     return 0;
@@ -344,6 +386,7 @@ void boris_demag_plan_destroy(boris_demag_plan* p) {
     if (!p) return;
     cudaFree(p->Kst); cudaFree(p->tw_x); cudaFree(p->tw_xpost); cudaFree(p->tw_y); cudaFree(p->tw_z);
     cudaFree(p->W); cudaFree(p->T); cudaFree(p->partial); cudaFree(p->partial_f);
+    cudaFree(p->X); cudaFree(p->P); cudaFree(p->KP); cudaFree(p->kidx); cudaFree(p->pl_tw); cudaFree(p->pl_zt);
     cudaFree(p->V); cudaFree(p->ptw_x); cudaFree(p->ptw_y); cudaFree(p->xpost); cudaFree(p->Mp); cudaFree(p->Hp);
     cudaFree(p->stage_M); cudaFree(p->stage_H); cudaFree(p->stage_E);
     delete p;
@@ -378,7 +421,33 @@ boris_demag_plan* boris_demag_plan_create(int ux, int uy, int uz, double hx, dou
     if (!rc) rc = upload_twiddles(p, &p->tw_xpost, nx / 2 + 1, 2 * nx);
     if (!rc) rc = upload_twiddles(p, &p->tw_y, Py, Py);
     if (!rc && nz > 1) rc = upload_twiddles(p, &p->tw_z, Pz, Pz);
-    if (p->cfg.tiled) {
+    if (p->cfg.plane.on) {
+        const bd::PlaneGeom& g = p->cfg.plane;
+        if (!rc) rc = dev_alloc(p, &p->X, (size_t)3 * nz * (nx + 1) * ny);
+        if (!rc) rc = dev_alloc(p, &p->P, (size_t)g.nq * 3 * nz * (nx + 1) * g.lsp);
+        if (!rc) rc = upload_pass_twiddles(p, &p->ptw_x, nx);
+        if (!rc) {
+            std::vector<float4> h((size_t)nx / 2 + 1);
+            bd::fill_xpost(h.data(), nx);
+            rc = dev_alloc(p, &p->xpost, h.size());
+            if (!rc && cudaMemcpy(p->xpost, h.data(), h.size() * sizeof(float4), cudaMemcpyHostToDevice) != cudaSuccess)
+                rc = fail(-2, "cudaMemcpy xpost");
+        }
+        if (!rc) {
+            std::vector<float2> h((size_t)g.nq * g.ls);
+            bd::plane_fill_tw(h.data(), ny, g);
+            rc = dev_alloc(p, &p->pl_tw, h.size());
+            if (!rc && cudaMemcpy(p->pl_tw, h.data(), h.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess)
+                rc = fail(-2, "cudaMemcpy pl_tw");
+        }
+        if (!rc) {
+            std::vector<float2> h((size_t)g.zs * 16);
+            bd::plane_fill_zt(h.data(), nz, g);
+            rc = dev_alloc(p, &p->pl_zt, h.size());
+            if (!rc && cudaMemcpy(p->pl_zt, h.data(), h.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess)
+                rc = fail(-2, "cudaMemcpy pl_zt");
+        }
+    } else if (p->cfg.tiled) {
         const size_t nv = (size_t)3 * Pz * kl.ntl * ny * kl.cols;
         if (!rc) rc = dev_alloc(p, &p->V, nv);
         // the padding columns of the last tile are transformed along with the rest: keep them finite
@@ -450,7 +519,7 @@ int boris_demag_apply(boris_demag_plan* p, const float* M, float* H, void* strea
 int boris_demag_apply_energy(boris_demag_plan* p, const float* M, float* H, double* E_dev, void* stream) {
     if (!E_dev) return fail(-1, "null argument");
     if (int rc = check_fields(p, M, H, false)) return rc;
-    if (!p->cfg.tiled) {
+    if (!p->cfg.tiled && !p->cfg.plane.on) {
         if (int rc = boris_demag_apply(p, M, H, stream)) return rc;
         return boris_demag_energy(p, M, H, E_dev, stream);
     }
@@ -583,6 +652,13 @@ int boris_demag_plan_info(const boris_demag_plan* p, long long* compulsory_bytes
         const long long vbytes = 3LL * kl.Pz * kl.ntl * p->ny * kl.cols * (long long)sizeof(float2);
         *designed_hbm_bytes = 24 * N + 4 * vbytes + 4LL * kl.storage_elems();
     }
+    if (designed_hbm_bytes && p->cfg.plane.on) {
+        // M in, X out | X in, stored spectrum in, P out | P in, H out
+        const bd::PlaneGeom& g = p->cfg.plane;
+        const long long xb = 3LL * p->nz * (p->nx + 1) * p->ny * (long long)sizeof(float2);
+        const long long pb = (long long)g.nq * 3 * p->nz * (p->nx + 1) * g.lsp * (long long)sizeof(float2);
+        *designed_hbm_bytes = 24 * N + 2 * xb + 2 * pb + 4LL * bd::make_plane_k(p->nx, p->ny, p->nz, g).storage_elems();
+    }
     if (designed_hbm_bytes && p->padmode) *designed_hbm_bytes += 48LL * p->ux * p->uy * p->uz;   // staging in and out
     if (workspace_bytes) *workspace_bytes = p->bytes;
     if (padded) { padded[0] = kl.Px; padded[1] = kl.Py; padded[2] = kl.Pz; }
@@ -594,6 +670,14 @@ int boris_demag_plan_layout(const boris_demag_plan* p, int* path, long long* spe
                             long long* kernel_storage_bytes, int* cols) {
     if (!p) return fail(-1, "null plan");
     const bd::KLayout& kl = p->kl;
+    if (p->cfg.plane.on) {
+        const bd::PlaneGeom& g = p->cfg.plane;
+        if (path) *path = 4;
+        if (spectrum_bytes) *spectrum_bytes = 3LL * p->nz * (p->nx + 1) * p->ny * (long long)sizeof(float2);
+        if (kernel_storage_bytes) *kernel_storage_bytes = 4LL * bd::make_plane_k(p->nx, p->ny, p->nz, g).storage_elems();
+        if (cols) *cols = g.nq;
+        return 0;
+    }
     if (path) *path = p->cfg.tiled ? (p->nz == 1 ? 2 : 3) : 0;
     if (spectrum_bytes)
         *spectrum_bytes = p->cfg.tiled ? 3LL * kl.Pz * kl.ntl * p->ny * kl.cols * (long long)sizeof(float2)
@@ -608,7 +692,10 @@ int boris_demag_plan_kernel_spectrum(const boris_demag_plan* p, float* out_host)
     const long n = p->kl.reduced_elems();
     float* d = nullptr;
     BD_CUDA(cudaMalloc((void**)&d, (size_t)n * sizeof(float)));
-    k_gather_natural<<<grid_for(n, 256), 256>>>(p->Kst, p->kl, d);
+    if (p->cfg.plane.on)
+        k_gather_plane<<<grid_for(n, 256), 256>>>(p->KP, bd::make_plane_k(p->nx, p->ny, p->nz, p->cfg.plane), p->kidx, d);
+    else
+        k_gather_natural<<<grid_for(n, 256), 256>>>(p->Kst, p->kl, d);
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaMemcpy(out_host, d, (size_t)n * sizeof(float), cudaMemcpyDeviceToHost);
     cudaFree(d);

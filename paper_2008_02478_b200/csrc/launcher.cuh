@@ -41,6 +41,8 @@ int cu_yfused3(CudaLauncher& run, const PlanView& p);                           
 int cu_xz_small(CudaLauncher& run, const PlanView& p, const float* M, float* H, bool fwd);  // tu_xz_a.cu  nz 2..16
 int cu_xz_32(CudaLauncher& run, const PlanView& p, const float* M, float* H, bool fwd);     // tu_xz_b.cu  nz 32
 int cu_xz_big(CudaLauncher& run, const PlanView& p, const float* M, float* H, bool fwd);    // tu_xz_c.cu  nz 64..256
+int cu_plane_x(CudaLauncher& run, const PlanView& p, const float* M, float* H, bool fwd);   // tu_plane_x.cu
+int cu_plane_yz(CudaLauncher& run, const PlanView& p);                                      // tu_plane_yz.cu
 
 struct CudaLauncher {
     cudaStream_t st;
@@ -76,6 +78,8 @@ struct CudaLauncher {
     // hooks of enqueue_apply (apply_seq.h)
     int tiled_2d(const PlanView& p, const float* M, float* H) { return cu_tiled_2d(*this, p, M, H); }
     int yfused3(const PlanView& p) { return cu_yfused3(*this, p); }
+    int plane_x(const PlanView& p, const float* M, float* H, bool fwd) { return cu_plane_x(*this, p, M, H, fwd); }
+    int plane_yz(const PlanView& p) { return cu_plane_yz(*this, p); }
     int xz(const PlanView& p, const float* M, float* H, bool fwd) {
         if (p.nz <= 16) return cu_xz_small(*this, p, M, H, fwd);
         if (p.nz == 32) return cu_xz_32(*this, p, M, H, fwd);

@@ -1,0 +1,552 @@
+// plane.h — the plane path of thin slabs (nz = 32, the paper's pipelined regime
+// of few cells along z): the x spectrum stays y- and z-UNPADDED in HBM and the whole padded
+// (y, z) plane of one kx is transformed, multiplied by the kernel spectrum and transformed back
+// on chip (S2..S6 of SURVEY.md §8(a) in one launch, all 3 components).
+//
+//   XFwdT<LX,1>   S1          M -> X[cz = c nz + z][kx (nx+1)][y (ny)]          (xt.h, y fastest)
+//   YZFused       S2..S6      X -> P[q (NQ)][cz][kx][n (LSP)]                   (this file)
+//   XInvP         S7 (+S8)    P -> H, summing the NQ partial planes            (this file)
+//
+// The padded plane of one kx (3 x nz x Py complex) does not fit one SM, so the y transform is
+// split by the residue q of ky modulo NQ (decimation in frequency, first stage done on load):
+//     X^[q + NQ k] = sum_{n < LS} W_LS^(n k) a_q[n],   LS = Py / NQ,
+//     a_q[n] = W_Py^(n q) sum_r x[n + LS r] W_NQ^(q r)            (x = 0 beyond ny: r < NQ/2)
+// Block (kx, q) holds its 3 x nz pencils of LS points in shared memory (3 x 32 x 256 complex =
+// 204 KB with padding), runs the z transform, the multiply and the inverse z transform in
+// registers per ky column (4 lanes per column, 16 frequencies kz = 4 m + p each), transforms
+// back along y and writes its PARTIAL result
+//     P_q[n] = W_Py^(-n q) sum_k H^[q + NQ k] W_LS^(-n k),        n < LS,
+// of which the inverse x kernel forms  h[n + LS r] = sum_q W_NQ^(-q r) P_q[n]  (r < NQ/2 kept).
+// HBM per evaluation at 512x512x32: 0.10 + 0.20 | 0.20 + 0.25 + 0.40 | 0.40 + 0.10 GB = 1.66 GB
+// (the tiled path: 2.04 GB), all of it in pieces of at least 64 contiguous bytes.
+#pragma once
+#include "xt.h"
+#include "xz.h"
+
+namespace bd {
+
+constexpr int kKindYZFused = 1;          // timing slot of the fused kernel (as YFused)
+constexpr int kPlaneNZ = 32;             // slab thickness the plane path is built for
+
+BD_HD constexpr int pl_pe(int e) { return e + (e >> 4); }            // shared pencil padding: 1 per 16
+BD_HD constexpr int pl_pitch(int LS) { return LS + (LS >> 4); }
+// sub-transform of LS = R0 x 16 points, two passes: position e = q0 16 + q1 holds k = q0 + R0 q1
+BD_HD int pl_freq_of_pos(int LS, int e) { return e / 16 + (LS / 16) * (e % 16); }
+BD_HD int pl_pos_of_freq(int LS, int k) { return (k % (LS / 16)) * 16 + k / (LS / 16); }
+
+struct PlaneGeom {
+    int on;        // 1: the mesh takes the plane path
+    int nq;        // residues of ky (1, 2 or 4)
+    int ls;        // points of the sub-transform, Py / nq  (64, 128 or 256)
+    int lsp;       // stored points of a partial plane: min(ls, ny)
+    int zs;        // lanes per ky column, Pz / 16
+    int nsl;       // kernel-spectrum slots per residue, ls / 2 + 1
+};
+// nq_force > 0: take that many residues if the geometry allows it (tests)
+inline PlaneGeom plane_geom(int nx, int ny, int nz, int nq_force = 0) {
+    PlaneGeom g{0, 1, 0, 0, 0, 0};
+    if (nz != kPlaneNZ || nx < 4 || ny < 32 || ny > 512) return g;
+    const int Py = 2 * ny;
+    int nq = 1;
+    while (Py / nq > 256) nq *= 2;
+    if (nq_force > 0) nq = nq_force;
+    if (nq != 1 && nq != 2 && nq != 4) return g;
+    const int ls = Py / nq;
+    if (ls < 64 || ls > 256) return g;
+    g.on = 1; g.nq = nq; g.ls = ls; g.lsp = ls < ny ? ls : ny; g.zs = 2 * nz / 16; g.nsl = ls / 2 + 1;
+    return g;
+}
+
+// ------------------------------------------------------------------ kernel spectrum, plane order
+// KP[kx][qs (NQ)][c (6)][pr (ZS+1)][h (2)][slot (NSL)][4]   fp32
+// Slot s of residue qs stands for one ky = qs + NQ k <= Py/2 (the direct frequencies of block qs, in the
+// order of their positions e); entry (pr, h, i) holds kz = ZS (4 h + i) + pr for pr < ZS — the direct
+// frequencies kz <= Pz/2 of lane pr — and kz = ZS (4 h + i + 1) for pr = ZS (lane 0's mirror list, which
+// ends in the Nyquist plane).  A column at ky > Py/2 reads the slot of Py - ky (residue (NQ - q) % NQ) and
+// negates the y-odd components; a lane's mirrored frequencies kz = ZS m + p, m >= 8, read entry 15 - m of
+// residue (ZS - p) % ZS (pr = ZS for p = 0) and negate the z-odd components.
+// kidx[q LS + e] = slot | qs << 12 | (ky > Py/2) << 15
+struct PlaneK {
+    int nx, ny, nz, nq, ls, zs, nsl;
+    BD_HD long per_kx() const { return (long)nq * 6 * (zs + 1) * 2 * nsl * 4; }
+    BD_HD long storage_elems() const { return (long)(nx + 1) * per_kx(); }
+    BD_HD long index(int kx, int qs, int c, int pr, int h, int slot, int i) const {
+        return ((((((long)kx * nq + qs) * 6 + c) * (zs + 1) + pr) * 2 + h) * nsl + slot) * 4 + i;
+    }
+};
+inline PlaneK make_plane_k(int nx, int ny, int nz, const PlaneGeom& g) {
+    return PlaneK{nx, ny, nz, g.nq, g.ls, g.zs, g.nsl};
+}
+// host tables: kidx as above, slot_ky[qs nsl + slot] = ky of the slot (-1: unused)
+inline void plane_fill_tables(int ny, const PlaneGeom& g, int* kidx, int* slot_ky) {
+    const int Py = 2 * ny, LS = g.ls, NQ = g.nq, NSL = g.nsl;
+    for (int i = 0; i < NQ * NSL; ++i) slot_ky[i] = -1;
+    for (int qs = 0; qs < NQ; ++qs) {
+        int n = 0;
+        for (int e = 0; e < LS; ++e) {
+            const int ky = qs + NQ * pl_freq_of_pos(LS, e);
+            if (2 * ky <= Py) { kidx[qs * LS + e] = n | (qs << 12); slot_ky[qs * NSL + n] = ky; ++n; }
+        }
+    }
+    for (int q = 0; q < NQ; ++q)
+        for (int e = 0; e < LS; ++e) {
+            const int ky = q + NQ * pl_freq_of_pos(LS, e);
+            if (2 * ky <= Py) continue;
+            const int km = Py - ky, qs = km % NQ, em = pl_pos_of_freq(LS, (km - qs) / NQ);
+            kidx[q * LS + e] = (kidx[qs * LS + em] & 0xfff) | (qs << 12) | (1 << 15);
+        }
+}
+// value of storage element idx from the natural reduced spectrum Kred[c][kz <= nz][ky <= ny][kx <= nx]
+BD_HD double plane_storage_value(const PlaneK& k, long idx, const int* slot_ky, const double* Kred) {
+    const int i = (int)(idx % 4); idx /= 4;
+    const int slot = (int)(idx % k.nsl); idx /= k.nsl;
+    const int h = (int)(idx % 2); idx /= 2;
+    const int pr = (int)(idx % (k.zs + 1)); idx /= (k.zs + 1);
+    const int c = (int)(idx % 6); idx /= 6;
+    const int qs = (int)(idx % k.nq); const int kx = (int)(idx / k.nq);
+    const int ky = slot_ky[qs * k.nsl + slot];
+    if (ky < 0) return 0.0;
+    const int kz = pr < k.zs ? k.zs * (4 * h + i) + pr : k.zs * (4 * h + i + 1);
+    return Kred[(((long)c * (k.nz + 1) + kz) * (k.ny + 1) + ky) * (k.nx + 1) + kx];
+}
+// storage index that holds the natural reduced entry (c, kz, ky, kx)
+BD_HD long plane_storage_index_of(const PlaneK& k, const int* kidx, int c, int kz, int ky, int kx) {
+    const int qs = ky % k.nq, e = pl_pos_of_freq(k.ls, ky / k.nq);
+    const int slot = kidx[qs * k.ls + e] & 0xfff;
+    int pr = kz % k.zs, m = kz / k.zs;
+    if (m >= 8) { pr = k.zs; m = 7; }          // the Nyquist plane kz = Pz/2 = ZS 8
+    return k.index(kx, qs, c, pr, m / 4, slot, m % 4);
+}
+
+// tw[(q R0 + q0) 16 + j] = W_Py^(j (NQ q0 + q)): output twiddle of the first pass (j < 16, q0 < R0) with the
+// common factor W_Py^(j q) of the residue's input twiddle folded in
+inline void plane_fill_tw(float2* h, int ny, const PlaneGeom& g) {
+    const double pi = 3.14159265358979323846264338327950288;
+    const int Py = 2 * ny, R0 = g.ls / 16;
+    for (int q = 0; q < g.nq; ++q)
+        for (int q0 = 0; q0 < R0; ++q0)
+            for (int j = 0; j < 16; ++j) {
+                const long m = ((long)j * (g.nq * q0 + q)) % Py;
+                float2 w;
+                if ((4 * m) % Py == 0) {
+                    const float cx[4] = {1.f, 0.f, -1.f, 0.f}, sy[4] = {0.f, -1.f, 0.f, 1.f};
+                    w = bd_f2(cx[(4 * m) / Py], sy[(4 * m) / Py]);
+                } else {
+                    const double a = -2.0 * pi * (double)m / (double)Py;
+                    w = bd_f2((float)std::cos(a), (float)std::sin(a));
+                }
+                h[(q * R0 + q0) * 16 + j] = w;
+            }
+}
+// zt[p 16 + j] = W_Pz^(j p), p < ZS, j < 16
+inline void plane_fill_zt(float2* h, int nz, const PlaneGeom& g) {
+    const double pi = 3.14159265358979323846264338327950288;
+    const int Pz = 2 * nz;
+    for (int p = 0; p < g.zs; ++p)
+        for (int j = 0; j < 16; ++j) {
+            const int m = (j * p) % Pz;
+            float2 w;
+            if ((4 * m) % Pz == 0) {
+                const float cx[4] = {1.f, 0.f, -1.f, 0.f}, sy[4] = {0.f, -1.f, 0.f, 1.f};
+                w = bd_f2(cx[(4 * m) / Pz], sy[(4 * m) / Pz]);
+            } else {
+                const double a = -2.0 * pi * (double)m / (double)Pz;
+                w = bd_f2((float)std::cos(a), (float)std::sin(a));
+            }
+            h[p * 16 + j] = w;
+        }
+}
+
+// ------------------------------------------------------------------ YZFused (S2..S6)
+struct YZArgs {
+    const float2* X;       // [3 NZ][nkx][ny]
+    float2* P;             // [NQ][3 NZ][nkx][LSP]
+    const float* KP;       // kernel spectrum, plane order
+    const int* kidx;       // [NQ][LS]
+    const float2* tw;      // plane_fill_tw
+    const float2* zt;      // plane_fill_zt
+    int nkx;               // nx + 1
+    int ny;
+};
+
+// (-i)^Q b + a
+template <int Q>
+BD_HD float2 pl_add_rot(float2 a, float2 b) {
+    if constexpr (Q == 0) return pk_add(a, b);
+    else if constexpr (Q == 1) return pk_add_ib<-1>(a, b);
+    else if constexpr (Q == 2) return pk_sub(a, b);
+    else return pk_add_ib<+1>(a, b);
+}
+
+// H^ = K^ M^ at one frequency: k = (xx, yy, zz, xy, xz, yz), real
+BD_HD void pl_mul3(float kxx, float kyy, float kzz, float kxy, float kxz, float kyz, float2& mx, float2& my, float2& mz) {
+    const float2 hx = pk_fma(pk_bc(kxz), mz, pk_fma(pk_bc(kxy), my, pk_mul(pk_bc(kxx), mx)));
+    const float2 hy = pk_fma(pk_bc(kyz), mz, pk_fma(pk_bc(kyy), my, pk_mul(pk_bc(kxy), mx)));
+    const float2 hz = pk_fma(pk_bc(kzz), mz, pk_fma(pk_bc(kyz), my, pk_mul(pk_bc(kxz), mx)));
+    mx = hx; my = hy; mz = hz;
+}
+
+BD_HD float pl_f4(const float4& v, int i) { return i == 0 ? v.x : (i == 1 ? v.y : (i == 2 ? v.z : v.w)); }
+
+// One lane of a ky column: frequencies kz = 4 m + p, m < 16, of the 64-point z transform of the
+// 32 cells; returns its part y[c][j] of the inverse transform,
+//     out[j] = sum_p y_p[j],   out[j + 16] = sum_p i^p y_p[j]          (j < 16).
+// col: the column in shared memory (element z of component c at col[(c 32 + z) pitch]);
+// kA / kB: the lane's direct and mirror lists (float4 pointers at h = 0 of component 0), kcs / khs: float4
+// strides between components and halves; sy = -1 for a column at ky > Py/2.
+BD_HD void pl_zlane32(int p, float sy, const float2* col, int pitch, const float4* __restrict__ kA,
+                      const float4* __restrict__ kB, long kcs, long khs, const float2* __restrict__ zt,
+                      float2 (&v)[3][16]) {
+    // (-i)^p as the pair (c, (-s, s)) of a twiddle
+    Tw rot;
+    rot.c = p == 0 ? 1.f : (p == 2 ? -1.f : 0.f);
+    { const float s = p == 1 ? -1.f : (p == 3 ? 1.f : 0.f); rot.ns = bd_f2(-s, s); }
+    BD_UNROLL
+    for (int j = 0; j < 16; ++j) {
+        const Tw t = make_tw(BD_LDG(&zt[p * 16 + j]));
+        BD_UNROLL
+        for (int c = 0; c < 3; ++c) {
+            const float2 x0 = col[(c * 32 + j) * pitch], x1 = col[(c * 32 + j + 16) * pitch];
+            const float2 a = pk_fma(pk_swap(x1), rot.ns, pk_fma(x1, pk_bc(rot.c), x0));
+            v[c][j] = pk_cmul(a, t);
+        }
+    }
+    BD_UNROLL
+    for (int c = 0; c < 3; ++c) PkDft<16, -1>::run(v[c]);
+    // direct frequencies m = 0..7, then the mirrored ones m = 15 - i
+    BD_UNROLL
+    for (int h = 0; h < 2; ++h) {
+        float4 k[6];
+        BD_UNROLL
+        for (int c = 0; c < 6; ++c) k[c] = BD_LDG(kA + c * kcs + h * khs);
+        BD_UNROLL
+        for (int i = 0; i < 4; ++i) {
+            const int m = 4 * h + i;
+            pl_mul3(pl_f4(k[0], i), pl_f4(k[1], i), pl_f4(k[2], i), sy * pl_f4(k[3], i), pl_f4(k[4], i),
+                    sy * pl_f4(k[5], i), v[0][m], v[1][m], v[2][m]);
+        }
+    }
+    BD_UNROLL
+    for (int h = 0; h < 2; ++h) {
+        float4 k[6];
+        BD_UNROLL
+        for (int c = 0; c < 6; ++c) k[c] = BD_LDG(kB + c * kcs + h * khs);
+        BD_UNROLL
+        for (int i = 0; i < 4; ++i) {
+            const int m = 15 - (4 * h + i);
+            pl_mul3(pl_f4(k[0], i), pl_f4(k[1], i), pl_f4(k[2], i), sy * pl_f4(k[3], i), -pl_f4(k[4], i),
+                    -sy * pl_f4(k[5], i), v[0][m], v[1][m], v[2][m]);
+        }
+    }
+    BD_UNROLL
+    for (int c = 0; c < 3; ++c) PkDft<16, +1>::run(v[c]);
+    BD_UNROLL
+    for (int j = 0; j < 16; ++j) {
+        const Tw t = make_tw(BD_LDG(&zt[p * 16 + j]));
+        BD_UNROLL
+        for (int c = 0; c < 3; ++c) v[c][j] = pk_cmulc(v[c][j], t);
+    }
+}
+
+template <int LS, int NQ>
+struct YZFused {
+    using Args = YZArgs;
+    static constexpr int KIND = kKindYZFused;
+    static constexpr int NZ = kPlaneNZ, NPEN = 3 * NZ, ZS = 2 * NZ / 16;
+    static constexpr int NT = 384;
+    static constexpr int MINB = 1;
+    static constexpr int NPHASES = 5;
+    static constexpr int R0 = LS / 16;                   // first-pass radix; the second pass is radix 16
+    static constexpr int PITCH = pl_pitch(LS);
+    static constexpr int NSL = LS / 2 + 1;
+    static constexpr int LSP = NQ == 1 ? LS / 2 : LS;    // stored points of a partial plane
+    static constexpr int NIN = NQ == 1 ? R0 / 2 : R0;    // first-pass inputs that are not zero padding
+    static_assert(NT % 16 == 0 && NT % R0 == 0 && NT % 4 == 0, "thread mapping");
+    static BD_HD long smem_elems(const Args&) { return (long)NPEN * PITCH; }
+
+    // blockIdx.x = kx NQ + o; residues q and NQ - q (which read each other's kernel-spectrum slots) are neighbours
+    static BD_HD int q_of_order(int o) { return NQ == 4 ? ((o >> 1) | ((o & 1) << 1)) : o; }     // 0, 2, 1, 3
+
+    // constant input twiddle of the residue: z * W_(NQ R0)^(DIR r Q)
+    template <int DIR, int Q>
+    static BD_HD float2 in_tw(float2 z, int r) {
+        if constexpr (Q == 0) return z;
+        else return pk_mul_w64<DIR>(z, r * Q * (64 / (NQ * R0)));
+    }
+
+    // phase 0: load, residue stage and first pass (radix R0, stride 16) of every pencil
+    template <int Q>
+    static BD_HD void load_pass(int tid, int kx, const Args& a, float2* sm) {
+        constexpr int PG = NT / 16;
+        const int j = tid % 16, pg = tid / 16;
+        Tw tw[R0];
+        BD_UNROLL
+        for (int q0 = 0; q0 < R0; ++q0) tw[q0] = make_tw(BD_LDG(&a.tw[(Q * R0 + q0) * 16 + j]));
+        constexpr int NLD = NQ == 4 ? 2 * R0 : NIN;
+        float2 nxt[NLD];
+        auto issue = [&](int pc) {
+            const float2* xp = a.X + ((long)pc * a.nkx + kx) * a.ny + j;
+            BD_UNROLL
+            for (int r = 0; r < NIN; ++r) nxt[r] = BD_LDCG(xp + 16 * r);
+            if constexpr (NQ == 4) {
+                BD_UNROLL
+                for (int r = 0; r < R0; ++r) nxt[R0 + r] = BD_LDCG(xp + 16 * r + LS);
+            }
+        };
+        if (pg < NPEN) issue(pg);
+        for (int pc = pg; pc < NPEN; pc += PG) {
+            float2 v[R0];
+            BD_UNROLL
+            for (int r = 0; r < NIN; ++r) {
+                if constexpr (NQ == 4) v[r] = in_tw<-1, Q>(pl_add_rot<Q>(nxt[r], nxt[R0 + r]), r);
+                else v[r] = in_tw<-1, Q>(nxt[r], r);
+            }
+            if (pc + PG < NPEN) issue(pc + PG);
+            if constexpr (NQ == 1) PkDftPruned<R0, -1>::run(v);
+            else PkDft<R0, -1>::run(v);
+            float2* po = sm + pc * PITCH + j;
+            BD_UNROLL
+            for (int q0 = 0; q0 < R0; ++q0) {
+                if (Q == 0 && q0 == 0) po[0] = v[0];
+                else po[17 * q0] = pk_cmul(v[q0], tw[q0]);
+            }
+        }
+    }
+
+    // phases 1 and 3: second pass (radix 16 on 16 contiguous points), forward / inverse
+    template <int DIR>
+    static BD_HD void pass16(int tid, float2* sm) {
+        constexpr int PG = NT / R0;
+        const int q0 = tid % R0, pg = tid / R0;
+        for (int pc = pg; pc < NPEN; pc += PG) {
+            float2* ps = sm + pc * PITCH + 17 * q0;
+            float2 v[16];
+            BD_UNROLL
+            for (int i = 0; i < 16; ++i) v[i] = ps[i];
+            PkDft<16, DIR>::run(v);
+            BD_UNROLL
+            for (int i = 0; i < 16; ++i) ps[i] = v[i];
+        }
+    }
+
+    // phase 4: inverse first pass, residue stage, store of the partial plane
+    template <int Q>
+    static BD_HD void pass_store(int tid, int kx, const Args& a, float2* sm) {
+        constexpr int PG = NT / 16;
+        const int j = tid % 16, pg = tid / 16;
+        Tw tw[R0];
+        BD_UNROLL
+        for (int q0 = 0; q0 < R0; ++q0) tw[q0] = make_tw(BD_LDG(&a.tw[(Q * R0 + q0) * 16 + j]));
+        for (int pc = pg; pc < NPEN; pc += PG) {
+            const float2* pi = sm + pc * PITCH + j;
+            float2 v[R0];
+            BD_UNROLL
+            for (int q0 = 0; q0 < R0; ++q0) {
+                if (Q == 0 && q0 == 0) v[0] = pi[0];
+                else v[q0] = pk_cmulc(pi[17 * q0], tw[q0]);
+            }
+            if constexpr (NQ == 1) PkDftTrunc<R0, +1>::run(v);
+            else PkDft<R0, +1>::run(v);
+            float2* po = a.P + (((long)Q * NPEN + pc) * a.nkx + kx) * LSP + j;
+            BD_UNROLL
+            for (int r = 0; r < NIN; ++r) { const float2 o = in_tw<+1, Q>(v[r], r); BD_STCG(po + 16 * r, o); }
+        }
+    }
+
+    // phase 2: z transform, multiply, inverse z transform of every ky column; 4 lanes per column
+    static BD_HD void zstage(int tid, int kx, int q, const Args& a, float2* sm) {
+        const float4* kbase = reinterpret_cast<const float4*>(a.KP) + (long)kx * (NQ * 6L * (ZS + 1) * 2 * NSL);
+        constexpr long KCS = (long)(ZS + 1) * 2 * NSL, KHS = NSL;
+        for (int w = tid; w < LS * ZS; w += NT) {
+            const int p = w & (ZS - 1), e = w / ZS;
+            const int ki = BD_LDG(&a.kidx[q * LS + e]);
+            const int slot = ki & 0xfff, qs = (ki >> 12) & 7;
+            const float sy = (ki >> 15) ? -1.f : 1.f;
+            float2* col = sm + pl_pe(e);
+            const float4* kq = kbase + (long)qs * 6 * KCS + slot;
+#if defined(__CUDA_ARCH__)
+            float2 y[3][16];
+            pl_zlane32(p, sy, col, PITCH, kq + (long)p * 2 * NSL, kq + (long)(p ? ZS - p : ZS) * 2 * NSL, KCS, KHS, a.zt, y);
+            // out[j] = sum_p y_p[j], out[j + 16] = sum_p i^p y_p[j]: two exchange rounds among the 4 lanes
+            const bool hi = (p & 2) != 0, lo = (p & 1) != 0;
+            const float sg = hi ? -1.f : 1.f;
+            float2 S[3][8], D[3][8];
+            BD_UNROLL
+            for (int c = 0; c < 3; ++c) {
+                BD_UNROLL
+                for (int i = 0; i < 8; ++i) {
+                    const float2 send = hi ? y[c][i] : y[c][8 + i], mine = hi ? y[c][8 + i] : y[c][i];
+                    float2 oth;
+                    oth.x = __shfl_xor_sync(0xffffffffu, send.x, 2);
+                    oth.y = __shfl_xor_sync(0xffffffffu, send.y, 2);
+                    S[c][i] = pk_add(mine, oth);
+                    D[c][i] = pk_mul(pk_sub(mine, oth), pk_bc(sg));
+                }
+            }
+            const int jb = (hi ? 8 : 0) + (lo ? 4 : 0);
+            BD_UNROLL
+            for (int c = 0; c < 3; ++c) {
+                BD_UNROLL
+                for (int i = 0; i < 4; ++i) {
+                    const float2 sS = lo ? S[c][i] : S[c][4 + i], sD = lo ? D[c][i] : D[c][4 + i];
+                    const float2 kS = lo ? S[c][4 + i] : S[c][i], kD = lo ? D[c][4 + i] : D[c][i];
+                    float2 rS, rD;
+                    rS.x = __shfl_xor_sync(0xffffffffu, sS.x, 1);
+                    rS.y = __shfl_xor_sync(0xffffffffu, sS.y, 1);
+                    rD.x = __shfl_xor_sync(0xffffffffu, sD.x, 1);
+                    rD.y = __shfl_xor_sync(0xffffffffu, sD.y, 1);
+                    const float2 ev = lo ? rD : kD, od = lo ? kD : rD;
+                    col[(c * 32 + jb + i) * PITCH] = pk_add(kS, rS);
+                    col[(c * 32 + 16 + jb + i) * PITCH] = pk_add_ib<+1>(ev, od);
+                }
+            }
+#else
+            // host emulation (tests/emu): lane 0 of a column runs the four lanes in turn, same arithmetic
+            if (p != 0) continue;
+            float2 y[4][3][16];
+            for (int pp = 0; pp < ZS; ++pp)
+                pl_zlane32(pp, sy, col, PITCH, kq + (long)pp * 2 * NSL, kq + (long)(pp ? ZS - pp : ZS) * 2 * NSL, KCS, KHS,
+                           a.zt, y[pp]);
+            for (int c = 0; c < 3; ++c)
+                for (int j = 0; j < 16; ++j) {
+                    const float2 Se = pk_add(y[0][c][j], y[2][c][j]), So = pk_add(y[1][c][j], y[3][c][j]);
+                    const float2 De = pk_sub(y[0][c][j], y[2][c][j]), Do = pk_sub(y[1][c][j], y[3][c][j]);
+                    col[(c * 32 + j) * PITCH] = pk_add(Se, So);
+                    col[(c * 32 + 16 + j) * PITCH] = pk_add_ib<+1>(De, Do);
+                }
+#endif
+        }
+    }
+
+    template <int PH>
+    static BD_HD void phase(int tid, int bx, int by, const Args& a, float2* sm) {
+        const int kx = bx / NQ, q = q_of_order(bx % NQ);
+        if constexpr (PH == 0) {
+            if (q == 0) load_pass<0>(tid, kx, a, sm);
+            if constexpr (NQ >= 2) { if (q == 1) load_pass<1>(tid, kx, a, sm); }
+            if constexpr (NQ == 4) { if (q == 2) load_pass<2>(tid, kx, a, sm); else if (q == 3) load_pass<3>(tid, kx, a, sm); }
+        } else if constexpr (PH == 1) {
+            pass16<-1>(tid, sm);
+        } else if constexpr (PH == 2) {
+            zstage(tid, kx, q, a, sm);
+        } else if constexpr (PH == 3) {
+            pass16<+1>(tid, sm);
+        } else {
+            if (q == 0) pass_store<0>(tid, kx, a, sm);
+            if constexpr (NQ >= 2) { if (q == 1) pass_store<1>(tid, kx, a, sm); }
+            if constexpr (NQ == 4) { if (q == 2) pass_store<2>(tid, kx, a, sm); else if (q == 3) pass_store<3>(tid, kx, a, sm); }
+        }
+    }
+};
+
+// ------------------------------------------------------------------ XInvP (S7, S8 on the way)
+struct XPArgs {
+    const float2* P;       // [NQ][3 nz][nkx][LSP]
+    float* H;              // [3][nz][ny][nx]
+    const float2* ptw;     // per-pass twiddles of length LX
+    const float4* xpost;   // fill_xpost table
+    int ny;
+    int nkx;               // nx + 1
+    int lsp;               // stored points of a partial plane
+    long qstride;          // elements between partial planes
+    EnergyArgs en;         // energy gathered while H is written (en.M == nullptr: off)
+};
+
+// rows of H that are not consecutive: row = hi JB + lo sits at y0 + lo + hi (hi_pitch / pitch)
+struct GRowsOutMap {
+    float* p; long pitch; long hi_pitch; int jbs;
+    static BD_HD constexpr int off(int S, int r) { return r * S; }
+    BD_HD float2* ptr(int row, int e) const {
+        return reinterpret_cast<float2*>(p + (row & ((1 << jbs) - 1)) * pitch + (row >> jbs) * hi_pitch) + e;
+    }
+    BD_HD void st(float2* q, float2 v) const { *q = v; }
+    BD_HD void pre(const float2*, int) const {}
+    BD_HD void stq(float2* q, float2 v, int) const { *q = v; }
+};
+struct GRowsOutMapE {
+    float* p; long pitch; long hi_pitch; int jbs; long m_minus_h; double* acc;
+    static BD_HD constexpr int off(int S, int r) { return r * S; }
+    BD_HD float2* ptr(int row, int e) const {
+        return reinterpret_cast<float2*>(p + (row & ((1 << jbs) - 1)) * pitch + (row >> jbs) * hi_pitch) + e;
+    }
+    mutable float2 mbuf[8];
+    BD_HD void pre(const float2* q, int r) const {
+        mbuf[r] = BD_LDCG(reinterpret_cast<const float2*>(reinterpret_cast<const char*>(q) + m_minus_h));
+    }
+    BD_HD void stq(float2* q, float2 v, int r) const {
+        *q = v;
+        *acc += (double)mbuf[r].x * v.x + (double)mbuf[r].y * v.y;
+    }
+    BD_HD void st(float2* q, float2 v) const { *q = v; }
+};
+
+// Z[kp], Z[LX - kp] of the half-length complex row from the spectrum pair Y[kp], Y[LX - kp] (xt.h header)
+BD_HD void xinv_pre(int LX, int kp, float2 Yk, float2 Ym, const float4& xp, float2* zr) {
+    if (kp == 0) { Yk.y = 0.f; Ym.y = 0.f; }            // DC and Nyquist of a real row are real
+    const float2 E = bd_f2(Yk.x + Ym.x, Yk.y - Ym.y);
+    const float2 D = bd_f2(Yk.x - Ym.x, Yk.y + Ym.y);
+    const float2 O = pk_cmulc(D, make_tw(bd_f2(xp.x, xp.y)));
+    zr[bd_float_as_int(xp.z)] = bd_f2(E.x - O.y, E.y + O.x);
+    if (kp != 0 && 2 * kp != LX) zr[bd_float_as_int(xp.w)] = bd_f2(E.x + O.y, O.x - E.y);
+}
+
+template <int LX, int NQ>
+struct XInvP {
+    using Args = XPArgs;
+    static constexpr int KIND = kKindXInvT;
+    static constexpr int NT = 256;
+    static constexpr int MINB = LX >= 1024 ? 1 : 3;
+    static constexpr int NP = dec_np(LX);
+    static constexpr int NPHASES = NP + 1;
+    static constexpr int RB = 16;                        // rows of H per block
+    static constexpr int JB = NQ == 4 ? 8 : 16, JBS = NQ == 4 ? 3 : 4;   // points of a partial plane per block
+    static BD_HD long smem_elems(const Args&) { return (long)RB * SRows<LX>::PITCH; }
+
+    template <int PH>
+    static BD_HD void phase(int tid, int bx, int by, const Args& a, float2* sm) {
+        const int bpc = a.lsp / JB;                        // blocks per (c, z)
+        const int cz = bx / bpc, j0 = (bx - cz * bpc) * JB;
+        SRows<LX> s{sm};
+        if constexpr (PH == 0) {
+            constexpr int items = (LX / 2 + 1) * JB;
+            for (int w = tid; w < items; w += NT) {
+                const int kp = w >> JBS, jj = w & (JB - 1), km = LX - kp;
+                const float4 xp = BD_LDG(&a.xpost[kp]);
+                const float2* pk = a.P + ((long)cz * a.nkx + kp) * a.lsp + j0 + jj;
+                const float2* pm = a.P + ((long)cz * a.nkx + km) * a.lsp + j0 + jj;
+                float2 ak[NQ], am[NQ];
+                BD_UNROLL
+                for (int q = 0; q < NQ; ++q) { ak[q] = BD_LDCG(pk + q * a.qstride); am[q] = BD_LDCG(pm + q * a.qstride); }
+                if constexpr (NQ == 4) {
+                    // h[n] = P0 + P1 + P2 + P3,  h[n + LS] = P0 + i P1 - P2 - i P3
+                    const float2 Yk0 = pk_add(pk_add(ak[0], ak[2]), pk_add(ak[1], ak[3]));
+                    const float2 Ym0 = pk_add(pk_add(am[0], am[2]), pk_add(am[1], am[3]));
+                    const float2 Yk1 = pk_add_ib<+1>(pk_sub(ak[0], ak[2]), pk_sub(ak[1], ak[3]));
+                    const float2 Ym1 = pk_add_ib<+1>(pk_sub(am[0], am[2]), pk_sub(am[1], am[3]));
+                    xinv_pre(LX, kp, Yk0, Ym0, xp, sm + jj * SRows<LX>::PITCH);
+                    xinv_pre(LX, kp, Yk1, Ym1, xp, sm + (JB + jj) * SRows<LX>::PITCH);
+                } else if constexpr (NQ == 2) {
+                    xinv_pre(LX, kp, pk_add(ak[0], ak[1]), pk_add(am[0], am[1]), xp, sm + jj * SRows<LX>::PITCH);
+                } else {
+                    xinv_pre(LX, kp, ak[0], am[0], xp, sm + jj * SRows<LX>::PITCH);
+                }
+            }
+        } else if constexpr (PH < NP) {
+            x_rows_pass<LX, NP - PH, true, NT>(tid, RB, s, s, a.ptw);
+        } else {
+            // row = hi JB + lo  ->  y = j0 + lo + hi lsp   (hi = 1 only for NQ = 4, where lsp = ny / 2)
+            float* h0 = a.H + ((long)cz * a.ny + j0) * LX;
+            if (a.en.M) {
+                double acc = 0.0;
+                GRowsOutMapE out{h0, LX, (long)a.lsp * LX, JBS, (long)((const char*)a.en.M - (const char*)a.H), &acc};
+                x_rows_pass<LX, 0, true, NT>(tid, RB, s, out, a.ptw);
+                energy_finish(acc, a.en);
+            } else {
+                GRowsOutMap out{h0, LX, (long)a.lsp * LX, JBS};
+                x_rows_pass<LX, 0, true, NT>(tid, RB, s, out, a.ptw);
+            }
+        }
+    }
+};
+
+}  // namespace bd

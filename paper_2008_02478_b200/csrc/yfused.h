@@ -95,6 +95,7 @@ struct GTile {                 // global: V tile [y][col], component stride cstr
 template <int L, int P, int NCT = 0, class In, class Out>
 BD_HD void fwd_passM(int it, int c0, int cstep, int cend, const In& in, const Out& out, const float2* __restrict__ ptw) {
     constexpr int NP = dec_np(L), R = dec_r(L, P), Lp = dec_sublen(L, P), S = Lp / R;
+    if (c0 >= cend) return;      // more row groups than rows: nothing to do (and nothing to read)
     const int blk = it / S, j = it - blk * S, base = blk * Lp + j;
     Tw tw[R];
     if constexpr (P < NP - 1) {
@@ -135,6 +136,7 @@ BD_HD void fwd_passM(int it, int c0, int cstep, int cend, const In& in, const Ou
 template <int L, int P, int NCT = 0, class In, class Out>
 BD_HD void inv_passM(int it, int c0, int cstep, int cend, const In& in, const Out& out, const float2* __restrict__ ptw) {
     constexpr int NP = dec_np(L), R = dec_r(L, P), Lp = dec_sublen(L, P), S = Lp / R;
+    if (c0 >= cend) return;
     const int blk = it / S, j = it - blk * S, base = blk * Lp + j;
     Tw tw[R];
     if constexpr (P < NP - 1) {

@@ -52,6 +52,8 @@ struct HostLauncher {
     int tiled_2d(const bd::PlanView& p, const float* M, float* H) { return bd::dispatch_tiled_2d(*this, p, M, H); }
     int yfused3(const bd::PlanView& p) { return bd::enqueue_yfused3(*this, p); }
     int xz(const bd::PlanView& p, const float* M, float* H, bool fwd) { return bd::enqueue_xz<2, 256>(*this, p, M, H, fwd); }
+    int plane_x(const bd::PlanView& p, const float* M, float* H, bool fwd) { return bd::enqueue_plane_x(*this, p, M, H, fwd); }
+    int plane_yz(const bd::PlanView& p) { return bd::enqueue_plane_yz(*this, p); }
 };
 
 }  // namespace
@@ -82,11 +84,19 @@ extern "C" {
 // Kred: natural reduced spectrum [ncomp][nzr][nyr][nxr] in fp64 including the folded
 // factor (as boris_demag_spectrum_host returns it).  M, H: fp32 [3][nz][ny][nx].
 // cs_override > 0 forces the number of kx slots per chunk (to exercise chunking).
+// nq_plane > 0: plane path with that many ky residues; 0: the plan's own choice; < 0: no plane path
+int emu_apply_ex(int nx, int ny, int nz, const double* Kred, const float* M, float* H, int cs_override, int nq_plane);
 int emu_apply(int nx, int ny, int nz, const double* Kred, const float* M, float* H, int cs_override) {
+    return emu_apply_ex(nx, ny, nz, Kred, M, H, cs_override, cs_override != 0 ? -1 : 0);
+}
+int emu_apply_ex(int nx, int ny, int nz, const double* Kred, const float* M, float* H, int cs_override, int nq_plane) {
     using namespace bd;
     LaunchCfg cfg = make_launch_cfg(nx, ny, nz);
     if (cs_override > 0) cfg.cs = cs_override;
     if (cs_override < 0) cfg.tiled = 0;          // force the untiled kernels
+    if (nq_plane < 0) cfg.plane.on = 0;
+    if (nq_plane > 0) cfg.plane = plane_geom(nx, ny, nz, nq_plane);
+    if (nq_plane > 0 && !cfg.plane.on) return -1;
     const KLayout kl = cfg.tiled ? make_klayout_tiled(nx, ny, nz, cfg.cols) : make_klayout(nx, ny, nz, cfg.ty);
     const int Py = 2 * ny, Pz = nz > 1 ? 2 * nz : 1, NS = nx + 1;
     std::vector<float> Kst((size_t)kl.storage_elems());
@@ -107,6 +117,33 @@ int emu_apply(int nx, int ny, int nz, const double* Kred, const float* M, float*
     std::vector<float4> xpost((size_t)nx / 2 + 1);
     fill_xpost(xpost.data(), nx);
     pv.ptw_x = ptwx.data(); pv.ptw_y = ptwy.data(); pv.V = V.data(); pv.xpost = xpost.data();
+    std::vector<float2> PX, PP, pltw, plzt;
+    std::vector<float> KP;
+    std::vector<int> kidx, slotky;
+    if (cfg.plane.on) {
+        const PlaneGeom& g = cfg.plane;
+        const PlaneK pk = make_plane_k(nx, ny, nz, g);
+        kidx.resize((size_t)g.nq * g.ls); slotky.resize((size_t)g.nq * g.nsl);
+        plane_fill_tables(ny, g, kidx.data(), slotky.data());
+        KP.resize((size_t)pk.storage_elems());
+        for (long i = 0; i < pk.storage_elems(); ++i) KP[(size_t)i] = (float)plane_storage_value(pk, i, slotky.data(), Kred);
+        // round trip of the layout: every natural entry is found where plane_storage_index_of says
+        for (int c = 0; c < 6; ++c)
+            for (int kz = 0; kz <= nz; ++kz)
+                for (int ky = 0; ky <= ny; ++ky)
+                    for (int kx = 0; kx <= nx; kx += (nx > 8 ? nx / 4 : 1)) {
+                        const long si = plane_storage_index_of(pk, kidx.data(), c, kz, ky, kx);
+                        const double ref = Kred[(((long)c * (nz + 1) + kz) * (ny + 1) + ky) * (nx + 1) + kx];
+                        if (si < 0 || si >= pk.storage_elems() || KP[(size_t)si] != (float)ref) return -200;
+                    }
+        PX.assign((size_t)3 * nz * (nx + 1) * ny, poison);
+        PP.assign((size_t)g.nq * 3 * nz * (nx + 1) * g.lsp, poison);
+        pltw.resize((size_t)g.nq * (g.ls / 16) * 16); plzt.resize((size_t)g.zs * 16);
+        plane_fill_tw(pltw.data(), ny, g);
+        plane_fill_zt(plzt.data(), nz, g);
+        pv.X = PX.data(); pv.P = PP.data(); pv.KP = KP.data(); pv.kidx = kidx.data();
+        pv.pl_tw = pltw.data(); pv.pl_zt = plzt.data();
+    }
     HostLauncher run;
     const int rc = enqueue_apply(run, pv, M, H);
     if (rc) return rc;

@@ -100,6 +100,13 @@ MEDIUM = [
     ((8, 512, 32), (2e-9, 2e-9, 1e-9), "helix"),          # Py = 1024 as in C5
     ((256, 4, 16), (2e-9, 2e-9, 2e-9), "random"),         # z columns in 16 passes of 32 points
     ((32, 16, 1024), (2e-9, 2e-9, 1e-9), "helix"),        # nz rows of nx = 1024 exceed shared memory: chunked fallback
+    ((32, 16, 16), (2e-9, 2e-9, 1e-9), "random"),         # nz = 32 but too few rows for the plane path: tiled 3-D
+    # plane path (csrc/plane.h): nz = 32, ny = 32..512
+    ((32, 32, 8), (2e-9, 3e-9, 1e-9), "random"),          # sub-transform of 64 points, one ky residue
+    ((32, 128, 64), (2e-9, 2e-9, 1e-9), "random"),        # 256 points, one residue
+    ((32, 256, 16), (5e-9, 4e-9, 3e-9), "vortex"),        # two residues
+    ((32, 512, 8), (2e-9, 2e-9, 1e-9), "helix"),          # four residues: C5's y and z
+    ((32, 64, 1024), (2e-9, 2e-9, 1e-9), "helix"),        # LX = 1024 rows on the plane path
 ]
 
 
@@ -199,7 +206,7 @@ def test_float3_layout_and_accumulate_variants_give_the_same_field(shape):
 
 
 def test_kernel_path_chosen_per_mesh():
-    expect = {(1, 32, 32): 2, (1, 1024, 1024): 2, (128, 128, 128): 3, (32, 512, 512): 3, (32, 16, 1024): 0, (512, 2, 4): 0}
+    expect = {(1, 32, 32): 2, (1, 1024, 1024): 2, (128, 128, 128): 3, (32, 512, 512): 4, (32, 256, 16): 4, (16, 512, 512): 3, (32, 16, 1024): 0, (512, 2, 4): 0}
     for (nz, ny, nx), path in expect.items():
         plan = binding.DemagPlan(nx, ny, nz, 2e-9, 2e-9, 1e-9)
         assert plan.layout()["path"] == path

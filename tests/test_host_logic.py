@@ -188,3 +188,47 @@ def test_phases_do_not_depend_on_the_order_of_their_threads(emu, shape, cs):
         emu.emu_set_thread_order(0)
     assert np.isfinite(out[0]).all()
     assert np.array_equal(out[0], out[1]) and np.array_equal(out[0], out[2])
+
+
+# plane path (csrc/plane.h): nz = 32 slabs; nq = residues of ky (0: the plan's own choice)
+PLANE_CASES = [
+    ((32, 32, 4), (2.0, 2.0, 1.0), "random", 0),          # LS = 64, one residue (pruned first pass)
+    ((32, 64, 8), (5.0, 4.0, 3.0), "random", 2),          # LS = 64, two residues
+    ((32, 128, 4), (2.0, 2.0, 1.0), "helix", 4),          # LS = 64, four residues
+    ((32, 128, 4), (2.0, 2.0, 1.0), "random", 2),         # LS = 128
+    ((32, 128, 16), (2.0, 3.0, 1.0), "random", 0),        # LS = 256, one residue
+    ((32, 256, 4), (2.0, 2.0, 1.0), "random", 0),         # LS = 256, two residues
+    ((32, 512, 4), (2.0, 2.0, 1.0), "helix", 0),          # LS = 256, four residues: C5's y and z
+]
+
+
+@pytest.mark.parametrize("shape,h,texture,nq", PLANE_CASES)
+def test_emulated_plane_path_matches_the_oracle(emu, shape, h, texture, nq):
+    nz, ny, nx = shape
+    Ms = 8e5
+    M = W.make_texture(texture, shape, Ms, seed=13)
+    K = binding.spectrum_host(nx, ny, nz, *h)
+    H = np.full(M.shape, np.nan, np.float32)
+    assert emu.emu_apply_ex(nx, ny, nz, vp(K), vp(M), vp(H), 0, nq) == 0
+    H_ref = demag_fft(M, h)
+    err = np.abs(H - H_ref)
+    assert err.max() <= 1e-5 * Ms
+    assert np.sqrt((err ** 2).sum() / (H_ref ** 2).sum()) <= 2e-6
+
+
+def test_plane_path_phases_do_not_depend_on_thread_order(emu):
+    shape, h = (32, 128, 4), (2.0, 3.0, 1.0)
+    nz, ny, nx = shape
+    M = W.make_texture("random", shape, 8e5, seed=19)
+    K = binding.spectrum_host(nx, ny, nz, *h)
+    out = []
+    try:
+        for order in (0, 1, 2):
+            emu.emu_set_thread_order(order)
+            H = np.full(M.shape, np.nan, np.float32)
+            assert emu.emu_apply_ex(nx, ny, nz, vp(K), vp(M), vp(H), 0, 4) == 0
+            out.append(H)
+    finally:
+        emu.emu_set_thread_order(0)
+    assert np.isfinite(out[0]).all()
+    assert np.array_equal(out[0], out[1]) and np.array_equal(out[0], out[2])
