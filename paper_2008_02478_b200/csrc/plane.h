@@ -25,11 +25,15 @@
 
 namespace bd {
 
+#ifndef BD_YZ_NT
+#define BD_YZ_NT 384
+#endif
 constexpr int kKindYZFused = 1;          // timing slot of the fused kernel (as YFused)
 constexpr int kPlaneNZ = 32;             // slab thickness the plane path is built for
 
 BD_HD constexpr int pl_pe(int e) { return e + (e >> 4); }            // shared pencil padding: 1 per 16
-BD_HD constexpr int pl_pitch(int LS) { return LS + (LS >> 4); }
+// odd: the four lanes of a ky column store rows 4 apart (zstage), which then fall into different banks
+BD_HD constexpr int pl_pitch(int LS) { return (LS + (LS >> 4)) | 1; }
 // sub-transform of LS = R0 x 16 points, two passes: position e = q0 16 + q1 holds k = q0 + R0 q1
 BD_HD int pl_freq_of_pos(int LS, int e) { return e / 16 + (LS / 16) * (e % 16); }
 BD_HD int pl_pos_of_freq(int LS, int k) { return (k % (LS / 16)) * 16 + k / (LS / 16); }
@@ -192,50 +196,55 @@ BD_HD float pl_f4(const float4& v, int i) { return i == 0 ? v.x : (i == 1 ? v.y 
 // 32 cells; returns its part y[c][j] of the inverse transform,
 //     out[j] = sum_p y_p[j],   out[j + 16] = sum_p i^p y_p[j]          (j < 16).
 // col: the column in shared memory (element z of component c at col[(c 32 + z) pitch]);
-// kA / kB: the lane's direct and mirror lists (float4 pointers at h = 0 of component 0), kcs / khs: float4
-// strides between components and halves; sy = -1 for a column at ky > Py/2.
-BD_HD void pl_zlane32(int p, float sy, const float2* col, int pitch, const float4* __restrict__ kA,
-                      const float4* __restrict__ kB, long kcs, long khs, const float2* __restrict__ zt,
-                      float2 (&v)[3][16]) {
+// k: the lane's direct and mirror lists (pl_load_k: kA / kB point at h = 0 of component 0, kcs / khs are the float4
+// strides between components and halves); sy = -1 for a column at ky > Py/2.
+struct PlK { float4 d[2][6]; const float4* kB; };     // a lane's direct list [h][c]; its mirror list is read when needed
+BD_HD void pl_load_k(const float4* __restrict__ kA, const float4* __restrict__ kB, long kcs, long khs, PlK& k) {
+    BD_UNROLL
+    for (int h = 0; h < 2; ++h) {
+        BD_UNROLL
+        for (int c = 0; c < 6; ++c) k.d[h][c] = BD_LDG(kA + c * kcs + h * khs);
+    }
+    k.kB = kB;
+}
+BD_HD void pl_zlane32(int p, float sy, const float2* col, int pitch, const PlK& k, long kcs, long khs,
+                      const float2* __restrict__ zt, float2 (&v)[3][16]) {
     // (-i)^p as the pair (c, (-s, s)) of a twiddle
     Tw rot;
     rot.c = p == 0 ? 1.f : (p == 2 ? -1.f : 0.f);
     { const float s = p == 1 ? -1.f : (p == 3 ? 1.f : 0.f); rot.ns = bd_f2(-s, s); }
     BD_UNROLL
-    for (int j = 0; j < 16; ++j) {
-        const Tw t = make_tw(BD_LDG(&zt[p * 16 + j]));
+    for (int c = 0; c < 3; ++c) {
         BD_UNROLL
-        for (int c = 0; c < 3; ++c) {
+        for (int j = 0; j < 16; ++j) {
+            const Tw t = make_tw(BD_LDG(&zt[p * 16 + j]));
             const float2 x0 = col[(c * 32 + j) * pitch], x1 = col[(c * 32 + j + 16) * pitch];
             const float2 a = pk_fma(pk_swap(x1), rot.ns, pk_fma(x1, pk_bc(rot.c), x0));
             v[c][j] = pk_cmul(a, t);
         }
+        PkDft<16, -1>::run(v[c]);
     }
-    BD_UNROLL
-    for (int c = 0; c < 3; ++c) PkDft<16, -1>::run(v[c]);
     // direct frequencies m = 0..7, then the mirrored ones m = 15 - i
     BD_UNROLL
     for (int h = 0; h < 2; ++h) {
-        float4 k[6];
-        BD_UNROLL
-        for (int c = 0; c < 6; ++c) k[c] = BD_LDG(kA + c * kcs + h * khs);
         BD_UNROLL
         for (int i = 0; i < 4; ++i) {
             const int m = 4 * h + i;
-            pl_mul3(pl_f4(k[0], i), pl_f4(k[1], i), pl_f4(k[2], i), sy * pl_f4(k[3], i), pl_f4(k[4], i),
-                    sy * pl_f4(k[5], i), v[0][m], v[1][m], v[2][m]);
+            pl_mul3(pl_f4(k.d[h][0], i), pl_f4(k.d[h][1], i), pl_f4(k.d[h][2], i), sy * pl_f4(k.d[h][3], i), pl_f4(k.d[h][4], i),
+                    sy * pl_f4(k.d[h][5], i), v[0][m], v[1][m], v[2][m]);
         }
     }
+    // the mirror list is the direct list of the partner lane (same warp, same iteration): mostly still in L1
     BD_UNROLL
     for (int h = 0; h < 2; ++h) {
-        float4 k[6];
+        float4 km[6];
         BD_UNROLL
-        for (int c = 0; c < 6; ++c) k[c] = BD_LDG(kB + c * kcs + h * khs);
+        for (int c = 0; c < 6; ++c) km[c] = BD_LDG(k.kB + c * kcs + h * khs);
         BD_UNROLL
         for (int i = 0; i < 4; ++i) {
             const int m = 15 - (4 * h + i);
-            pl_mul3(pl_f4(k[0], i), pl_f4(k[1], i), pl_f4(k[2], i), sy * pl_f4(k[3], i), -pl_f4(k[4], i),
-                    -sy * pl_f4(k[5], i), v[0][m], v[1][m], v[2][m]);
+            pl_mul3(pl_f4(km[0], i), pl_f4(km[1], i), pl_f4(km[2], i), sy * pl_f4(km[3], i), -pl_f4(km[4], i),
+                    -sy * pl_f4(km[5], i), v[0][m], v[1][m], v[2][m]);
         }
     }
     BD_UNROLL
@@ -253,7 +262,7 @@ struct YZFused {
     using Args = YZArgs;
     static constexpr int KIND = kKindYZFused;
     static constexpr int NZ = kPlaneNZ, NPEN = 3 * NZ, ZS = 2 * NZ / 16;
-    static constexpr int NT = 384;
+    static constexpr int NT = BD_YZ_NT;
     static constexpr int MINB = 1;
     static constexpr int NPHASES = 5;
     static constexpr int R0 = LS / 16;                   // first-pass radix; the second pass is radix 16
@@ -357,16 +366,22 @@ struct YZFused {
     static BD_HD void zstage(int tid, int kx, int q, const Args& a, float2* sm) {
         const float4* kbase = reinterpret_cast<const float4*>(a.KP) + (long)kx * (NQ * 6L * (ZS + 1) * 2 * NSL);
         constexpr long KCS = (long)(ZS + 1) * 2 * NSL, KHS = NSL;
-        for (int w = tid; w < LS * ZS; w += NT) {
+        // item w = (column e, lane p): its kernel-spectrum lists and the sign of the y-odd components
+        auto lists = [&](int w, PlK& k) {
             const int p = w & (ZS - 1), e = w / ZS;
             const int ki = BD_LDG(&a.kidx[q * LS + e]);
-            const int slot = ki & 0xfff, qs = (ki >> 12) & 7;
-            const float sy = (ki >> 15) ? -1.f : 1.f;
+            const float4* kq = kbase + (long)((ki >> 12) & 7) * 6 * KCS + (ki & 0xfff);
+            pl_load_k(kq + (long)p * 2 * NSL, kq + (long)(p ? ZS - p : ZS) * 2 * NSL, KCS, KHS, k);
+            return (ki >> 15) ? -1.f : 1.f;
+        };
+        for (int w = tid; w < LS * ZS; w += NT) {
+            const int p = w & (ZS - 1), e = w / ZS;
             float2* col = sm + pl_pe(e);
-            const float4* kq = kbase + (long)qs * 6 * KCS + slot;
 #if defined(__CUDA_ARCH__)
+            PlK kc;
+            const float sy = lists(w, kc);
             float2 y[3][16];
-            pl_zlane32(p, sy, col, PITCH, kq + (long)p * 2 * NSL, kq + (long)(p ? ZS - p : ZS) * 2 * NSL, KCS, KHS, a.zt, y);
+            pl_zlane32(p, sy, col, PITCH, kc, KCS, KHS, a.zt, y);
             // out[j] = sum_p y_p[j], out[j + 16] = sum_p i^p y_p[j]: two exchange rounds among the 4 lanes
             const bool hi = (p & 2) != 0, lo = (p & 1) != 0;
             const float sg = hi ? -1.f : 1.f;
@@ -404,9 +419,11 @@ struct YZFused {
             // host emulation (tests/emu): lane 0 of a column runs the four lanes in turn, same arithmetic
             if (p != 0) continue;
             float2 y[4][3][16];
-            for (int pp = 0; pp < ZS; ++pp)
-                pl_zlane32(pp, sy, col, PITCH, kq + (long)pp * 2 * NSL, kq + (long)(pp ? ZS - pp : ZS) * 2 * NSL, KCS, KHS,
-                           a.zt, y[pp]);
+            for (int pp = 0; pp < ZS; ++pp) {
+                PlK k;
+                const float sy = lists(w + pp, k);
+                pl_zlane32(pp, sy, col, PITCH, k, KCS, KHS, a.zt, y[pp]);
+            }
             for (int c = 0; c < 3; ++c)
                 for (int j = 0; j < 16; ++j) {
                     const float2 Se = pk_add(y[0][c][j], y[2][c][j]), So = pk_add(y[1][c][j], y[3][c][j]);
@@ -422,6 +439,13 @@ struct YZFused {
     static BD_HD void phase(int tid, int bx, int by, const Args& a, float2* sm) {
         const int kx = bx / NQ, q = q_of_order(bx % NQ);
         if constexpr (PH == 0) {
+            {
+                // the kernel-spectrum slots of this residue start towards L2 while the pencils are loaded (the
+                // blocks of one kx run side by side: between them they fetch all of its slots)
+                constexpr long KB = 6L * (ZS + 1) * 2 * NSL * 4 * (long)sizeof(float);
+                const char* kq = reinterpret_cast<const char*>(a.KP) + ((long)kx * NQ + q) * KB;
+                for (long o = (long)tid * 128; o < KB; o += NT * 128) bd_prefetch_l2(kq + o);
+            }
             if (q == 0) load_pass<0>(tid, kx, a, sm);
             if constexpr (NQ >= 2) { if (q == 1) load_pass<1>(tid, kx, a, sm); }
             if constexpr (NQ == 4) { if (q == 2) load_pass<2>(tid, kx, a, sm); else if (q == 3) load_pass<3>(tid, kx, a, sm); }
