@@ -68,8 +68,9 @@ def kind_bytes(cfg, info):
             "XInv": sp + 12 * N}
 
 
-def path_flops(cfg):
-    """SURVEY.md §8(d) count: 5 P log2 P per complex FFT, real x FFT as half-length complex + post pass."""
+def flops_parts(cfg):
+    """SURVEY.md §8(d) count: 5 P log2 P per complex FFT, real x FFT as half-length complex + post pass.
+    Returns (x one way, y one way, z one way, multiply)."""
     nx, ny, nz = cfg.nx, cfg.ny, cfg.nz
     Px, Py, Pz = 2 * nx, 2 * ny, (2 * nz if nz > 1 else 1)
     NS = nx + 1
@@ -78,7 +79,53 @@ def path_flops(cfg):
     fy = 3 * nz * NS * 5 * Py * lg(Py)
     fz = 3 * Py * NS * 5 * Pz * lg(Pz) if nz > 1 else 0.0
     mul = (30 if nz > 1 else 20) * NS * Py * Pz
-    return float(2 * (fx + fy + fz) + mul)
+    return float(fx), float(fy), float(fz), float(mul)
+
+
+def path_flops(cfg):
+    fx, fy, fz, mul = flops_parts(cfg)
+    return 2 * (fx + fy + fz) + mul
+
+
+def kind_flops(cfg, info):
+    """The same count split over the kernels of the plan's path (which steps each kernel runs: DESIGN.md §5)."""
+    fx, fy, fz, mul = flops_parts(cfg)
+    if info["path"] == 2:
+        return {"XFwdT": fx, "YFused": 2 * fy + mul, "XInvT": fx}
+    if info["path"] == 3:
+        return {"XZFwd": fx + fz, "YFused": 2 * fy + mul, "ZXInv": fx + fz}
+    if info["path"] == 4:
+        return {"XFwdT": fx, "YZFused": 2 * (fy + fz) + mul, "XInvP": fx}
+    return {"XFwd": fx, "YFwd": fy, "ZFused": 2 * fz + mul, "YInv": fy, "XInv": fx}
+
+
+# ----------------------------------------------------------------- ncu DRAM traffic (profiles/)
+def csrc_sha():
+    """Hash of the kernel sources: a stored ncu number is only quoted for the sources it was captured from."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2008_02478_b200", "csrc")
+    for name in sorted(os.listdir(d)):
+        if name.endswith((".h", ".cu", ".cuh")):
+            h.update(name.encode())
+            h.update(open(os.path.join(d, name), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(config, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` on `config`, from the committed ncu
+    summary profiles/ncu_traffic.csv (written by paper_2008_02478_b200/ncu_summary.py from an ncu --set full
+    report); None when no capture of the CURRENT kernel sources is on file."""
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    sha = csrc_sha()
+    best = None
+    for line in open(path).read().splitlines()[1:]:
+        f = [x.strip() for x in line.split(",")]
+        if len(f) >= 5 and f[0] == config and f[1] == kernel and f[4] == sha:
+            best = int(f[2]) + int(f[3])
+    return best
 
 
 # ----------------------------------------------------------------- clocks
@@ -122,7 +169,7 @@ class ClockSampler:
 
 
 # ----------------------------------------------------------------- GPU arm
-def time_config(torch, binding, cfg, steps, warmup, flush, peak_gbs, profile_reps=5):
+def time_config(torch, binding, cfg, steps, warmup, flush, peak_gbs, sm_max_mhz=1965.0, profile_reps=5):
     """Times `steps` steps of apply+energy on one config.  flush=True: L2 flushed between steps and each
     step timed with its own event pair; flush=False: one event pair around all steps (inputs > L2)."""
     M_host = W.make_input(cfg)
@@ -203,12 +250,23 @@ def time_config(torch, binding, cfg, steps, warmup, flush, peak_gbs, profile_rep
         torch.cuda.synchronize()
         ems += ea.elapsed_time(eb)
     kb = kind_bytes(cfg, info)
+    kf = kind_flops(cfg, info)
+    alu_peak = 148 * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6          # flop/s, FMA counted as 2
+    comp = info["compulsory_bytes"]
+    # every launch of every kind covers the whole mesh (launches_per_eval > 1 only on the chunked fallback, whose
+    # launches together cover it once), so the algorithmic bytes of a kind per evaluation are the compulsory bytes
+    # of the evaluation (24 B per cell + the reduced kernel spectrum); the bytes the kernel is
+    # DESIGNED to move (its inputs and outputs once, intermediate spectra included) are reported beside them
     per_kind = {k: {"ms_per_eval": t / profile_reps, "launches_per_eval": n // profile_reps,
-                    "algorithmic_bytes": kb[k], "gbs": kb[k] / (t / profile_reps) / 1e6}
+                    "algorithmic_bytes": comp, "gbs": comp / (t / profile_reps) / 1e6,
+                    "hbm_frac": comp / (t / profile_reps) / 1e6 / peak_gbs,
+                    "designed_bytes": kb[k], "kernel_gbs_designed": kb[k] / (t / profile_reps) / 1e6,
+                    "flops_5NlogN": kf.get(k), "alu_frac": (kf[k] / (t / profile_reps * 1e-3) / alu_peak) if k in kf else None}
                 for k, (t, n) in kinds.items()}
     # the stand-alone energy kernel (boris_demag_energy); the timed step gathers E inside its last kernel instead
     per_kind["Energy"] = {"ms_per_eval": ems / profile_reps, "launches_per_eval": 1,
-                          "algorithmic_bytes": 24 * cfg.cells, "gbs": 24 * cfg.cells / (ems / profile_reps) / 1e6}
+                          "algorithmic_bytes": 24 * cfg.cells, "gbs": 24 * cfg.cells / (ems / profile_reps) / 1e6,
+                          "hbm_frac": 24 * cfg.cells / (ems / profile_reps) / 1e6 / peak_gbs}
     ms_step = ms / steps
     res = {"config": cfg.name, "mesh": [cfg.nx, cfg.ny, cfg.nz], "padded": list(info["padded"]),
            "ms_per_step": ms_step, "evals_per_s": 1e3 / ms_step, "mcell_per_s": cfg.cells / ms_step / 1e3,
@@ -236,41 +294,29 @@ def time_e2e(torch, plan, cfg, M_host, steps, warmup):
 
 
 # ----------------------------------------------------------------- oracle arm (CPU baseline / --impl reference)
-def oracle_sample_config(cfg):
-    """Bounded sample of the workload the fp64 oracle finishes in ~1-2 s per evaluation:
-    the same mesh with at most 2^21 cells (fewer z layers, then fewer y rows)."""
-    nz, ny = cfg.nz, cfg.ny
-    while cfg.nx * ny * nz > (1 << 21) and nz > 1:
-        nz //= 2
-    while cfg.nx * ny * nz > (1 << 21):
-        ny //= 2
-    return W.Config(cfg.name + "-sample", cfg.nx, ny, nz, cfg.hx, cfg.hy, cfg.hz, cfg.Ms, cfg.seed, cfg.texture)
-
-
 def oracle_setup(cfg):
+    """The fp64 oracle on the FULL mesh of the workload (no sub-sampling, nothing scaled); its kernel spectrum is
+    precomputed and excluded from the timing, as the GPU plan's is."""
     from oracle.demag_direct import tensor_table          # the only place bench.py touches oracle/
     from oracle.demag_fft import demag_fft, kernel_spectrum
-    sc = oracle_sample_config(cfg)
-    M = W.make_input(sc)
-    Khat = kernel_spectrum(sc.shape, sc.h, table=tensor_table(sc.shape, sc.h))     # plan-time, excluded (as the GPU plan)
-    what = (f"{sc.nx}x{sc.ny}x{sc.nz} cells of {cfg.name}'s {cfg.nx}x{cfg.ny}x{cfg.nz} mesh "
-            f"({sc.cells / cfg.cells:.3g} of its cells), fp64 zero-padded FFT convolution oracle/demag_fft.py, "
-            "kernel spectrum precomputed; eval/s scaled by the cell ratio")
-    return sc, M, Khat, (lambda: demag_fft(M, sc.h, Khat=Khat)), what
+    M = W.make_input(cfg)
+    Khat = kernel_spectrum(cfg.shape, cfg.h, table=tensor_table(cfg.shape, cfg.h))
+    what = (f"the full {cfg.nx}x{cfg.ny}x{cfg.nz} mesh of {cfg.name}, fp64 zero-padded FFT convolution "
+            "oracle/demag_fft.py (scipy pocketfft, all host cores), kernel spectrum precomputed")
+    return M, Khat, (lambda: demag_fft(M, cfg.h, Khat=Khat)), what
 
 
-def cpu_baseline(cfg, budget_s=15.0):
-    sc, M, Khat, run, what = oracle_setup(cfg)
+def cpu_baseline(cfg, budget_s=12.0):
+    M, Khat, run, what = oracle_setup(cfg)
     run()
     n, t0 = 0, time.perf_counter()
     while True:
         run()
         n += 1
         dt = time.perf_counter() - t0
-        if dt > budget_s or n >= 20:
+        if (dt > budget_s and n >= 3) or n >= 20:
             break
-    cells_per_s = sc.cells * n / dt
-    return {"value": cells_per_s / cfg.cells, "unit": UNIT, "mcell_per_s": cells_per_s / 1e6,
+    return {"value": n / dt, "unit": UNIT, "mcell_per_s": cfg.cells * n / dt / 1e6,
             "cores": os.cpu_count(), "kind": "oracle", "sample": f"{n} evaluations of {what}",
             "cpu": cpu_model()}
 
@@ -288,14 +334,14 @@ def cpu_model():
 def run_reference(args, cfg):
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    sc, M, Khat, run, what = oracle_setup(cfg)
+    M, Khat, run, what = oracle_setup(cfg)
     for _ in range(args.warmup):
         run()
     t0 = time.perf_counter()
     for _ in range(args.steps):
         run()
     dt = time.perf_counter() - t0
-    value = sc.cells * args.steps / dt / cfg.cells
+    value = args.steps / dt
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -305,6 +351,28 @@ def run_reference(args, cfg):
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
+
+
+# ----------------------------------------------------------------- device probes (profiles/*_microbench.md)
+def run_micro(torch, binding, build):
+    """FP32 lane rate per instruction kind and HBM throughput per piece size, as one JSON line and a table."""
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --micro needs a CUDA device")
+    build.build()
+    peak_gbs, sm_max_mhz, peak_src = measured_peaks()
+    names = ["FADD", "FFMA", "FADD2 (packed)", "FFMA2 (packed)"]
+    rate = {n: binding.micro_fp32_rate(i) for i, n in enumerate(names)}
+    nominal = 148 * FP32_LANES_PER_SM * sm_max_mhz * 1e6
+    seg = {str(sb): {"read_gbs": binding.micro_segment_bw(sb, False), "write_gbs": binding.micro_segment_bw(sb, True)}
+           for sb in (16, 32, 64, 128, 256, 512)}
+    print("| instruction | T lane-ops/s | of 148 SM x 128 lanes x %.0f MHz |" % sm_max_mhz, file=sys.stderr)
+    for n in names:
+        print(f"| {n} | {rate[n] / 1e12:.2f} | {rate[n] / nominal:.3f} |", file=sys.stderr)
+    print("| piece bytes | read GB/s | write GB/s | read / %.0f GB/s (%s) |" % (peak_gbs, peak_src), file=sys.stderr)
+    for sb, v in seg.items():
+        print(f"| {sb} | {v['read_gbs']:.0f} | {v['write_gbs']:.0f} | {v['read_gbs'] / peak_gbs:.3f} |", file=sys.stderr)
+    print(json.dumps({"micro": {"fp32_lane_ops_per_s": rate, "nominal_lane_rate": nominal, "segments": seg,
+                                "hbm_peak_gbs": peak_gbs, "peak_source": peak_src}}))
 
 
 # ----------------------------------------------------------------- multi-GPU: replicas only (DESIGN.md §9)
@@ -333,6 +401,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-all-configs", action="store_true", help="skip the four secondary configs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--micro", action="store_true",
+                    help="print the table of the two device probes of include/boris_micro.h and exit")
     args = ap.parse_args()
     cfg = W.CONFIGS[args.config]
     args.warmup = max(args.warmup, 0)
@@ -342,6 +412,9 @@ def main():
 
     import torch
     from paper_2008_02478_b200 import binding, build
+    if args.micro:
+        run_micro(torch, binding, build)
+        return
     rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
@@ -368,7 +441,7 @@ def main():
     sampler = ClockSampler(local)
     barrier()
     sampler.start()
-    res, plan, (M_host, M, H, E) = time_config(torch, binding, cfg, args.steps, warmup, flush, peak_gbs)
+    res, plan, (M_host, M, H, E) = time_config(torch, binding, cfg, args.steps, warmup, flush, peak_gbs, sm_max_mhz)
     barrier()
     clocks = sampler.stop()
     ms_step = res["ms_per_step"]
@@ -380,17 +453,18 @@ def main():
         dist.destroy_process_group()
         return
 
-    # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the ncu --set full
-    # captures summarised in profiles/r01_tiled.md (one capture per workload; None where none was taken)
-    ncu_traffic = {("C5", "YFused"): 648591360 + 357802240, ("C3", "YFused"): 42233088 + 1280}
     kernels = res["kernels"]
     dom = max((k for k in kernels if k != "Energy"), key=lambda k: kernels[k]["ms_per_eval"])
     dk = kernels[dom]
     launches = max(dk["launches_per_eval"], 1)
+    # achieved = algorithmic (compulsory) bytes of the work one launch covers / its duration;
+    # the throughput over the bytes the kernel is designed to move is reported under its own key
     roofline = {"kernel": dom, "bound": "hbm", "achieved": dk["gbs"], "peak": peak_gbs, "unit": "GB/s",
-                "frac": dk["gbs"] / peak_gbs, "traffic": ncu_traffic.get((cfg.name, dom)), "peak_source": peak_src,
+                "frac": dk["gbs"] / peak_gbs, "traffic": ncu_traffic(cfg.name, dom), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": dk["algorithmic_bytes"] / launches,
                 "avg_launch_ms": dk["ms_per_eval"] / launches, "launches_per_eval": launches,
+                "kernel_gbs_designed": dk["kernel_gbs_designed"], "designed_bytes_per_launch": dk["designed_bytes"] / launches,
+                "alu_frac": dk["alu_frac"],
                 "share_of_eval": dk["ms_per_eval"] / sum(v["ms_per_eval"] for k, v in kernels.items() if k != "Energy")}
     alu_peak = 148 * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
     path = {"compulsory_bytes": res["compulsory_bytes"], "hbm_frac_of_peak": res["compulsory_bytes"] / (ms_step * 1e-3) / (peak_gbs * 1e9),
@@ -440,7 +514,7 @@ def main():
                 continue
             c = W.CONFIGS[name]
             steps = 200 if c.cells <= (1 << 20) else 50
-            r, p, bufs = time_config(torch, binding, c, steps, 5, 24 * c.cells < (192 << 20), peak_gbs, profile_reps=3)
+            r, p, bufs = time_config(torch, binding, c, steps, 5, 24 * c.cells < (192 << 20), peak_gbs, sm_max_mhz, profile_reps=3)
             allc[name] = r
             p.close()
             del bufs

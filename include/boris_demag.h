@@ -24,8 +24,9 @@
  *     kernels per call; M and H then only need 4-byte alignment.
  *   - All fp32 arithmetic on the device; fp64 only at plan time and in the energy sum.
  *   - A plan owns the kernel spectrum, twiddle tables and workspace on the device
- *     that was current when it was created.  It may be used from one stream at a
- *     time (the workspace is shared).  The caller owns M, H and E.
+ *     that was current when it was created; every apply / energy call checks that the
+ *     same device is current and fails with -1 otherwise.  It may be used from one
+ *     stream at a time (the workspace is shared).  The caller owns M, H and E.
  *   - Return codes: 0 ok; -1 invalid argument; -2 CUDA error; -3 out of memory.
  *     boris_demag_last_error() returns a thread-local message for the last failure.
  *   - There is no CPU fallback: without a CUDA device plan_create fails with -2.
@@ -60,8 +61,8 @@ int boris_demag_apply(boris_demag_plan* plan, const float* M, float* H, void* st
  *   BORIS_DEMAG_ACCUMULATE  H += -N * M instead of H = -N * M: the demag term added to an effective field
  *                           that already holds other contributions ("additive field contributions").
  * Both go through plan-owned planar staging buffers and two copy kernels (M in, H out); on a power-of-two
- * mesh the buffers are allocated by the FIRST such call (24 bytes per cell), which is the one case in which an
- * apply allocates.  M, H: DEVICE pointers, 4-byte aligned, must not alias.  Error codes as boris_demag_apply. */
+ * mesh the buffers are allocated (both or neither) by the FIRST such call (24 bytes per cell), which is the
+ * one case in which an apply allocates and synchronises — do not make that first call inside a stream capture.  M, H: DEVICE pointers, 4-byte aligned, must not alias.  Error codes as boris_demag_apply. */
 #define BORIS_DEMAG_AOS 1u
 #define BORIS_DEMAG_ACCUMULATE 2u
 int boris_demag_apply_ex(boris_demag_plan* plan, const float* M, float* H, unsigned flags, void* stream);
@@ -111,6 +112,10 @@ const char* boris_demag_last_error(void);
 int boris_demag_plan_info(const boris_demag_plan* plan, long long* compulsory_bytes,
                           long long* designed_hbm_bytes, long long* workspace_bytes,
                           int padded[3], int* kernel_launches);
+
+/* The caller's mesh the plan was created for: cells[3] = (nx, ny, nz), sides[3] = (hx, hy, hz) in metres
+ * (one rectangular mesh of equal cuboid cells).  Either out pointer may be NULL. */
+int boris_demag_plan_mesh(const boris_demag_plan* plan, int cells[3], double sides[3]);
 
 /* Which kernel path the plan uses and how much it stores (harness bookkeeping).
  * Any out pointer may be NULL.

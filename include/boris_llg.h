@@ -26,7 +26,8 @@ typedef struct boris_llg boris_llg;   /* opaque; owns device work arrays, borrow
 
 /* `plan` is the demag plan of the same nx x ny x nz mesh and cell (it must outlive the solver and is used on
  * the solver's stream).  Ms > 0 (A/m), A >= 0 (J/m), alpha >= 0, gamma > 0 (m/(A s); mu0 |gamma_e| = 2.2128e5).
- * Returns NULL on failure. */
+ * (nx, ny, nz) and (hx, hy, hz) are checked against the plan (boris_demag_plan_mesh): a mismatch is rejected.
+ * Returns NULL on failure, with the reason in boris_demag_last_error(). */
 boris_llg* boris_llg_create(boris_demag_plan* plan, int nx, int ny, int nz, double hx, double hy, double hz,
                             double Ms, double A, double alpha, double gamma);
 void boris_llg_destroy(boris_llg* s);

@@ -72,6 +72,12 @@ def lib():
         L.boris_llg_effective_field.argtypes = [c_vp, c_vp, c_vp, c_vp]
         L.boris_llg_rk4.restype = c_int
         L.boris_llg_rk4.argtypes = [c_vp, c_vp, c_dbl, c_int, c_vp]
+        L.boris_demag_plan_mesh.restype = c_int
+        L.boris_demag_plan_mesh.argtypes = [c_vp, ctypes.POINTER(c_int), ctypes.POINTER(c_dbl)]
+        L.boris_micro_fp32_rate.restype = c_int
+        L.boris_micro_fp32_rate.argtypes = [c_int, ctypes.POINTER(c_dbl)]
+        L.boris_micro_segment_bw.restype = c_int
+        L.boris_micro_segment_bw.argtypes = [c_int, c_int, ctypes.POINTER(c_dbl)]
         _lib = L
     return _lib
 
@@ -225,6 +231,12 @@ class DemagPlan:
         return {"compulsory_bytes": comp.value, "designed_hbm_bytes": des.value, "workspace_bytes": ws.value,
                 "padded": tuple(padded), "kernel_launches": nl.value, **lay}
 
+    def mesh(self):
+        """((nx, ny, nz), (hx, hy, hz)) the plan was created for."""
+        cells, sides = (ctypes.c_int * 3)(), (ctypes.c_double * 3)()
+        _check(lib().boris_demag_plan_mesh(self._h, cells, sides), "boris_demag_plan_mesh")
+        return tuple(cells), tuple(sides)
+
     def kernel_spectrum(self):
         """Natural reduced fp32 spectrum [ncomp][nzr][nyr][nxr] read back from the device."""
         ncomp = 6 if self.nz > 1 else 4
@@ -283,3 +295,22 @@ class LLG:
             self.close()
         except Exception:
             pass
+
+
+# ----------------------------------------------------------------- device probes (include/boris_micro.h)
+def micro_fp32_rate(op):
+    """Lane operations per second of FADD (0), FFMA (1), FADD2 (2) or FFMA2 (3) over the whole device."""
+    out = ctypes.c_double(0.0)
+    rc = lib().boris_micro_fp32_rate(int(op), ctypes.byref(out))
+    if rc:
+        raise DemagError(f"boris_micro_fp32_rate failed ({rc}): {last_error()}")
+    return out.value
+
+
+def micro_segment_bw(seg_bytes, write):
+    """GB/s of a read (write = False) or write stream that touches HBM in pieces of seg_bytes."""
+    out = ctypes.c_double(0.0)
+    rc = lib().boris_micro_segment_bw(int(seg_bytes), 1 if write else 0, ctypes.byref(out))
+    if rc:
+        raise DemagError(f"boris_micro_segment_bw failed ({rc}): {last_error()}")
+    return out.value

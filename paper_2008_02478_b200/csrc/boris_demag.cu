@@ -174,6 +174,12 @@ int grid_for(long total, int threads) {
 
 }  // namespace
 
+// the other translation units of the library report their failures through the same thread-local text
+namespace bd {
+int micro_fail(cudaError_t e, const char* what) { return cuda_fail(e, what); }
+int set_error(int code, const char* msg) { return fail(code, msg); }
+}  // namespace bd
+
 // ------------------------------------------------------------------ plan
 struct boris_demag_plan {
     // nx, ny, nz: the mesh the kernels work on (powers of two).  ux, uy, uz: the caller's mesh; where it is
@@ -481,9 +487,17 @@ boris_demag_plan* boris_demag_plan_create(int ux, int uy, int uz, double hx, dou
 }
 
 namespace {
+// a plan belongs to the device it was created on (its tables, workspace and shared-memory opt-ins live there)
+int check_device(const boris_demag_plan* p) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != p->device)
+        return fail(-1, "the current CUDA device is not the one the plan was created on");
+    return 0;
+}
 int check_fields(const boris_demag_plan* p, const void* M, const void* H, bool alias_ok) {
     if (!p || !M || !H) return fail(-1, "null argument");
     if (!alias_ok && M == H) return fail(-1, "M and H must not alias");
+    if (int rc = check_device(p)) return rc;
     // the kernels read rows as 16-byte vectors; a mesh staged through Mp / Hp is copied element by element
     if ((((uintptr_t)M | (uintptr_t)H) & (p->padmode ? 3 : 15)) != 0)
         return fail(-1, p->padmode ? "M and H must be 4-byte aligned" : "M and H must be 16-byte aligned");
@@ -507,7 +521,7 @@ int boris_demag_apply(boris_demag_plan* p, const float* M, float* H, void* strea
     }
     float* Hu = H;
     if (p->padmode) H = p->Hp;
-    CudaLauncher run{(cudaStream_t)stream};
+    CudaLauncher run{(cudaStream_t)stream, p->device};
     const bd::PlanView pv = plan_view(p);
     const int rc = bd::enqueue_apply(run, pv, M, H);
     if (rc == -2) return cuda_fail(run.err, "kernel launch");
@@ -528,7 +542,7 @@ int boris_demag_apply_energy(boris_demag_plan* p, const float* M, float* H, doub
         if (int rc = stage(p, true, M, p->Mp, (cudaStream_t)stream)) return rc;
         M = p->Mp; H = p->Hp;
     }
-    CudaLauncher run{(cudaStream_t)stream};
+    CudaLauncher run{(cudaStream_t)stream, p->device};
     bd::PlanView pv = plan_view(p);
     pv.en = bd::EnergyArgs{M, p->partial_f, reinterpret_cast<unsigned*>(p->partial_f + kFusedEnergySlots), E_dev,
                            -0.5 * (4e-7 * bd::kPi) * p->hx * p->hy * p->hz};
@@ -545,16 +559,20 @@ int boris_demag_apply_ex(boris_demag_plan* p, const float* M, float* H, unsigned
     if (flags & ~(unsigned)(BORIS_DEMAG_AOS | BORIS_DEMAG_ACCUMULATE)) return fail(-1, "unknown flag");
     if (flags == 0) return boris_demag_apply(p, M, H, stream);
     if (((uintptr_t)M | (uintptr_t)H) & 3) return fail(-1, "M and H must be 4-byte aligned");
-    if (!p->Mp) {                // first use of a staged variant on a power-of-two mesh
+    if (int rc = check_device(p)) return rc;
+    if (!p->Mp || !p->Hp) {      // first use of a staged variant on a power-of-two mesh: both buffers or neither
         const size_t np = (size_t)3 * p->nx * p->ny * p->nz;
-        if (int rc = dev_alloc(p, &p->Mp, np)) return rc;
-        if (int rc = dev_alloc(p, &p->Hp, np)) return rc;
-        BD_CUDA(cudaMemsetAsync(p->Mp, 0, np * sizeof(float), (cudaStream_t)stream));
+        float *mp = nullptr, *hp = nullptr;
+        int rc = dev_alloc(p, &mp, np);
+        if (!rc) rc = dev_alloc(p, &hp, np);
+        if (!rc && cudaMemset(mp, 0, np * sizeof(float)) != cudaSuccess) rc = fail(-2, "cudaMemset");
+        if (rc) { cudaFree(mp); cudaFree(hp); return rc; }
+        p->Mp = mp; p->Hp = hp;
     }
     cudaStream_t st = (cudaStream_t)stream;
     const bool aos = (flags & BORIS_DEMAG_AOS) != 0, acc = (flags & BORIS_DEMAG_ACCUMULATE) != 0;
     if (int rc = stage(p, true, M, p->Mp, st, aos)) return rc;
-    CudaLauncher run{st};
+    CudaLauncher run{st, p->device};
     const bd::PlanView pv = plan_view(p);
     const int rc = bd::enqueue_apply(run, pv, p->Mp, p->Hp);
     if (rc == -2) return cuda_fail(run.err, "kernel launch");
@@ -567,15 +585,27 @@ int boris_demag_apply_timed(boris_demag_plan* p, const float* M, float* H, void*
     if (!ms_by_kind || !launches_by_kind) return fail(-1, "null argument");
     if (int rc = check_fields(p, M, H, false)) return rc;
     float* Hu = H;
-    if (p->padmode) {            // the staging copies are not among the timed kinds
-        if (int rc = stage(p, true, M, p->Mp, (cudaStream_t)stream)) return rc;
+    std::vector<TimedLaunch> timed;
+    auto timed_stage = [&](bool in, const float* src, float* dst, int kind) {
+        TimedLaunch t{kind, nullptr, nullptr};
+        if (cudaEventCreate(&t.t0) != cudaSuccess) return fail(-2, "cudaEventCreate");
+        if (cudaEventCreate(&t.t1) != cudaSuccess) { cudaEventDestroy(t.t0); return fail(-2, "cudaEventCreate"); }
+        timed.push_back(t);
+        cudaEventRecord(t.t0, (cudaStream_t)stream);
+        const int rc = stage(p, in, src, dst, (cudaStream_t)stream);
+        cudaEventRecord(t.t1, (cudaStream_t)stream);
+        return rc;
+    };
+    int rc = 0;
+    if (p->padmode) {            // the staging copies count with the x kernels they feed (kinds 0 and 5)
+        rc = timed_stage(true, M, p->Mp, 0);
         M = p->Mp; H = p->Hp;
     }
-    std::vector<TimedLaunch> timed;
-    CudaLauncher run{(cudaStream_t)stream};
+    CudaLauncher run{(cudaStream_t)stream, p->device};
     run.timed = &timed;
     const bd::PlanView pv = plan_view(p);
-    int rc = bd::enqueue_apply(run, pv, M, H);
+    if (!rc) rc = bd::enqueue_apply(run, pv, M, H);
+    if (!rc && p->padmode) rc = timed_stage(false, p->Hp, Hu, 5);
     cudaError_t e = cudaStreamSynchronize((cudaStream_t)stream);
     for (int k = 0; k < bd::kNumKinds; ++k) { ms_by_kind[k] = 0.f; launches_by_kind[k] = 0; }
     for (const TimedLaunch& t : timed) {
@@ -589,7 +619,6 @@ int boris_demag_apply_timed(boris_demag_plan* p, const float* M, float* H, void*
     if (rc == -2) return cuda_fail(run.err, "kernel launch");
     if (rc) return fail(rc, "unsupported size");
     if (e != cudaSuccess) return cuda_fail(e, "cudaStreamSynchronize");
-    if (p->padmode) return stage(p, false, p->Hp, Hu, (cudaStream_t)stream);
     return 0;
 }
 
@@ -663,6 +692,13 @@ int boris_demag_plan_info(const boris_demag_plan* p, long long* compulsory_bytes
     if (workspace_bytes) *workspace_bytes = p->bytes;
     if (padded) { padded[0] = kl.Px; padded[1] = kl.Py; padded[2] = kl.Pz; }
     if (kernel_launches) *kernel_launches = bd::apply_launch_count(p->nx, p->nz, p->cfg) + (p->padmode ? 2 : 0);
+    return 0;
+}
+
+int boris_demag_plan_mesh(const boris_demag_plan* p, int cells[3], double sides[3]) {
+    if (!p) return fail(-1, "null plan");
+    if (cells) { cells[0] = p->ux; cells[1] = p->uy; cells[2] = p->uz; }
+    if (sides) { sides[0] = p->hx; sides[1] = p->hy; sides[2] = p->hz; }
     return 0;
 }
 

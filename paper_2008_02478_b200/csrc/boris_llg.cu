@@ -10,7 +10,11 @@
 
 #include "../../include/boris_llg.h"
 
+namespace bd { int set_error(int code, const char* msg); }   // boris_demag.cu: the library's thread-local error text
+
 namespace {
+
+int llg_fail(int code, const char* msg) { return bd::set_error(code, msg); }
 
 constexpr double kMu0 = 4e-7 * 3.14159265358979323846264338327950288;
 
@@ -115,32 +119,48 @@ void boris_llg_destroy(boris_llg* s) {
 boris_llg* boris_llg_create(boris_demag_plan* plan, int nx, int ny, int nz, double hx, double hy, double hz,
                             double Ms, double A, double alpha, double gamma) {
     if (!plan || nx < 1 || ny < 1 || nz < 1 || !(hx > 0) || !(hy > 0) || !(hz > 0) || !(Ms > 0) || !(A >= 0) ||
-        !(alpha >= 0) || !(gamma > 0))
+        !(alpha >= 0) || !(gamma > 0)) {
+        llg_fail(-1, "boris_llg_create: invalid argument");
         return nullptr;
-    int padded[3];
-    long long comp = 0;
-    if (boris_demag_plan_info(plan, &comp, nullptr, nullptr, padded, nullptr)) return nullptr;
+    }
+    // the work arrays are sized from (nx, ny, nz) and boris_demag_apply reads and writes the plan's mesh:
+    // the two must be the same mesh
+    int cells[3];
+    double sides[3];
+    if (boris_demag_plan_mesh(plan, cells, sides)) return nullptr;
+    if (cells[0] != nx || cells[1] != ny || cells[2] != nz) {
+        llg_fail(-1, "boris_llg_create: (nx, ny, nz) differ from the mesh the demag plan was created for");
+        return nullptr;
+    }
+    const double tol = 1e-12;
+    if (std::fabs(sides[0] - hx) > tol * hx || std::fabs(sides[1] - hy) > tol * hy || std::fabs(sides[2] - hz) > tol * hz) {
+        llg_fail(-1, "boris_llg_create: (hx, hy, hz) differ from the cell sides of the demag plan");
+        return nullptr;
+    }
     boris_llg* s = new (std::nothrow) boris_llg();
-    if (!s) return nullptr;
+    if (!s) { llg_fail(-3, "boris_llg_create: out of host memory"); return nullptr; }
     s->plan = plan; s->d = Dims{nx, ny, nz};
     s->hx = hx; s->hy = hy; s->hz = hz; s->Ms = Ms; s->A = A; s->alpha = alpha; s->gamma = gamma;
     const size_t bytes = (size_t)3 * nx * ny * nz * sizeof(float);
     if (cudaMalloc((void**)&s->H, bytes) != cudaSuccess || cudaMalloc((void**)&s->u, bytes) != cudaSuccess ||
         cudaMalloc((void**)&s->u2, bytes) != cudaSuccess || cudaMalloc((void**)&s->acc, bytes) != cudaSuccess) {
+        cudaGetLastError();
         boris_llg_destroy(s);
+        llg_fail(-3, "boris_llg_create: out of device memory");
         return nullptr;
     }
     return s;
 }
 
 int boris_llg_set_applied_field(boris_llg* s, double Hx, double Hy, double Hz) {
-    if (!s || !std::isfinite(Hx) || !std::isfinite(Hy) || !std::isfinite(Hz)) return -1;
+    if (!s || !std::isfinite(Hx) || !std::isfinite(Hy) || !std::isfinite(Hz))
+        return llg_fail(-1, "boris_llg_set_applied_field: invalid argument");
     s->Hext[0] = Hx; s->Hext[1] = Hy; s->Hext[2] = Hz;
     return 0;
 }
 
 int boris_llg_effective_field(boris_llg* s, const float* m, float* Heff, void* stream) {
-    if (!s || !m || !Heff || m == Heff) return -1;
+    if (!s || !m || !Heff || m == Heff) return llg_fail(-1, "boris_llg_effective_field: null or aliasing argument");
     cudaStream_t st = (cudaStream_t)stream;
     if (int rc = boris_demag_apply(s->plan, m, Heff, stream)) return rc;          // H_demag of the unit field
     const double c = 2.0 * s->A / (kMu0 * s->Ms);
@@ -149,13 +169,13 @@ int boris_llg_effective_field(boris_llg* s, const float* m, float* Heff, void* s
     k_exchange_zeeman<<<(unsigned)(rows < (1L << 20) ? rows : (1L << 20)), threads, 0, st>>>(
         m, Heff, s->d, (float)s->Ms, (float)(c / (s->hx * s->hx)), (float)(c / (s->hy * s->hy)), (float)(c / (s->hz * s->hz)),
         (float)s->Hext[0], (float)s->Hext[1], (float)s->Hext[2]);
-    return cudaGetLastError() == cudaSuccess ? 0 : -2;
+    if (cudaError_t e = cudaGetLastError(); e != cudaSuccess) return llg_fail(-2, cudaGetErrorString(e));
+    return 0;
 }
 
 int boris_llg_rk4(boris_llg* s, float* m, double dt, int nsteps, void* stream) {
-    if (!s || !m || !(dt > 0) || nsteps < 0) return -1;
+    if (!s || !m || !(dt > 0) || nsteps < 0) return llg_fail(-1, "boris_llg_rk4: invalid argument");
     cudaStream_t st = (cudaStream_t)stream;
-    const long cells = (long)s->d.nx * s->d.ny * s->d.nz;
     const float g = (float)(s->gamma / (1.0 + s->alpha * s->alpha)), al = (float)s->alpha;
     const float w[4] = {1.f, 2.f, 2.f, 1.f};
     const float a[4] = {(float)(0.5 * dt), (float)(0.5 * dt), (float)dt, 0.f};
@@ -164,7 +184,6 @@ int boris_llg_rk4(boris_llg* s, float* m, double dt, int nsteps, void* stream) {
     const long rows = (long)s->d.nz * s->d.ny;
     const int threads = s->d.nx >= 256 ? 256 : (s->d.nx >= 64 ? 64 : 32);
     const unsigned blocks = (unsigned)(rows < (1L << 20) ? rows : (1L << 20));
-    (void)cells;
     for (int step = 0; step < nsteps; ++step) {
         const float* u = m;                                      // stage state: m0, then the two work arrays in turn
         for (int k = 0; k < 4; ++k) {
@@ -173,10 +192,11 @@ int boris_llg_rk4(boris_llg* s, float* m, double dt, int nsteps, void* stream) {
             k_rk4_stage_fused<<<blocks, threads, 0, st>>>(m, u, s->H, s->acc, un, m, s->d, (float)s->Ms, cx, cy, cz,
                                                           (float)s->Hext[0], (float)s->Hext[1], (float)s->Hext[2], g, al,
                                                           w[k], a[k], (float)(dt / 6.0), k == 0, k == 3);
+            if (cudaError_t e = cudaGetLastError(); e != cudaSuccess) return llg_fail(-2, cudaGetErrorString(e));
             u = un;
         }
     }
-    return cudaGetLastError() == cudaSuccess ? 0 : -2;
+    return 0;
 }
 
 }  // extern "C"

@@ -5,6 +5,7 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <atomic>
 #include <type_traits>
 #include <vector>
 
@@ -44,8 +45,11 @@ int cu_xz_big(CudaLauncher& run, const PlanView& p, const float* M, float* H, bo
 int cu_plane_x(CudaLauncher& run, const PlanView& p, const float* M, float* H, bool fwd);   // tu_plane_x.cu
 int cu_plane_yz(CudaLauncher& run, const PlanView& p);                                      // tu_plane_yz.cu
 
+constexpr int kMaxDevices = 64;
+
 struct CudaLauncher {
     cudaStream_t st;
+    int dev = 0;                                   // the plan's device (the current one: checked by the entry points)
     cudaError_t err = cudaSuccess;
     std::vector<TimedLaunch>* timed = nullptr;     // boris_demag_apply_timed only
     template <class K>
@@ -65,11 +69,14 @@ struct CudaLauncher {
     template <class K>
     int launch(Grid g, const typename K::Args& a) {
         const size_t smem = (size_t)K::smem_elems(a) * sizeof(float2);
-        static size_t opted = 48 * 1024;           // per kernel instantiation
-        if (smem > opted) {
+        // the opt-in to more than 48 KB of dynamic shared memory is per kernel AND per device
+        static std::atomic<size_t> opted[kMaxDevices];
+        const int d = dev >= 0 && dev < kMaxDevices ? dev : 0;
+        if (smem > 48 * 1024 && smem > opted[d].load(std::memory_order_relaxed)) {
             err = cudaFuncSetAttribute(phase_kernel<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             if (err != cudaSuccess) return -2;
-            opted = smem;
+            size_t seen = opted[d].load(std::memory_order_relaxed);
+            while (seen < smem && !opted[d].compare_exchange_weak(seen, smem, std::memory_order_relaxed)) {}
         }
         phase_kernel<K><<<dim3(g.x, g.y), K::NT, smem, st>>>(a);
         err = cudaGetLastError();

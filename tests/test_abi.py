@@ -10,6 +10,7 @@ from paper_2008_02478_b200 import binding, build
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 HEADER = os.path.join(ROOT, "include", "boris_demag.h")
 HEADER_LLG = os.path.join(ROOT, "include", "boris_llg.h")
+HEADER_MICRO = os.path.join(ROOT, "include", "boris_micro.h")
 
 
 @pytest.fixture(scope="session", autouse=True)
@@ -18,9 +19,9 @@ def built_library():
 
 
 def declared_symbols():
-    text = open(HEADER).read() + open(HEADER_LLG).read()
+    text = open(HEADER).read() + open(HEADER_LLG).read() + open(HEADER_MICRO).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(boris_(?:demag|llg)_\w+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(boris_(?:demag|llg|micro)_\w+)\s*\(", text)))
 
 
 def test_header_declares_the_entry_points_the_north_star_names():

@@ -1,7 +1,8 @@
 """GPU parity of the LLG evaluation around the demag path (include/boris_llg.h) with oracle/llg.py."""
 import numpy as np
 import pytest
-import torch
+
+torch = pytest.importorskip("torch")
 
 from oracle import llg as O
 from paper_2008_02478_b200 import binding, build, workloads as W
@@ -23,8 +24,11 @@ def unit_field(shape, seed):
     return W.make_texture("vortex" if shape[0] == 1 else "helix", shape, 1.0, seed=seed)     # |m| = 1, fp32
 
 
+# the last two: more rows than the stage kernel has blocks to spare per row group, plane strides of 16 K and
+# 64 K elements (the stencil's +-plane neighbours), and the 2-D row walk of a 256 x 256 film
 @pytest.mark.parametrize("shape,h", [((1, 32, 64), (4e-9, 4e-9, 3e-9)), ((8, 16, 32), (3e-9, 3e-9, 2e-9)),
-                                     ((3, 10, 6), (4e-9, 5e-9, 3e-9))])
+                                     ((3, 10, 6), (4e-9, 5e-9, 3e-9)), ((32, 128, 128), (3e-9, 3e-9, 2e-9)),
+                                     ((1, 256, 256), (4e-9, 4e-9, 4e-9))])
 def test_effective_field_matches_the_oracle(shape, h):
     nz, ny, nx = shape
     m_host = unit_field(shape, 61)
@@ -44,12 +48,13 @@ def test_effective_field_matches_the_oracle(shape, h):
     plan.close()
 
 
-@pytest.mark.parametrize("shape,h", [((1, 16, 32), (4e-9, 4e-9, 3e-9)), ((4, 8, 16), (3e-9, 3e-9, 3e-9)),
-                                     ((2, 5, 7), (4e-9, 4e-9, 4e-9))])
-def test_rk4_steps_match_the_oracle(shape, h):
+@pytest.mark.parametrize("shape,h,n", [((1, 16, 32), (4e-9, 4e-9, 3e-9), 10), ((4, 8, 16), (3e-9, 3e-9, 3e-9), 10),
+                                       ((2, 5, 7), (4e-9, 4e-9, 4e-9), 10), ((32, 128, 128), (3e-9, 3e-9, 2e-9), 3),
+                                       ((1, 256, 256), (4e-9, 4e-9, 4e-9), 5)])
+def test_rk4_steps_match_the_oracle(shape, h, n):
     nz, ny, nx = shape
     m_host = unit_field(shape, 62)
-    Hext, alpha, dt, n = (-2e4, 4e3, 0.0), 0.1, 1e-13, 10
+    Hext, alpha, dt = (-2e4, 4e3, 0.0), 0.1, 1e-13
     plan = binding.DemagPlan(nx, ny, nz, *h)
     solver = binding.LLG(plan, MS, A_EX, alpha, Hext=Hext)
     m = torch.from_numpy(m_host).cuda()
@@ -62,7 +67,7 @@ def test_rk4_steps_match_the_oracle(shape, h):
     got = m.cpu().numpy()
     assert np.abs((got.astype(np.float64) ** 2).sum(0) - 1).max() <= 1e-6
     assert np.abs(got - ref).max() <= 2e-5                      # 40 fp32 evaluations of fields of ~1e6 A/m
-    assert np.abs(ref - m_host).max() >= 1e-3                   # the steps did move the magnetization
+    assert np.abs(ref - m_host).max() >= 1e-4 * n               # the steps did move the magnetization
     solver.close()
     plan.close()
 
@@ -82,4 +87,17 @@ def test_single_cubic_cell_follows_the_closed_form_damped_precession():
     ref = np.array([np.sqrt(1 - mz ** 2) * np.cos(phi), np.sqrt(1 - mz ** 2) * np.sin(phi), mz])
     assert np.abs(m.cpu().numpy().ravel() - ref).max() <= 2e-5
     solver.close()
+    plan.close()
+
+
+def test_solver_rejects_a_mesh_or_cell_that_differs_from_the_plan():
+    plan = binding.DemagPlan(16, 8, 4, 3e-9, 3e-9, 2e-9)
+    L = binding.lib()
+    assert not L.boris_llg_create(plan._h, 16, 8, 8, 3e-9, 3e-9, 2e-9, MS, A_EX, 0.1, O.GAMMA)
+    assert "differ from the mesh" in binding.last_error()
+    assert not L.boris_llg_create(plan._h, 16, 8, 4, 3e-9, 4e-9, 2e-9, MS, A_EX, 0.1, O.GAMMA)
+    assert "cell sides" in binding.last_error()
+    assert not L.boris_llg_create(plan._h, 16, 8, 4, 3e-9, 3e-9, 2e-9, -1.0, A_EX, 0.1, O.GAMMA)
+    assert "invalid argument" in binding.last_error()
+    assert plan.mesh() == ((16, 8, 4), (3e-9, 3e-9, 2e-9))
     plan.close()
