@@ -21,6 +21,11 @@ are restated in ``oracle/newell.py``), evaluated
   (``oracle/demag_fft.py``).  It is an accelerator for large meshes and is
   itself checked against the double sum.
 
+``oracle/demag_pbc.py`` adds periodic boundary conditions by the multiple-images
+method (Ref. [51]): the same sum over a finite block of copies of the
+mesh, pinned in ``tests/test_oracle_pbc.py`` (the non-periodic double sum over the
+tiled macro-geometry, trace, the infinite-film limit).
+
 All arithmetic is fp64; the tensor is evaluated in x87 extended precision
 (numpy.longdouble) because the closed form cancels catastrophically with
 distance (reading R3).
