@@ -46,6 +46,18 @@ typedef struct boris_demag_plan boris_demag_plan;   /* opaque; owns device memor
  * fp64 on the device, stores it as fp32.  Returns NULL on failure (see last_error). */
 boris_demag_plan* boris_demag_plan_create(int nx, int ny, int nz, double hx, double hy, double hz);
 
+/* The same with periodic boundary conditions by the multiple-images method (section 3: "we
+ * extend this algorithm to use periodic boundary conditions based on the multiple images method [51]"; Ref. [51]
+ * at L434).  images_x / _y / _z >= 0: copies of the mesh on EACH side along x / y / z (0: open boundary; all 0
+ * is boris_demag_plan_create).  The field in the mesh is that of the finite block of (2 images + 1) copies per
+ * periodic direction, all carrying the mesh's own M:
+ *     H(r0) = - sum_{|n_a| <= images_a} sum_r N(r - r0 + (n_x nx hx, n_y ny hy, n_z nz hz)) M(r).
+ * Only the plan-time tensor changes (the copies' tensors are summed into the kernel spectrum in fp64); apply,
+ * energy and every other call work as for an open mesh and cost the same.  Plan time grows with the number
+ * of copies.  Returns NULL on failure (images < 0 or > 1000: -1). */
+boris_demag_plan* boris_demag_plan_create_pbc(int nx, int ny, int nz, double hx, double hy, double hz,
+                                              int images_x, int images_y, int images_z);
+
 /* Free everything the plan owns.  NULL is allowed. */
 void boris_demag_plan_destroy(boris_demag_plan* plan);
 
@@ -142,6 +154,10 @@ int boris_demag_plan_kernel_spectrum(const boris_demag_plan* plan, float* out_ho
  * evaluated on the host with the same source code the device kernel compiles.
  * out[6][nz][ny][nx]: N_c at displacement (i hx, j hy, k hz), c = xx,yy,zz,xy,xz,yz. */
 int boris_demag_tensor_host(int nx, int ny, int nz, double hx, double hy, double hz, double* out);
+
+/* The tensor of boris_demag_plan_create_pbc (the image sum above), same layout.  Small meshes and few copies. */
+int boris_demag_tensor_host_pbc(int nx, int ny, int nz, double hx, double hy, double hz, int images_x, int images_y,
+                                int images_z, double* out);
 
 /* The natural-order reduced kernel spectrum (as boris_demag_plan_kernel_spectrum, in
  * fp64, same folded factor) computed on the host from boris_demag_tensor_host by the

@@ -31,6 +31,10 @@ def lib():
         c_int, c_dbl, c_vp = ctypes.c_int, ctypes.c_double, ctypes.c_void_p
         L.boris_demag_plan_create.restype = c_vp
         L.boris_demag_plan_create.argtypes = [c_int, c_int, c_int, c_dbl, c_dbl, c_dbl]
+        L.boris_demag_plan_create_pbc.restype = c_vp
+        L.boris_demag_plan_create_pbc.argtypes = [c_int, c_int, c_int, c_dbl, c_dbl, c_dbl, c_int, c_int, c_int]
+        L.boris_demag_tensor_host_pbc.restype = c_int
+        L.boris_demag_tensor_host_pbc.argtypes = [c_int, c_int, c_int, c_dbl, c_dbl, c_dbl, c_int, c_int, c_int, c_vp]
         L.boris_demag_plan_destroy.restype = None
         L.boris_demag_plan_destroy.argtypes = [c_vp]
         L.boris_demag_apply.restype = c_int
@@ -95,10 +99,11 @@ def version():
     return lib().boris_demag_version().decode()
 
 
-def tensor_host(nx, ny, nz, hx, hy, hz):
-    """boris_demag_tensor_host: the library's real-space tensor, fp64 [6][nz][ny][nx] (host only)."""
+def tensor_host(nx, ny, nz, hx, hy, hz, images=(0, 0, 0)):
+    """boris_demag_tensor_host[_pbc]: the library's real-space tensor, fp64 [6][nz][ny][nx] (host only)."""
     out = np.empty((6, nz, ny, nx), np.float64)
-    _check(lib().boris_demag_tensor_host(nx, ny, nz, hx, hy, hz, out.ctypes.data), "boris_demag_tensor_host")
+    _check(lib().boris_demag_tensor_host_pbc(nx, ny, nz, hx, hy, hz, *[int(v) for v in images], out.ctypes.data),
+           "boris_demag_tensor_host_pbc")
     return out
 
 
@@ -116,11 +121,16 @@ class DemagPlan:
     M, H are torch CUDA float32 tensors of shape [3, nz, ny, nx] (contiguous).
     """
 
-    def __init__(self, nx, ny, nz, hx, hy, hz):
+    def __init__(self, nx, ny, nz, hx, hy, hz, images=(0, 0, 0)):
+        """images = (ix, iy, iz): copies of the mesh on each side along x, y, z (boris_demag_plan_create_pbc)."""
         self._h = None
         self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
         self.h = (float(hx), float(hy), float(hz))
-        h = lib().boris_demag_plan_create(self.nx, self.ny, self.nz, *self.h)
+        self.images = tuple(int(v) for v in images)
+        if any(self.images):
+            h = lib().boris_demag_plan_create_pbc(self.nx, self.ny, self.nz, *self.h, *self.images)
+        else:
+            h = lib().boris_demag_plan_create(self.nx, self.ny, self.nz, *self.h)
         if not h:
             raise DemagError(f"boris_demag_plan_create failed: {last_error()}")
         self._h = h

@@ -39,12 +39,14 @@ int cuda_fail(cudaError_t e, const char* what) {
 
 
 // ------------------------------------------------------------------ plan-time kernels (fp64)
-__global__ void k_tensor(double* N, int ncomp, int nx, int ny, int nz, double hx, double hy, double hz) {
+struct Images { int per[3]; int img[3]; };      // period in cells and copies per side along x, y, z (plan_math.h)
+
+__global__ void k_tensor(double* N, int ncomp, int nx, int ny, int nz, double hx, double hy, double hz, Images im) {
     const long total = (long)nx * ny * nz;
     for (long idx = blockIdx.x * (long)blockDim.x + threadIdx.x; idx < total; idx += (long)gridDim.x * blockDim.x) {
         const int i = (int)(idx % nx), j = (int)((idx / nx) % ny), k = (int)(idx / ((long)nx * ny));
         double out[6];
-        tensor_point(i, j, k, hx, hy, hz, out);
+        tensor_point_images(i, j, k, im.per, im.img, hx, hy, hz, out);
         for (int c = 0; c < ncomp; ++c) N[c * total + idx] = out[c];
     }
 }
@@ -186,6 +188,7 @@ struct boris_demag_plan {
     // not one the kernels take, it sits in the corner of the next power-of-two mesh whose other cells
     // hold M = 0 (exact: empty cells add nothing to the sum of PAPER.md:L323), staged through Mp / Hp.
     int ux, uy, uz;
+    int images[3] = {0, 0, 0};       // copies per side along x, y, z (periodic boundary conditions; 0: open)
     bool padmode = false;
     float* Mp = nullptr;             // [3][nz][ny][nx], zero outside the caller's cells
     float* Hp = nullptr;
@@ -290,7 +293,8 @@ int build_spectrum(boris_demag_plan* p) {
     const long nA = (long)nc * nz * ny * kl.nxr(), nB = (long)nc * nz * kl.nyr() * kl.nxr(), nC = kl.reduced_elems();
     BD_TRY(cudaMalloc((void**)&dN, (size_t)nc * cells * sizeof(double)));
     BD_TRY(cudaMalloc((void**)&dA, (size_t)nA * sizeof(double)));
-    k_tensor<<<grid_for(cells, 128), 128>>>(dN, nc, nx, ny, nz, p->hx, p->hy, p->hz);
+    const Images im{{p->ux, p->uy, p->uz}, {p->images[0], p->images[1], p->images[2]}};
+    k_tensor<<<grid_for(cells, 128), 128>>>(dN, nc, nx, ny, nz, p->hx, p->hy, p->hz, im);
     BD_TRY(cudaGetLastError());
     if ((rc = upload_cs_table(&csx, kl.Px))) { cleanup(); return rc; }
     if ((rc = upload_cs_table(&csy, kl.Py))) { cleanup(); return rc; }
@@ -349,6 +353,7 @@ int check_sizes(int nx, int ny, int nz, double hx, double hy, double hz) {
 }
 
 int next_pow2(int n) { int p = 1; while (p < n) p <<= 1; return p; }
+constexpr int kMaxImages = 1000;
 
 // (used by the entry points below)
 // caller's mesh [3][uz][uy][ux] <-> its corner of the kernels' mesh [3][nz][ny][nx]
@@ -399,8 +404,18 @@ void boris_demag_plan_destroy(boris_demag_plan* p) {
 }
 
 boris_demag_plan* boris_demag_plan_create(int ux, int uy, int uz, double hx, double hy, double hz) {
+    return boris_demag_plan_create_pbc(ux, uy, uz, hx, hy, hz, 0, 0, 0);
+}
+
+boris_demag_plan* boris_demag_plan_create_pbc(int ux, int uy, int uz, double hx, double hy, double hz, int images_x,
+                                              int images_y, int images_z) {
     g_err.clear();
     if (check_sizes(ux, uy, uz, hx, hy, hz)) return nullptr;
+    if (images_x < 0 || images_y < 0 || images_z < 0 || images_x > kMaxImages || images_y > kMaxImages ||
+        images_z > kMaxImages) {
+        fail(-1, "images per side must be in [0, 1000]");
+        return nullptr;
+    }
     // the kernels take power-of-two meshes: nx >= 4, ny >= 2, nz = 1 or >= 2
     const int nx = next_pow2(ux < 4 ? 4 : ux), ny = next_pow2(uy < 2 ? 2 : uy), nz = uz == 1 ? 1 : next_pow2(uz);
     int dev = 0;
@@ -410,6 +425,7 @@ boris_demag_plan* boris_demag_plan_create(int ux, int uy, int uz, double hx, dou
     if (!p) { fail(-3, "out of host memory"); return nullptr; }
     p->nx = nx; p->ny = ny; p->nz = nz; p->hx = hx; p->hy = hy; p->hz = hz; p->device = dev;
     p->ux = ux; p->uy = uy; p->uz = uz;
+    p->images[0] = images_x; p->images[1] = images_y; p->images[2] = images_z;
     p->padmode = nx != ux || ny != uy || nz != uz;
     const int Py = 2 * ny, Pz = nz > 1 ? 2 * nz : 1;
     p->cfg = bd::make_launch_cfg(nx, ny, nz);
@@ -741,12 +757,20 @@ int boris_demag_plan_kernel_spectrum(const boris_demag_plan* p, float* out_host)
 
 // ---- host-only entry points ----------------------------------------------------------
 int boris_demag_tensor_host(int nx, int ny, int nz, double hx, double hy, double hz, double* out) {
-    if (!out || nx < 1 || ny < 1 || nz < 1 || !(hx > 0) || !(hy > 0) || !(hz > 0)) return fail(-1, "invalid argument");
+    return boris_demag_tensor_host_pbc(nx, ny, nz, hx, hy, hz, 0, 0, 0, out);
+}
+
+int boris_demag_tensor_host_pbc(int nx, int ny, int nz, double hx, double hy, double hz, int images_x, int images_y,
+                                int images_z, double* out) {
+    if (!out || nx < 1 || ny < 1 || nz < 1 || !(hx > 0) || !(hy > 0) || !(hz > 0) || images_x < 0 || images_y < 0 ||
+        images_z < 0)
+        return fail(-1, "invalid argument");
     const long cells = (long)nx * ny * nz;
+    const int per[3] = {nx, ny, nz}, img[3] = {images_x, images_y, images_z};
     for (long idx = 0; idx < cells; ++idx) {
         const int i = (int)(idx % nx), j = (int)((idx / nx) % ny), k = (int)(idx / ((long)nx * ny));
         double v[6];
-        bd::tensor_point(i, j, k, hx, hy, hz, v);
+        bd::tensor_point_images(i, j, k, per, img, hx, hy, hz, v);
         for (int c = 0; c < 6; ++c) out[c * cells + idx] = v[c];
     }
     return 0;

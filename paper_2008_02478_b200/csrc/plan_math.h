@@ -123,6 +123,37 @@ BD_HD void tensor_point(int i, int j, int k, double hx, double hy, double hz, do
     if (k == 0) { out[4] = 0.0; out[5] = 0.0; }
 }
 
+// Periodic boundary conditions by the multiple-images method (Ref. [51]; reading R15):
+// the tensor of a mesh repeated `img[d]` times on each side along dimension d with period per[d] cells,
+//     N^img_c(i, j, k) = sum_{|a| <= img[0]} sum_{|b| <= img[1]} sum_{|e| <= img[2]} N_c(i + a per[0], j + b per[1], k + e per[2]),
+// negative displacements by the parity of the component.  img = (0, 0, 0) is tensor_point itself.
+BD_HD void tensor_point_images(int i, int j, int k, const int per[3], const int img[3], double hx, double hy, double hz,
+                               double out[6]) {
+    if (img[0] == 0 && img[1] == 0 && img[2] == 0) { tensor_point(i, j, k, hx, hy, hz, out); return; }
+    double acc[6] = {0, 0, 0, 0, 0, 0};
+    // far copies first: the small terms are added before the large ones
+    for (int e = img[2]; e >= -img[2]; e = (e > 0 ? -e : -e - 1)) {
+        for (int b = img[1]; b >= -img[1]; b = (b > 0 ? -b : -b - 1)) {
+            for (int a = img[0]; a >= -img[0]; a = (a > 0 ? -a : -a - 1)) {
+                const int ii = i + a * per[0], jj = j + b * per[1], kk = k + e * per[2];
+                const double sx = ii < 0 ? -1.0 : 1.0, sy = jj < 0 ? -1.0 : 1.0, sz = kk < 0 ? -1.0 : 1.0;
+                double t[6];
+                tensor_point(ii < 0 ? -ii : ii, jj < 0 ? -jj : jj, kk < 0 ? -kk : kk, hx, hy, hz, t);
+                acc[0] += t[0]; acc[1] += t[1]; acc[2] += t[2];
+                acc[3] += sx * sy * t[3]; acc[4] += sx * sz * t[4]; acc[5] += sy * sz * t[5];
+                if (a == 0) break;
+            }
+            if (b == 0) break;
+        }
+        if (e == 0) break;
+    }
+    for (int c = 0; c < 6; ++c) out[c] = acc[c];
+    // the symmetric block of copies keeps every component's parity: exact zeros on the nodal planes
+    if (i == 0) { out[3] = 0.0; out[4] = 0.0; }
+    if (j == 0) { out[3] = 0.0; out[5] = 0.0; }
+    if (k == 0) { out[4] = 0.0; out[5] = 0.0; }
+}
+
 // parity of component c along dimension d (0 = x, 1 = y, 2 = z): true = odd
 BD_HD bool comp_is_odd(int c, int d) {
     return (c == 3 && (d == 0 || d == 1)) || (c == 4 && (d == 0 || d == 2)) || (c == 5 && (d == 1 || d == 2));

@@ -49,6 +49,25 @@ def test_library_tensor_agrees_with_oracle_tensor(dims, h):
     assert np.abs(tr).max() < 2e-12            # pin P1 on the library's tensor
 
 
+@pytest.mark.parametrize("shape,h,images", [((1, 6, 5), (4.0, 3.0, 2.0), (3, 2, 0)), ((3, 4, 5), (2.0, 3.0, 1.0), (2, 0, 1)),
+                                            ((2, 12, 20), (2.0, 2.0, 1.0), (4, 0, 0)), ((1, 16, 16), (4.0, 4.0, 1.0), (12, 12, 0))])
+def test_library_image_summed_tensor_agrees_with_oracle(shape, h, images):
+    """Periodic boundary conditions: the library's sum over copies (plan_math.h, Gauss-quadrature far
+    field) against the oracle's (oracle/demag_pbc.py, x87 Newell everywhere)."""
+    from oracle.demag_pbc import image_tensor_table
+    build.build()
+    nz, ny, nx = shape
+    lib_T = binding.tensor_host(nx, ny, nz, *h, images=images)
+    ora_T = image_tensor_table(shape, h, images)
+    # one copy: 2e-11 as above; every further copy adds its own far-field error (library quadrature <= 3e-13 beyond 10 cells)
+    copies = (2 * images[0] + 1) * (2 * images[1] + 1) * (2 * images[2] + 1)
+    assert np.abs(lib_T - ora_T).max() < 2e-11 + 3e-13 * copies
+    tr = lib_T[0] + lib_T[1] + lib_T[2]
+    tr[0, 0, 0] -= 1
+    assert np.abs(tr).max() < 1e-11
+    assert np.abs(lib_T - binding.tensor_host(nx, ny, nz, *h)).max() > 1e-5          # the copies do change it
+
+
 @pytest.mark.parametrize("shape,h", [((1, 8, 16), (5.0, 5.0, 3.0)), ((4, 6, 8), (5.0, 4.0, 3.0)),
                                      ((1, 64, 32), (2.0, 2.0, 1.0)), ((8, 16, 16), (2.0, 2.0, 1.0))])
 def test_library_spectrum_agrees_with_oracle_spectrum(shape, h):
