@@ -6,6 +6,7 @@
 #include <cuda_runtime.h>
 
 #include <atomic>
+#include <cstdlib>
 #include <type_traits>
 #include <vector>
 
@@ -27,9 +28,17 @@ struct MinBlocks { static constexpr int value = 1; };
 template <class K>
 struct MinBlocks<K, std::void_t<decltype(K::MINB)>> { static constexpr int value = K::MINB; };
 
+// The kernels of one evaluation are launched with programmatic stream serialization: a kernel's blocks may
+// become resident while the last blocks of its predecessor drain (launch_dependents at the top lets the
+// successor's launch begin once every block of this grid has started), and wait here until the predecessor
+// grid has completed and its writes are visible.  Every kernel of the library waits before it touches memory,
+// so completion orders chain: nothing runs ahead of data it reads or overwrites.  Outside such a launch both
+// instructions are no-ops.
 template <class K>
 __global__ void __launch_bounds__(K::NT, MinBlocks<K>::value) phase_kernel(const __grid_constant__ typename K::Args a) {
     extern __shared__ __align__(16) float2 bd_smem[];
+    asm volatile("griddepcontrol.launch_dependents;");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     run_phases<K, 0>(a, bd_smem);
 }
 
@@ -47,10 +56,17 @@ int cu_plane_yz(CudaLauncher& run, const PlanView& p);                          
 
 constexpr int kMaxDevices = 64;
 
+// BORIS_DEMAG_NO_PDL=1 in the environment launches the kernels plainly (A/B measurements)
+inline bool pdl_enabled() {
+    static const bool on = [] { const char* v = getenv("BORIS_DEMAG_NO_PDL"); return !(v && v[0] == '1'); }();
+    return on;
+}
+
 struct CudaLauncher {
     cudaStream_t st;
     int dev = 0;                                   // the plan's device (the current one: checked by the entry points)
     cudaError_t err = cudaSuccess;
+    bool pdl = pdl_enabled();                      // programmatic dependent launch between the kernels of an evaluation
     std::vector<TimedLaunch>* timed = nullptr;     // boris_demag_apply_timed only
     template <class K>
     int run(Grid g, const typename K::Args& a) {
@@ -78,8 +94,17 @@ struct CudaLauncher {
             size_t seen = opted[d].load(std::memory_order_relaxed);
             while (seen < smem && !opted[d].compare_exchange_weak(seen, smem, std::memory_order_relaxed)) {}
         }
-        phase_kernel<K><<<dim3(g.x, g.y), K::NT, smem, st>>>(a);
-        err = cudaGetLastError();
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(g.x, g.y);
+        cfg.blockDim = dim3(K::NT);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = pdl ? 1 : 0;
+        err = cudaLaunchKernelEx(&cfg, phase_kernel<K>, a);
         return err == cudaSuccess ? 0 : -2;
     }
     // hooks of enqueue_apply (apply_seq.h)
