@@ -505,6 +505,30 @@ def main():
             del mu
         except Exception as e:
             print(f"[bench] LLG evaluation timing skipped: {e}", file=sys.stderr)
+    # the double-precision variant (include/boris_demag_f64.h; "single or double"): side information
+    if world == 1:
+        try:
+            p64 = binding.DemagPlanF64(cfg.nx, cfg.ny, cfg.nz, *cfg.h)
+            M64 = M.double()
+            H64 = torch.empty_like(M64)
+            for _ in range(2):
+                p64.apply(M64, H64)
+            torch.cuda.synchronize()
+            fa, fb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            nrep = 5
+            fa.record(torch.cuda.current_stream())
+            for _ in range(nrep):
+                p64.apply(M64, H64)
+            fb.record(torch.cuda.current_stream())
+            torch.cuda.synchronize()
+            ms64 = fa.elapsed_time(fb) / nrep
+            dev = (H64.float() - H).abs().max().item() / cfg.Ms
+            line["f64"] = {"ms_per_evaluation": ms64, "evaluations_per_s": 1e3 / ms64, "kernel_launches": 5,
+                           "max_abs_diff_to_f32_over_Ms": dev, "workspace_bytes": p64.info()["workspace_bytes"]}
+            p64.close()
+            del M64, H64
+        except Exception as e:
+            print(f"[bench] fp64 variant timing skipped: {e}", file=sys.stderr)
     del plan, M, H, E
     torch.cuda.empty_cache()
     if world == 1 and not args.no_all_configs:

@@ -76,6 +76,16 @@ def lib():
         L.boris_llg_effective_field.argtypes = [c_vp, c_vp, c_vp, c_vp]
         L.boris_llg_rk4.restype = c_int
         L.boris_llg_rk4.argtypes = [c_vp, c_vp, c_dbl, c_int, c_vp]
+        L.boris_demag_f64_plan_create.restype = c_vp
+        L.boris_demag_f64_plan_create.argtypes = [c_int, c_int, c_int, c_dbl, c_dbl, c_dbl, c_int, c_int, c_int]
+        L.boris_demag_f64_plan_destroy.restype = None
+        L.boris_demag_f64_plan_destroy.argtypes = [c_vp]
+        L.boris_demag_f64_apply.restype = c_int
+        L.boris_demag_f64_apply.argtypes = [c_vp, c_vp, c_vp, c_vp]
+        L.boris_demag_f64_energy.restype = c_int
+        L.boris_demag_f64_energy.argtypes = [c_vp, c_vp, c_vp, c_vp, c_vp]
+        L.boris_demag_f64_plan_info.restype = c_int
+        L.boris_demag_f64_plan_info.argtypes = [c_vp, ctypes.POINTER(ctypes.c_longlong), ctypes.POINTER(c_int), ctypes.POINTER(c_int)]
         L.boris_demag_plan_mesh.restype = c_int
         L.boris_demag_plan_mesh.argtypes = [c_vp, ctypes.POINTER(c_int), ctypes.POINTER(c_dbl)]
         L.boris_micro_fp32_rate.restype = c_int
@@ -305,6 +315,61 @@ class LLG:
             self.close()
         except Exception:
             pass
+
+
+# ----------------------------------------------------------------- fp64 variant (include/boris_demag_f64.h)
+class DemagPlanF64:
+    """boris_demag_f64_plan_create / apply / energy.  M, H: torch CUDA float64 tensors [3, nz, ny, nx] (contiguous)."""
+
+    def __init__(self, nx, ny, nz, hx, hy, hz, images=(0, 0, 0)):
+        self._h = None
+        self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
+        self.h = (float(hx), float(hy), float(hz))
+        h = lib().boris_demag_f64_plan_create(self.nx, self.ny, self.nz, *self.h, *[int(v) for v in images])
+        if not h:
+            raise DemagError(f"boris_demag_f64_plan_create failed: {last_error()}")
+        self._h = h
+
+    def close(self):
+        if self._h:
+            lib().boris_demag_f64_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _ptr(self, t, name):
+        import torch
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+                and tuple(t.shape) == (3, self.nz, self.ny, self.nx)):
+            raise DemagError(f"{name} must be a contiguous CUDA float64 tensor of shape {(3, self.nz, self.ny, self.nx)}")
+        return t.data_ptr()
+
+    @staticmethod
+    def _stream(stream):
+        import torch
+        return (stream or torch.cuda.current_stream()).cuda_stream
+
+    def apply(self, M, H, stream=None):
+        _check(lib().boris_demag_f64_apply(self._h, self._ptr(M, "M"), self._ptr(H, "H"), self._stream(stream)),
+               "boris_demag_f64_apply")
+        return H
+
+    def energy(self, M, H, stream=None):
+        import torch
+        E = torch.zeros(1, dtype=torch.float64, device=M.device)
+        _check(lib().boris_demag_f64_energy(self._h, self._ptr(M, "M"), self._ptr(H, "H"), E.data_ptr(),
+                                            self._stream(stream)), "boris_demag_f64_energy")
+        return E
+
+    def info(self):
+        ws, nl = ctypes.c_longlong(), ctypes.c_int()
+        padded = (ctypes.c_int * 3)()
+        _check(lib().boris_demag_f64_plan_info(self._h, ctypes.byref(ws), padded, ctypes.byref(nl)), "boris_demag_f64_plan_info")
+        return {"workspace_bytes": ws.value, "padded": tuple(padded), "kernel_launches": nl.value}
 
 
 # ----------------------------------------------------------------- device probes (include/boris_micro.h)

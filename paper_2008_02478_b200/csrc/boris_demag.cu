@@ -183,6 +183,7 @@ int grid_for(long total, int threads) {
 namespace bd {
 int micro_fail(cudaError_t e, const char* what) { return cuda_fail(e, what); }
 int set_error(int code, const char* msg) { return fail(code, msg); }
+void clear_error() { g_err.clear(); }
 }  // namespace bd
 
 // ------------------------------------------------------------------ plan
@@ -277,10 +278,10 @@ int upload_cs_table(double2** dst, int P) {
     return 0;
 }
 
-// Build the kernel spectrum on the device (fp64), store it as fp32 in fused-pass order.
-int build_spectrum(boris_demag_plan* p) {
-    const bd::KLayout& kl = p->kl;
-    const int nx = p->nx, ny = p->ny, nz = p->nz, nc = kl.ncomp;
+// The natural, symmetry-reduced spectrum Kred[c][kz][ky][kx] of khat_layout.h on the device (fp64), with the
+// factor of reading R12 folded in.  *out is cudaMalloc'ed here; the caller frees it.
+int build_reduced(const bd::KLayout& kl, double hx, double hy, double hz, const Images& im, double** out) {
+    const int nx = kl.nx, ny = kl.ny, nz = kl.nz, nc = kl.ncomp;
     const long cells = (long)nx * ny * nz;
     double *dN = nullptr, *dA = nullptr, *dB = nullptr, *dC = nullptr;
     double2 *csx = nullptr, *csy = nullptr, *csz = nullptr;
@@ -296,8 +297,7 @@ int build_spectrum(boris_demag_plan* p) {
     const long nA = (long)nc * nz * ny * kl.nxr(), nB = (long)nc * nz * kl.nyr() * kl.nxr(), nC = kl.reduced_elems();
     BD_TRY(cudaMalloc((void**)&dN, (size_t)nc * cells * sizeof(double)));
     BD_TRY(cudaMalloc((void**)&dA, (size_t)nA * sizeof(double)));
-    const Images im{{p->ux, p->uy, p->uz}, {p->images[0], p->images[1], p->images[2]}};
-    k_tensor<<<grid_for(cells, 128), 128>>>(dN, nc, nx, ny, nz, p->hx, p->hy, p->hz, im);
+    k_tensor<<<grid_for(cells, 128), 128>>>(dN, nc, nx, ny, nz, hx, hy, hz, im);
     BD_TRY(cudaGetLastError());
     if ((rc = upload_cs_table(&csx, kl.Px))) { cleanup(); return rc; }
     if ((rc = upload_cs_table(&csy, kl.Py))) { cleanup(); return rc; }
@@ -319,6 +319,28 @@ int build_spectrum(boris_demag_plan* p) {
     const double scale = -1.0 / (2.0 * (double)kl.Px * (double)kl.Py * (double)kl.Pz);
     k_scale_sign<<<grid_for(nC, 256), 256>>>(dC, kl, scale);
     BD_TRY(cudaGetLastError());
+    BD_TRY(cudaDeviceSynchronize());
+#undef BD_TRY
+    *out = dC;
+    dC = nullptr;
+    cleanup();
+    return 0;
+}
+
+// Build the kernel spectrum on the device (fp64), store it as fp32 in fused-pass order.
+int build_spectrum(boris_demag_plan* p) {
+    const bd::KLayout& kl = p->kl;
+    const int nx = p->nx, ny = p->ny, nz = p->nz;
+    double* dC = nullptr;
+    const Images im{{p->ux, p->uy, p->uz}, {p->images[0], p->images[1], p->images[2]}};
+    int rc = build_reduced(kl, p->hx, p->hy, p->hz, im, &dC);
+    if (rc) return rc;
+    auto cleanup = [&]() { cudaFree(dC); };
+#define BD_TRY(call)                                                              \
+    do {                                                                          \
+        cudaError_t e_ = (call);                                                  \
+        if (e_ != cudaSuccess) { rc = cuda_fail(e_, #call); cleanup(); return rc; } \
+    } while (0)
     if (p->cfg.plane.on) {
         const bd::PlaneGeom& g = p->cfg.plane;
         const bd::PlaneK pk = bd::make_plane_k(nx, ny, nz, g);
@@ -390,6 +412,17 @@ __global__ void k_crop(const float* __restrict__ src, float* __restrict__ dst, i
 }
 
 }  // namespace
+
+namespace bd {
+// for the fp64 engine (boris_demag_f64.cu): the reduced fp64 spectrum of a power-of-two mesh nx x ny x nz whose
+// copies repeat with period per[] cells, img[] copies a side; *out is cudaMalloc'ed, the caller frees it
+int build_reduced_spectrum(int nx, int ny, int nz, double hx, double hy, double hz, const int per[3], const int img[3],
+                           double** out) {
+    const Images im{{per[0], per[1], per[2]}, {img[0], img[1], img[2]}};
+    return build_reduced(bd::make_klayout(nx, ny, nz, 1), hx, hy, hz, im, out);
+}
+int check_mesh_args(int nx, int ny, int nz, double hx, double hy, double hz) { return check_sizes(nx, ny, nz, hx, hy, hz); }
+}  // namespace bd
 
 extern "C" {
 
