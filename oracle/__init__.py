@@ -26,6 +26,12 @@ method (Ref. [51]): the same sum over a finite block of copies of 
 mesh, pinned in ``tests/test_oracle_pbc.py`` (the non-periodic double sum over the
 tiled macro-geometry, trace, the infinite-film limit).
 
+``oracle/multilayer.py`` is the multi-layered convolution of PAPER.md:L71-L76 (Eq. 4)
+for a stack of one-cell-thick layers of unequal thickness at arbitrary heights
+(reading R17), pinned in ``tests/test_oracle_multilayer.py`` (brute-force
+quadrature between unequal cuboids, additivity, reciprocity, the single-mesh double
+sum on a stack that sits on a common grid).
+
 All arithmetic is fp64; the tensor is evaluated in x87 extended precision
 (numpy.longdouble) because the closed form cancels catastrophically with
 distance (reading R3).
