@@ -86,6 +86,16 @@ def lib():
         L.boris_demag_f64_energy.argtypes = [c_vp, c_vp, c_vp, c_vp, c_vp]
         L.boris_demag_f64_plan_info.restype = c_int
         L.boris_demag_f64_plan_info.argtypes = [c_vp, ctypes.POINTER(ctypes.c_longlong), ctypes.POINTER(c_int), ctypes.POINTER(c_int)]
+        L.boris_demag_ml_plan_create.restype = c_vp
+        L.boris_demag_ml_plan_create.argtypes = [c_int, c_int, c_int, c_dbl, c_dbl, c_vp, c_vp, c_int]
+        L.boris_demag_ml_plan_destroy.restype = None
+        L.boris_demag_ml_plan_destroy.argtypes = [c_vp]
+        L.boris_demag_ml_apply.restype = c_int
+        L.boris_demag_ml_apply.argtypes = [c_vp, c_vp, c_vp, c_vp]
+        L.boris_demag_ml_energy.restype = c_int
+        L.boris_demag_ml_energy.argtypes = [c_vp, c_vp, c_vp, c_vp, c_vp]
+        L.boris_demag_ml_pair_tensor_host.restype = c_int
+        L.boris_demag_ml_pair_tensor_host.argtypes = [c_int, c_int, c_dbl, c_dbl, c_dbl, c_dbl, c_dbl, c_vp]
         L.boris_demag_plan_mesh.restype = c_int
         L.boris_demag_plan_mesh.argtypes = [c_vp, ctypes.POINTER(c_int), ctypes.POINTER(c_dbl)]
         L.boris_micro_fp32_rate.restype = c_int
@@ -370,6 +380,65 @@ class DemagPlanF64:
         padded = (ctypes.c_int * 3)()
         _check(lib().boris_demag_f64_plan_info(self._h, ctypes.byref(ws), padded, ctypes.byref(nl)), "boris_demag_f64_plan_info")
         return {"workspace_bytes": ws.value, "padded": tuple(padded), "kernel_launches": nl.value}
+
+
+# ----------------------------------------------------------------- multi-layered convolution (include/boris_demag_ml.h)
+def ml_pair_tensor_host(nx, ny, hx, hy, tk, ti, Z):
+    """boris_demag_ml_pair_tensor_host: the library's tensor between unequal cuboids, fp64 [6][ny][nx] (host only)."""
+    out = np.empty((6, ny, nx), np.float64)
+    _check(lib().boris_demag_ml_pair_tensor_host(nx, ny, hx, hy, tk, ti, Z, out.ctypes.data), "boris_demag_ml_pair_tensor_host")
+    return out
+
+
+class MultiLayerPlan:
+    """boris_demag_ml_plan_create / apply / energy.  M, H: torch CUDA tensors [3, nlayers, ny, nx], float32 or (fp64=True)
+    float64, contiguous.  thickness, z_centre: per-layer cell height and centre height in metres."""
+
+    def __init__(self, nx, ny, hx, hy, thickness, z_centre, fp64=False):
+        self._h = None
+        t = np.ascontiguousarray(thickness, np.float64)
+        z = np.ascontiguousarray(z_centre, np.float64)
+        if t.ndim != 1 or t.shape != z.shape:
+            raise DemagError("thickness and z_centre must be 1-D arrays of the same length")
+        self.nx, self.ny, self.n, self.fp64 = int(nx), int(ny), int(t.size), bool(fp64)
+        h = lib().boris_demag_ml_plan_create(self.nx, self.ny, self.n, float(hx), float(hy), t.ctypes.data, z.ctypes.data,
+                                             1 if fp64 else 0)
+        if not h:
+            raise DemagError(f"boris_demag_ml_plan_create failed: {last_error()}")
+        self._h = h
+
+    def close(self):
+        if self._h:
+            lib().boris_demag_ml_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _ptr(self, t, name):
+        import torch
+        want = torch.float64 if self.fp64 else torch.float32
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == want and t.is_contiguous()
+                and tuple(t.shape) == (3, self.n, self.ny, self.nx)):
+            raise DemagError(f"{name} must be a contiguous CUDA {want} tensor of shape {(3, self.n, self.ny, self.nx)}")
+        return t.data_ptr()
+
+    def apply(self, M, H, stream=None):
+        import torch
+        st = (stream or torch.cuda.current_stream()).cuda_stream
+        _check(lib().boris_demag_ml_apply(self._h, self._ptr(M, "M"), self._ptr(H, "H"), st), "boris_demag_ml_apply")
+        return H
+
+    def energy(self, M, H, stream=None):
+        import torch
+        st = (stream or torch.cuda.current_stream()).cuda_stream
+        E = torch.zeros(1, dtype=torch.float64, device=M.device)
+        _check(lib().boris_demag_ml_energy(self._h, self._ptr(M, "M"), self._ptr(H, "H"), E.data_ptr(), st),
+               "boris_demag_ml_energy")
+        return E
 
 
 # ----------------------------------------------------------------- device probes (include/boris_micro.h)

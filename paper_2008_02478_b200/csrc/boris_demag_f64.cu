@@ -7,11 +7,11 @@
 // multiplication and the inverse z FFT for all three components (the z-padded spectrum exists only in shared
 // memory), then inverse y and inverse x FFTs: five launches.
 //
-//   k64_x_fwd   S1     M [3][uz][uy][ux] real  -> X[3][nz][ny][nx+1]            (zero padding to Px = 2 nx on load)
-//   k64_y<fwd>  S2     X -> Y[3][nz][Py][nx+1]                                   (y in bit-reversed order)
-//   k64_z_mul   S3-S5  Y -> Y in place, per (ky, kx): z FFT, H^ = K^ M^, inverse z FFT, first nz kept
-//   k64_y<inv>  S6     Y -> X, first ny kept
-//   k64_x_inv   S7     X -> H, Hermitian half spectrum -> real row, first ux kept
+//   x_fwd       S1     M [3][uz][uy][ux] real  -> X[3][nz][ny][nx+1]            (simple_engine.cuh; zero padding on load)
+//   y_pass<fwd> S2     X -> Y[3][nz][Py][nx+1]                                   (y in bit-reversed order)
+//   k64_z_mul   S3-S5  Y -> Y in place, per (ky, kx): z FFT, H^ = K^ M^, inverse z FFT, first nz kept   (this file)
+//   y_pass<inv> S6     Y -> X, first ny kept
+//   x_inv       S7     X -> H, Hermitian half spectrum -> real row, first ux kept
 //
 // Transforms: in-place radix-2 in shared memory, decimation in frequency forward (natural -> bit-reversed),
 // decimation in time inverse (bit-reversed -> natural): nothing is reordered, the multiply looks the frequency of
@@ -26,6 +26,7 @@
 #include <vector>
 
 #include "../../include/boris_demag_f64.h"
+#include "simple_engine.cuh"
 
 namespace bd {
 int micro_fail(cudaError_t e, const char* what);
@@ -38,131 +39,15 @@ int check_mesh_args(int nx, int ny, int nz, double hx, double hy, double hz);
 
 namespace {
 
+using namespace se;
 constexpr double kPi64 = 3.14159265358979323846264338327950288;
-constexpr int kThreads = 256;
-
-__device__ __forceinline__ double2 c_add(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ double2 c_sub(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
-__device__ __forceinline__ double2 c_mul(double2 a, double2 w) { return make_double2(a.x * w.x - a.y * w.y, a.x * w.y + a.y * w.x); }
-__device__ __forceinline__ double2 c_mulc(double2 a, double2 w) { return make_double2(a.x * w.x + a.y * w.y, a.y * w.x - a.x * w.y); }
-
-// `batch` pencils of L = 2^logL points, pencil b at s + b * L.  tw[k] = exp(-2 pi i k / L), k < L / 2.
-// Forward: decimation in frequency, natural order in, bit-reversed order out.
-__device__ void fft_dif(double2* s, int L, int logL, int batch, const double2* __restrict__ tw) {
-    for (int st = 0; st < logL; ++st) {
-        const int half = L >> (st + 1);
-        for (int w = threadIdx.x; w < batch * (L / 2); w += blockDim.x) {
-            const int b = w / (L / 2), r = w - b * (L / 2);
-            const int g = r / half, j = r - g * half;
-            double2* p = s + (size_t)b * L + g * 2 * half + j;
-            const double2 x0 = p[0], x1 = p[half];
-            p[0] = c_add(x0, x1);
-            p[half] = c_mul(c_sub(x0, x1), tw[j << st]);
-        }
-        __syncthreads();
-    }
-}
-// Inverse (unnormalised): decimation in time, bit-reversed order in, natural order out.
-__device__ void fft_dit_inv(double2* s, int L, int logL, int batch, const double2* __restrict__ tw) {
-    for (int st = logL - 1; st >= 0; --st) {
-        const int half = L >> (st + 1);
-        for (int w = threadIdx.x; w < batch * (L / 2); w += blockDim.x) {
-            const int b = w / (L / 2), r = w - b * (L / 2);
-            const int g = r / half, j = r - g * half;
-            double2* p = s + (size_t)b * L + g * 2 * half + j;
-            const double2 x0 = p[0], x1 = c_mulc(p[half], tw[j << st]);
-            p[0] = c_add(x0, x1);
-            p[half] = c_sub(x0, x1);
-        }
-        __syncthreads();
-    }
-}
-__device__ __forceinline__ int bitrev(int v, int bits) { return bits == 0 ? 0 : (int)(__brev((unsigned)v) >> (32 - bits)); }
-
-struct Geo {
-    int ux, uy, uz;        // the caller's mesh
-    int nx, ny, nz;        // the power-of-two mesh the transforms work on
-    int Px, Py, Pz, lx, ly, lz;   // padded lengths and their log2 (Pz = 1, lz = 0 when nz = 1)
-    int nxr;               // nx + 1 frequencies along x
-};
-
-// S1: one block per row (c, z, y) of the power-of-two mesh
-__global__ void __launch_bounds__(kThreads) k64_x_fwd(const double* __restrict__ M, double2* __restrict__ X, Geo g,
-                                                       const double2* __restrict__ twx) {
-    extern __shared__ double2 sm64[];
-    const int row = blockIdx.x, y = row % g.ny, z = (row / g.ny) % g.nz, c = row / (g.ny * g.nz);
-    double2* out = X + (size_t)row * g.nxr;
-    if (y >= g.uy || z >= g.uz) {                       // a row of the zero padding around the caller's mesh
-        for (int k = threadIdx.x; k < g.nxr; k += blockDim.x) out[k] = make_double2(0.0, 0.0);
-        return;
-    }
-    const double* in = M + (((size_t)c * g.uz + z) * g.uy + y) * g.ux;
-    for (int i = threadIdx.x; i < g.Px; i += blockDim.x) sm64[i] = make_double2(i < g.ux ? in[i] : 0.0, 0.0);
-    __syncthreads();
-    fft_dif(sm64, g.Px, g.lx, 1, twx);
-    for (int k = threadIdx.x; k < g.nxr; k += blockDim.x) out[k] = sm64[bitrev(k, g.lx)];
-}
-
-// S7: Hermitian half spectrum -> real row
-__global__ void __launch_bounds__(kThreads) k64_x_inv(const double2* __restrict__ X, double* __restrict__ H, Geo g,
-                                                       const double2* __restrict__ twx) {
-    extern __shared__ double2 sm64[];
-    const int row = blockIdx.x, y = row % g.ny, z = (row / g.ny) % g.nz, c = row / (g.ny * g.nz);
-    if (y >= g.uy || z >= g.uz) return;
-    const double2* in = X + (size_t)row * g.nxr;
-    for (int k = threadIdx.x; k < g.nxr; k += blockDim.x) {
-        double2 v = in[k];
-        if (k == 0 || k == g.nx) v.y = 0.0;               // DC and Nyquist of a real row are real
-        sm64[bitrev(k, g.lx)] = v;
-        if (k > 0 && k < g.nx) sm64[bitrev(g.Px - k, g.lx)] = make_double2(v.x, -v.y);
-    }
-    __syncthreads();
-    fft_dit_inv(sm64, g.Px, g.lx, 1, twx);
-    double* out = H + (((size_t)c * g.uz + z) * g.uy + y) * g.ux;
-    for (int i = threadIdx.x; i < g.ux; i += blockDim.x) out[i] = sm64[i].x;
-}
-
-// S2 / S6: block = tc consecutive kx of one (c, z); pencils along y (element stride nxr)
-template <bool INV>
-__global__ void __launch_bounds__(kThreads) k64_y(double2* __restrict__ X, double2* __restrict__ Y, Geo g, int tc,
-                                                  const double2* __restrict__ twy) {
-    extern __shared__ double2 sm64[];
-    const int tiles = (g.nxr + tc - 1) / tc;
-    const int cz = blockIdx.x / tiles, k0 = (blockIdx.x - cz * tiles) * tc;
-    const int cols = min(tc, g.nxr - k0);
-    double2* x = X + (size_t)cz * g.ny * g.nxr + k0;
-    double2* yv = Y + (size_t)cz * g.Py * g.nxr + k0;
-    if (!INV) {
-        for (int w = threadIdx.x; w < g.Py * tc; w += blockDim.x) {
-            const int e = w / tc, col = w - e * tc;
-            sm64[(size_t)col * g.Py + e] = (e < g.ny && col < cols) ? x[(size_t)e * g.nxr + col] : make_double2(0.0, 0.0);
-        }
-        __syncthreads();
-        fft_dif(sm64, g.Py, g.ly, tc, twy);
-        for (int w = threadIdx.x; w < g.Py * tc; w += blockDim.x) {
-            const int e = w / tc, col = w - e * tc;
-            if (col < cols) yv[(size_t)e * g.nxr + col] = sm64[(size_t)col * g.Py + e];
-        }
-    } else {
-        for (int w = threadIdx.x; w < g.Py * tc; w += blockDim.x) {
-            const int e = w / tc, col = w - e * tc;
-            sm64[(size_t)col * g.Py + e] = col < cols ? yv[(size_t)e * g.nxr + col] : make_double2(0.0, 0.0);
-        }
-        __syncthreads();
-        fft_dit_inv(sm64, g.Py, g.ly, tc, twy);
-        for (int w = threadIdx.x; w < g.ny * tc; w += blockDim.x) {
-            const int e = w / tc, col = w - e * tc;
-            if (col < cols) x[(size_t)e * g.nxr + col] = sm64[(size_t)col * g.Py + e];
-        }
-    }
-}
 
 // S3 + S4 + S5 (the pipelined step of PAPER.md:L275): block = tc consecutive kx at one y position, all 3 components.
 // Kred[c][kz <= Pz/2][ky <= Py/2][kx]: real, with -1/(2 Px Py Pz) folded in (x 2 here: these are plain complex
 // transforms, reading R12); a mirrored frequency reads the stored value with the sign of the odd components.
 __global__ void __launch_bounds__(kThreads) k64_z_mul(double2* __restrict__ Y, const double* __restrict__ Kred, Geo g, int tc,
                                                       const double2* __restrict__ twz) {
-    extern __shared__ double2 sm64[];
+    double2* sm64 = smem<double>();
     const int tiles = (g.nxr + tc - 1) / tc;
     const int pos_y = blockIdx.x / tiles, k0 = (blockIdx.x - pos_y * tiles) * tc;
     const int cols = min(tc, g.nxr - k0);
@@ -208,44 +93,6 @@ __global__ void __launch_bounds__(kThreads) k64_z_mul(double2* __restrict__ Y, c
         if (col < cols) base[c * cstride + e * zstride + col] = sm64[((size_t)c * tc + col) * g.Pz + e];
     }
 }
-
-// S8: fp64 sum M.H, two levels in one launch, the last block adds the partial sums in index order
-__global__ void __launch_bounds__(kThreads) k64_energy(const double* __restrict__ M, const double* __restrict__ H, size_t n,
-                                                       double* partial, unsigned* ticket, double factor, double* E) {
-    __shared__ double sh[kThreads];
-    __shared__ bool last;
-    double acc = 0.0;
-    const size_t per = (n + gridDim.x - 1) / gridDim.x, lo = blockIdx.x * per, hi = lo + per < n ? lo + per : n;
-    for (size_t i = lo + threadIdx.x; i < hi; i += blockDim.x) acc += M[i] * H[i];
-    sh[threadIdx.x] = acc;
-    __syncthreads();
-    for (int o = kThreads / 2; o > 0; o >>= 1) {
-        if (threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
-        __syncthreads();
-    }
-    if (threadIdx.x == 0) {
-        partial[blockIdx.x] = sh[0];
-        __threadfence();
-        last = atomicAdd(ticket, 1u) == gridDim.x - 1;
-    }
-    __syncthreads();
-    if (!last) return;
-    __threadfence();
-    double tot = 0.0;
-    for (int i = threadIdx.x; i < (int)gridDim.x; i += blockDim.x) tot += __ldcg(&partial[i]);
-    sh[threadIdx.x] = tot;
-    __syncthreads();
-    for (int o = kThreads / 2; o > 0; o >>= 1) {
-        if (threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
-        __syncthreads();
-    }
-    if (threadIdx.x == 0) { *E = factor * sh[0]; *ticket = 0u; }
-}
-
-int ilog2(int v) { int l = 0; while ((1 << l) < v) ++l; return l; }
-int next_pow2(int n) { int p = 1; while (p < n) p <<= 1; return p; }
-constexpr int kEnergyBlocks64 = 592;
-constexpr size_t kMaxSmem = 200 * 1024;
 
 int upload_tw(double2** dst, int L) {
     const int n = L > 1 ? L / 2 : 1;
@@ -326,18 +173,18 @@ boris_demag_f64_plan* boris_demag_f64_plan_create(int ux, int uy, int uz, double
     };
     alloc((void**)&p->X, nX * sizeof(double2));
     alloc((void**)&p->Y, nY * sizeof(double2));
-    alloc((void**)&p->partial, (kEnergyBlocks64 + 1) * sizeof(double));
-    if (!rc && cudaMemset(p->partial, 0, (kEnergyBlocks64 + 1) * sizeof(double)) != cudaSuccess) rc = bd::set_error(-2, "cudaMemset");
+    alloc((void**)&p->partial, (kEnergyBlocks + 1) * sizeof(double));
+    if (!rc && cudaMemset(p->partial, 0, (kEnergyBlocks + 1) * sizeof(double)) != cudaSuccess) rc = bd::set_error(-2, "cudaMemset");
     auto optin = [&](const void* f, size_t smem) {
         if (rc || smem <= 48 * 1024) return;
         if (smem > kMaxSmem) { rc = bd::set_error(-1, "mesh too large for the fp64 engine's shared-memory tiles"); return; }
         if (cudaError_t e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); e != cudaSuccess)
             rc = bd::micro_fail(e, "cudaFuncSetAttribute");
     };
-    optin((const void*)k64_x_fwd, p->smem_x);
-    optin((const void*)k64_x_inv, p->smem_x);
-    optin((const void*)k64_y<false>, p->smem_y);
-    optin((const void*)k64_y<true>, p->smem_y);
+    optin((const void*)x_fwd<double>, p->smem_x);
+    optin((const void*)x_inv<double>, p->smem_x);
+    optin((const void*)y_pass<double, false>, p->smem_y);
+    optin((const void*)y_pass<double, true>, p->smem_y);
     optin((const void*)k64_z_mul, p->smem_z);
     if (rc) { boris_demag_f64_plan_destroy(p); return nullptr; }
     return p;
@@ -353,11 +200,11 @@ int boris_demag_f64_apply(boris_demag_f64_plan* p, const double* M, double* H, v
     const Geo& g = p->g;
     const int rows = 3 * g.nz * g.ny;
     const int ytiles = (g.nxr + p->tc_y - 1) / p->tc_y, ztiles = (g.nxr + p->tc_z - 1) / p->tc_z;
-    k64_x_fwd<<<rows, kThreads, p->smem_x, st>>>(M, p->X, g, p->twx);
-    k64_y<false><<<3 * g.nz * ytiles, kThreads, p->smem_y, st>>>(p->X, p->Y, g, p->tc_y, p->twy);
+    x_fwd<double><<<rows, kThreads, p->smem_x, st>>>(M, p->X, g, p->twx);
+    y_pass<double, false><<<3 * g.nz * ytiles, kThreads, p->smem_y, st>>>(p->X, p->Y, g, p->tc_y, p->twy);
     k64_z_mul<<<g.Py * ztiles, kThreads, p->smem_z, st>>>(p->Y, p->Kred, g, p->tc_z, p->twz);
-    k64_y<true><<<3 * g.nz * ytiles, kThreads, p->smem_y, st>>>(p->X, p->Y, g, p->tc_y, p->twy);
-    k64_x_inv<<<rows, kThreads, p->smem_x, st>>>(p->X, H, g, p->twx);
+    y_pass<double, true><<<3 * g.nz * ytiles, kThreads, p->smem_y, st>>>(p->X, p->Y, g, p->tc_y, p->twy);
+    x_inv<double><<<rows, kThreads, p->smem_x, st>>>(p->X, H, g, p->twx);
     if (cudaError_t e = cudaGetLastError(); e != cudaSuccess) return bd::micro_fail(e, "fp64 kernel launch");
     return 0;
 }
@@ -366,10 +213,10 @@ int boris_demag_f64_energy(boris_demag_f64_plan* p, const double* M, const doubl
     if (!p || !M || !H || !E_dev) return bd::set_error(-1, "null argument");
     const size_t n = (size_t)3 * p->g.ux * p->g.uy * p->g.uz;
     size_t nblk = (n + 4 * kThreads - 1) / (4 * kThreads);
-    nblk = nblk < 1 ? 1 : (nblk > (size_t)kEnergyBlocks64 ? (size_t)kEnergyBlocks64 : nblk);
+    nblk = nblk < 1 ? 1 : (nblk > (size_t)kEnergyBlocks ? (size_t)kEnergyBlocks : nblk);
     const double factor = -0.5 * (4e-7 * kPi64) * p->hx * p->hy * p->hz;
-    k64_energy<<<(unsigned)nblk, kThreads, 0, (cudaStream_t)stream>>>(M, H, n, p->partial,
-                                                                      reinterpret_cast<unsigned*>(p->partial + kEnergyBlocks64), factor, E_dev);
+    energy<double><<<(unsigned)nblk, kThreads, 0, (cudaStream_t)stream>>>(M, H, n, n, 1, nullptr, p->partial,
+                                                                         reinterpret_cast<unsigned*>(p->partial + kEnergyBlocks), factor, E_dev);
     if (cudaError_t e = cudaGetLastError(); e != cudaSuccess) return bd::micro_fail(e, "k64_energy");
     return 0;
 }

@@ -251,3 +251,15 @@ def test_plane_path_phases_do_not_depend_on_thread_order(emu):
         emu.emu_set_thread_order(0)
     assert np.isfinite(out[0]).all()
     assert np.array_equal(out[0], out[1]) and np.array_equal(out[0], out[2])
+
+
+@pytest.mark.parametrize("nx,ny,hx,hy,tk,ti,Z", [(24, 20, 5.0, 4.0, 4.9, 2.9, 4.5), (64, 8, 2.0, 2.0, 1.0, 1.0, 0.0),
+                                                 (40, 40, 5.0, 5.0, 0.6, 4.9, -30.0), (16, 16, 3.0, 3.0, 2.0, 2.0, 2.0),
+                                                 (200, 4, 2.0, 2.0, 1.0, 3.0, 2.5)])
+def test_library_tensor_between_unequal_cuboids_agrees_with_oracle(nx, ny, hx, hy, tk, ti, Z):
+    """Multi-layered convolution: csrc/ml_math.h (fp64 closed form near, Gauss quadrature of the dipole
+    far) against oracle/multilayer.py (x87 closed form everywhere)."""
+    from oracle.multilayer import pair_tensor_table
+    build.build()
+    lib_T = binding.ml_pair_tensor_host(nx, ny, hx, hy, tk, ti, Z)
+    assert np.abs(lib_T - pair_tensor_table(nx, ny, hx, hy, tk, ti, Z)).max() < 2e-11
