@@ -174,3 +174,12 @@ def test_brute_force_quadrature_of_the_dipolar_kernel(disp):
         brute = V * np.sum(W * num / r5) / (4 * np.pi)
         got = newell.newell_point(c, *R, *h)
         assert abs(got - brute) < 2e-9, (c, got, brute)
+
+
+def test_golden_file_is_what_its_generator_writes():
+    """tests/golden/make_self_terms.py (Aharoni's closed form, 50-digit mpmath, no oracle, no product code)."""
+    import subprocess
+    import sys
+    pytest.importorskip("mpmath")
+    gen = os.path.join(os.path.dirname(GOLDEN), "make_self_terms.py")
+    assert subprocess.run([sys.executable, gen, "--check"], capture_output=True).returncode == 0
