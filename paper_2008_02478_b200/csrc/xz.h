@@ -16,144 +16,17 @@
 
 namespace bd {
 
+// cos(2 pi m / 64): the first quarter turn rounded once from fp64, the rest by symmetry (m is known after unrolling)
 BD_HD constexpr float cos64(int m) {
-    switch (m & 63) {
-        case 0: return 1.000000000e+00f;
-        case 1: return 9.951847267e-01f;
-        case 2: return 9.807852804e-01f;
-        case 3: return 9.569403357e-01f;
-        case 4: return 9.238795325e-01f;
-        case 5: return 8.819212643e-01f;
-        case 6: return 8.314696123e-01f;
-        case 7: return 7.730104534e-01f;
-        case 8: return 7.071067812e-01f;
-        case 9: return 6.343932842e-01f;
-        case 10: return 5.555702330e-01f;
-        case 11: return 4.713967368e-01f;
-        case 12: return 3.826834324e-01f;
-        case 13: return 2.902846773e-01f;
-        case 14: return 1.950903220e-01f;
-        case 15: return 9.801714033e-02f;
-        case 16: return 0.000000000e+00f;
-        case 17: return -9.801714033e-02f;
-        case 18: return -1.950903220e-01f;
-        case 19: return -2.902846773e-01f;
-        case 20: return -3.826834324e-01f;
-        case 21: return -4.713967368e-01f;
-        case 22: return -5.555702330e-01f;
-        case 23: return -6.343932842e-01f;
-        case 24: return -7.071067812e-01f;
-        case 25: return -7.730104534e-01f;
-        case 26: return -8.314696123e-01f;
-        case 27: return -8.819212643e-01f;
-        case 28: return -9.238795325e-01f;
-        case 29: return -9.569403357e-01f;
-        case 30: return -9.807852804e-01f;
-        case 31: return -9.951847267e-01f;
-        case 32: return -1.000000000e+00f;
-        case 33: return -9.951847267e-01f;
-        case 34: return -9.807852804e-01f;
-        case 35: return -9.569403357e-01f;
-        case 36: return -9.238795325e-01f;
-        case 37: return -8.819212643e-01f;
-        case 38: return -8.314696123e-01f;
-        case 39: return -7.730104534e-01f;
-        case 40: return -7.071067812e-01f;
-        case 41: return -6.343932842e-01f;
-        case 42: return -5.555702330e-01f;
-        case 43: return -4.713967368e-01f;
-        case 44: return -3.826834324e-01f;
-        case 45: return -2.902846773e-01f;
-        case 46: return -1.950903220e-01f;
-        case 47: return -9.801714033e-02f;
-        case 48: return 0.000000000e+00f;
-        case 49: return 9.801714033e-02f;
-        case 50: return 1.950903220e-01f;
-        case 51: return 2.902846773e-01f;
-        case 52: return 3.826834324e-01f;
-        case 53: return 4.713967368e-01f;
-        case 54: return 5.555702330e-01f;
-        case 55: return 6.343932842e-01f;
-        case 56: return 7.071067812e-01f;
-        case 57: return 7.730104534e-01f;
-        case 58: return 8.314696123e-01f;
-        case 59: return 8.819212643e-01f;
-        case 60: return 9.238795325e-01f;
-        case 61: return 9.569403357e-01f;
-        case 62: return 9.807852804e-01f;
-        case 63: return 9.951847267e-01f;
-        default: return 0.f;
-    }
+    constexpr float q[17] = {
+        1.000000000e+00f, 9.951847267e-01f, 9.807852804e-01f, 9.569403357e-01f, 9.238795325e-01f, 8.819212643e-01f,
+        8.314696123e-01f, 7.730104534e-01f, 7.071067812e-01f, 6.343932842e-01f, 5.555702330e-01f, 4.713967368e-01f,
+        3.826834324e-01f, 2.902846773e-01f, 1.950903220e-01f, 9.801714033e-02f, 0.000000000e+00f
+    };
+    m &= 63;
+    return m <= 16 ? q[m] : (m <= 32 ? -q[32 - m] : (m <= 48 ? -q[m - 32] : q[64 - m]));
 }
-BD_HD constexpr float sin64(int m) {
-    switch (m & 63) {
-        case 0: return 0.000000000e+00f;
-        case 1: return 9.801714033e-02f;
-        case 2: return 1.950903220e-01f;
-        case 3: return 2.902846773e-01f;
-        case 4: return 3.826834324e-01f;
-        case 5: return 4.713967368e-01f;
-        case 6: return 5.555702330e-01f;
-        case 7: return 6.343932842e-01f;
-        case 8: return 7.071067812e-01f;
-        case 9: return 7.730104534e-01f;
-        case 10: return 8.314696123e-01f;
-        case 11: return 8.819212643e-01f;
-        case 12: return 9.238795325e-01f;
-        case 13: return 9.569403357e-01f;
-        case 14: return 9.807852804e-01f;
-        case 15: return 9.951847267e-01f;
-        case 16: return 1.000000000e+00f;
-        case 17: return 9.951847267e-01f;
-        case 18: return 9.807852804e-01f;
-        case 19: return 9.569403357e-01f;
-        case 20: return 9.238795325e-01f;
-        case 21: return 8.819212643e-01f;
-        case 22: return 8.314696123e-01f;
-        case 23: return 7.730104534e-01f;
-        case 24: return 7.071067812e-01f;
-        case 25: return 6.343932842e-01f;
-        case 26: return 5.555702330e-01f;
-        case 27: return 4.713967368e-01f;
-        case 28: return 3.826834324e-01f;
-        case 29: return 2.902846773e-01f;
-        case 30: return 1.950903220e-01f;
-        case 31: return 9.801714033e-02f;
-        case 32: return 0.000000000e+00f;
-        case 33: return -9.801714033e-02f;
-        case 34: return -1.950903220e-01f;
-        case 35: return -2.902846773e-01f;
-        case 36: return -3.826834324e-01f;
-        case 37: return -4.713967368e-01f;
-        case 38: return -5.555702330e-01f;
-        case 39: return -6.343932842e-01f;
-        case 40: return -7.071067812e-01f;
-        case 41: return -7.730104534e-01f;
-        case 42: return -8.314696123e-01f;
-        case 43: return -8.819212643e-01f;
-        case 44: return -9.238795325e-01f;
-        case 45: return -9.569403357e-01f;
-        case 46: return -9.807852804e-01f;
-        case 47: return -9.951847267e-01f;
-        case 48: return -1.000000000e+00f;
-        case 49: return -9.951847267e-01f;
-        case 50: return -9.807852804e-01f;
-        case 51: return -9.569403357e-01f;
-        case 52: return -9.238795325e-01f;
-        case 53: return -8.819212643e-01f;
-        case 54: return -8.314696123e-01f;
-        case 55: return -7.730104534e-01f;
-        case 56: return -7.071067812e-01f;
-        case 57: return -6.343932842e-01f;
-        case 58: return -5.555702330e-01f;
-        case 59: return -4.713967368e-01f;
-        case 60: return -3.826834324e-01f;
-        case 61: return -2.902846773e-01f;
-        case 62: return -1.950903220e-01f;
-        case 63: return -9.801714033e-02f;
-        default: return 0.f;
-    }
-}
+BD_HD constexpr float sin64(int m) { return cos64(m - 16); }
 
 // z * exp(DIR 2 pi i m / 64), m known after unrolling
 template <int DIR>
