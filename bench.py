@@ -506,6 +506,26 @@ def main():
             del mu
         except Exception as e:
             print(f"[bench] LLG evaluation timing skipped: {e}", file=sys.stderr)
+    # boris_demag_apply_ex(ACCUMULATE): fused into the kernel that writes H on the tiled / plane paths
+    if world == 1:
+        try:
+            def timed(fn, nrep=5):
+                fn()
+                torch.cuda.synchronize()
+                ta, tb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                ta.record(torch.cuda.current_stream())
+                for _ in range(nrep):
+                    fn()
+                tb.record(torch.cuda.current_stream())
+                torch.cuda.synchronize()
+                return ta.elapsed_time(tb) / nrep
+            Hacc = torch.zeros_like(H)
+            t_plain = timed(lambda: plan.apply(M, H))
+            t_acc = timed(lambda: plan.apply_ex(M, Hacc, plan.ACCUMULATE))
+            line["apply_ex"] = {"apply_ms": t_plain, "accumulate_ms": t_acc, "accumulate_over_apply": t_acc / t_plain}
+            del Hacc
+        except Exception as e:
+            print(f"[bench] apply_ex timing skipped: {e}", file=sys.stderr)
     # the double-precision variant (include/boris_demag_f64.h; "single or double"): side information
     if world == 1:
         try:

@@ -72,7 +72,10 @@ int boris_demag_apply(boris_demag_plan* plan, const float* M, float* H, void* st
  *                           library instead of planar components;
  *   BORIS_DEMAG_ACCUMULATE  H += -N * M instead of H = -N * M: the demag term added to an effective field
  *                           that already holds other contributions ("additive field contributions").
- * Both go through plan-owned planar staging buffers and two copy kernels (M in, H out); on a power-of-two
+ * ACCUMULATE alone, on a mesh the tiled or plane kernels take as it is (power-of-two sizes), is
+ * fused: the kernel that writes H reads the old value and adds (12 more bytes per cell, no extra launch, M and H
+ * 16-byte aligned as for boris_demag_apply).  Every other combination (AOS, other meshes) goes
+ * through plan-owned planar staging buffers and two copy kernels (M in, H out); on a power-of-two
  * mesh the buffers are allocated (both or neither) by the FIRST such call (24 bytes per cell), which is the
  * one case in which an apply allocates and synchronises — do not make that first call inside a stream capture.  M, H: DEVICE pointers, 4-byte aligned, must not alias.  Error codes as boris_demag_apply. */
 #define BORIS_DEMAG_AOS 1u

@@ -610,6 +610,17 @@ int boris_demag_apply_ex(boris_demag_plan* p, const float* M, float* H, unsigned
     if (M == H) return fail(-1, "M and H must not alias");
     if (flags & ~(unsigned)(BORIS_DEMAG_AOS | BORIS_DEMAG_ACCUMULATE)) return fail(-1, "unknown flag");
     if (flags == 0) return boris_demag_apply(p, M, H, stream);
+    if (flags == BORIS_DEMAG_ACCUMULATE && !p->padmode && (p->cfg.tiled || p->cfg.plane.on)) {
+        // planar fields on a mesh the tiled / plane kernels take as it is: the kernel that writes H adds to it
+        if (int rc = check_fields(p, M, H, false)) return rc;
+        CudaLauncher run{(cudaStream_t)stream, p->device};
+        bd::PlanView pv = plan_view(p);
+        pv.en.accumulate = 1;
+        const int rc = bd::enqueue_apply(run, pv, M, H);
+        if (rc == -2) return cuda_fail(run.err, "kernel launch");
+        if (rc) return fail(rc, "unsupported size");
+        return 0;
+    }
     if (((uintptr_t)M | (uintptr_t)H) & 3) return fail(-1, "M and H must be 4-byte aligned");
     if (int rc = check_device(p)) return rc;
     if (!p->Mp || !p->Hp) {      // first use of a staged variant on a power-of-two mesh: both buffers or neither

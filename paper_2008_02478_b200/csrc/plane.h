@@ -487,6 +487,17 @@ struct GRowsOutMap {
     BD_HD void pre(const float2*, int) const {}
     BD_HD void stq(float2* q, float2 v, int) const { *q = v; }
 };
+struct GRowsOutMapA {          // H += the field (xt.h GRowsOutA)
+    float* p; long pitch; long hi_pitch; int jbs;
+    static BD_HD constexpr int off(int S, int r) { return r * S; }
+    BD_HD float2* ptr(int row, int e) const {
+        return reinterpret_cast<float2*>(p + (row & ((1 << jbs) - 1)) * pitch + (row >> jbs) * hi_pitch) + e;
+    }
+    mutable float2 hbuf[8];
+    BD_HD void pre(const float2* q, int r) const { hbuf[r] = BD_LDCG(q); }
+    BD_HD void stq(float2* q, float2 v, int r) const { *q = bd_f2(hbuf[r].x + v.x, hbuf[r].y + v.y); }
+    BD_HD void st(float2* q, float2 v) const { *q = v; }
+};
 struct GRowsOutMapE {
     float* p; long pitch; long hi_pitch; int jbs; long m_minus_h; double* acc;
     static BD_HD constexpr int off(int S, int r) { return r * S; }
@@ -565,6 +576,9 @@ struct XInvP {
                 GRowsOutMapE out{h0, LX, (long)a.lsp * LX, JBS, (long)((const char*)a.en.M - (const char*)a.H), &acc};
                 x_rows_pass<LX, 0, true, NT>(tid, RB, s, out, a.ptw);
                 energy_finish(acc, a.en);
+            } else if (a.en.accumulate) {
+                GRowsOutMapA out{h0, LX, (long)a.lsp * LX, JBS};
+                x_rows_pass<LX, 0, true, NT>(tid, RB, s, out, a.ptw);
             } else {
                 GRowsOutMap out{h0, LX, (long)a.lsp * LX, JBS};
                 x_rows_pass<LX, 0, true, NT>(tid, RB, s, out, a.ptw);

@@ -68,6 +68,18 @@ struct GRowsOutE {
     BD_HD void st(float2* q, float2 v) const { *q = v; }
 };
 
+// H += the field instead of H = it (BORIS_DEMAG_ACCUMULATE, the additive effective field of PAPER.md:L36): the old
+// pairs are loaded before the last butterfly is computed
+struct GRowsOutA {
+    float* p; long pitch;
+    static BD_HD constexpr int off(int S, int r) { return r * S; }
+    BD_HD float2* ptr(int row, int e) const { return reinterpret_cast<float2*>(p + row * pitch) + e; }
+    mutable float2 hbuf[8];
+    BD_HD void pre(const float2* q, int r) const { hbuf[r] = BD_LDCG(q); }
+    BD_HD void stq(float2* q, float2 v, int r) const { *q = bd_f2(hbuf[r].x + v.x, hbuf[r].y + v.y); }
+    BD_HD void st(float2* q, float2 v) const { *q = v; }
+};
+
 // Energy fused into the last kernel of an evaluation (boris_demag_apply_energy): every block
 // leaves sum M.H of its rows in partial[block]; the block that finishes last adds them in
 // index order (the ticket decides who adds, not what: E is bit-identical across calls).
@@ -77,6 +89,7 @@ struct EnergyArgs {
     unsigned* ticket;
     double* E;             // device scalar
     double factor;         // -(mu0/2) hx hy hz
+    int accumulate;        // 1: the last kernel adds the field to H instead of overwriting it (no energy then)
 };
 BD_HD void energy_finish(double acc, const EnergyArgs& en) {
 #if defined(__CUDA_ARCH__)
@@ -283,6 +296,9 @@ struct XInvT {
                 GRowsOutE out{a.H + g0 * LX, LX, (long)((const char*)a.en.M - (const char*)a.H), &acc};
                 x_rows_pass<LX, 0, true, NT>(tid, a.rb, s, out, a.ptw);
                 energy_finish(acc, a.en);
+            } else if (a.en.accumulate) {
+                GRowsOutA out{a.H + g0 * LX, LX};
+                x_rows_pass<LX, 0, true, NT>(tid, a.rb, s, out, a.ptw);
             } else {
                 GRowsOut out{a.H + g0 * LX, LX};
                 x_rows_pass<LX, 0, true, NT>(tid, a.rb, s, out, a.ptw);

@@ -401,6 +401,9 @@ struct ZXInv {
                               (long)((const char*)a.en.M - (const char*)a.H), &acc};
                 x_rows_pass<LX, 0, true, NT>(tid, NZ, s, out, a.ptw);
                 energy_finish(acc, a.en);
+            } else if (a.en.accumulate) {
+                GRowsOutA out{a.H + ((long)c * NZ * a.ny + y) * LX, (long)a.ny * LX};
+                x_rows_pass<LX, 0, true, NT>(tid, NZ, s, out, a.ptw);
             } else {
                 GRowsOut out{a.H + ((long)c * NZ * a.ny + y) * LX, (long)a.ny * LX};
                 x_rows_pass<LX, 0, true, NT>(tid, NZ, s, out, a.ptw);

@@ -86,6 +86,9 @@ extern "C" {
 // cs_override > 0 forces the number of kx slots per chunk (to exercise chunking).
 // nq_plane > 0: plane path with that many ky residues; 0: the plan's own choice; < 0: no plane path
 int emu_apply_ex(int nx, int ny, int nz, const double* Kred, const float* M, float* H, int cs_override, int nq_plane);
+// 1: the last kernel of the following emu_apply calls adds the field to H (BORIS_DEMAG_ACCUMULATE, fused)
+static int g_emu_accumulate = 0;
+void emu_set_accumulate(int on) { g_emu_accumulate = on; }
 int emu_apply(int nx, int ny, int nz, const double* Kred, const float* M, float* H, int cs_override) {
     return emu_apply_ex(nx, ny, nz, Kred, M, H, cs_override, cs_override != 0 ? -1 : 0);
 }
@@ -117,6 +120,7 @@ int emu_apply_ex(int nx, int ny, int nz, const double* Kred, const float* M, flo
     std::vector<float4> xpost((size_t)nx / 2 + 1);
     fill_xpost(xpost.data(), nx);
     pv.ptw_x = ptwx.data(); pv.ptw_y = ptwy.data(); pv.V = V.data(); pv.xpost = xpost.data();
+    pv.en.accumulate = g_emu_accumulate;
     std::vector<float2> PX, PP, pltw, plzt;
     std::vector<float> KP;
     std::vector<int> kidx, slotky;

@@ -263,3 +263,22 @@ def test_library_tensor_between_unequal_cuboids_agrees_with_oracle(nx, ny, hx, h
     build.build()
     lib_T = binding.ml_pair_tensor_host(nx, ny, hx, hy, tk, ti, Z)
     assert np.abs(lib_T - pair_tensor_table(nx, ny, hx, hy, tk, ti, Z)).max() < 2e-11
+
+
+@pytest.mark.parametrize("shape,nq", [((1, 16, 64), 0), ((4, 8, 16), 0), ((32, 64, 8), 2)])       # XInvT, ZXInv, XInvP
+def test_emulated_accumulate_adds_the_same_field_to_what_h_holds(emu, shape, nq):
+    """BORIS_DEMAG_ACCUMULATE fused into the kernel that writes H (GRowsOutA / GRowsOutMapA): H0 + the plain result, bit for bit."""
+    nz, ny, nx = shape
+    h = (3.0, 2.0, 1.0)
+    M = W.make_texture("random", shape, 8e5, seed=17)
+    K = binding.spectrum_host(nx, ny, nz, *h)
+    H = np.full(M.shape, np.nan, np.float32)
+    assert emu.emu_apply_ex(nx, ny, nz, vp(K), vp(M), vp(H), 0, nq) == 0
+    H0 = (np.random.default_rng(18).standard_normal(M.shape) * 1e4).astype(np.float32)
+    Hacc = H0.copy()
+    emu.emu_set_accumulate(1)
+    try:
+        assert emu.emu_apply_ex(nx, ny, nz, vp(K), vp(M), vp(Hacc), 0, nq) == 0
+    finally:
+        emu.emu_set_accumulate(0)
+    assert np.array_equal(Hacc, H0 + H)
