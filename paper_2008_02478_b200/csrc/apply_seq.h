@@ -217,6 +217,7 @@ int enqueue_plane_x(Launcher& run, const PlanView& p, const float* M, float* H, 
             case 1: return run.template run<XInvP<LX, 1>>(gi, ia);
             case 2: return run.template run<XInvP<LX, 2>>(gi, ia);
             case 4: return run.template run<XInvP<LX, 4>>(gi, ia);
+            case 8: return run.template run<XInvP<LX, 8>>(gi, ia);
             default: return -1;
         }
     });
@@ -232,6 +233,7 @@ int enqueue_plane_yz(Launcher& run, const PlanView& p) {
             case 1: return run.template run<YZFused<LS, 1>>(gy, ya);
             case 2: return run.template run<YZFused<LS, 2>>(gy, ya);
             case 4: return run.template run<YZFused<LS, 4>>(gy, ya);
+            case 8: return run.template run<YZFused<LS, 8>>(gy, ya);
             default: return -1;
         }
     };

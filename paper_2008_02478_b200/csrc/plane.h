@@ -40,7 +40,7 @@ BD_HD int pl_pos_of_freq(int LS, int k) { return (k % (LS / 16)) * 16 + k / (LS 
 
 struct PlaneGeom {
     int on;        // 1: the mesh takes the plane path
-    int nq;        // residues of ky (1, 2 or 4)
+    int nq;        // residues of ky (1, 2, 4 or 8)
     int ls;        // points of the sub-transform, Py / nq  (64, 128 or 256)
     int lsp;       // stored points of a partial plane: min(ls, ny)
     int zs;        // lanes per ky column, Pz / 16
@@ -49,12 +49,12 @@ struct PlaneGeom {
 // nq_force > 0: take that many residues if the geometry allows it (tests)
 inline PlaneGeom plane_geom(int nx, int ny, int nz, int nq_force = 0) {
     PlaneGeom g{0, 1, 0, 0, 0, 0};
-    if (nz != kPlaneNZ || nx < 4 || ny < 32 || ny > 512) return g;
+    if (nz != kPlaneNZ || nx < 4 || ny < 32 || ny > 1024) return g;
     const int Py = 2 * ny;
     int nq = 1;
     while (Py / nq > 256) nq *= 2;
     if (nq_force > 0) nq = nq_force;
-    if (nq != 1 && nq != 2 && nq != 4) return g;
+    if (nq != 1 && nq != 2 && nq != 4 && nq != 8) return g;
     const int ls = Py / nq;
     if (ls < 64 || ls > 256) return g;
     g.on = 1; g.nq = nq; g.ls = ls; g.lsp = ls < ny ? ls : ny; g.zs = 2 * nz / 16; g.nsl = ls / 2 + 1;
@@ -257,6 +257,31 @@ BD_HD void pl_zlane32(int p, float sy, const float2* col, int pitch, const PlK& 
     }
 }
 
+// cos(2 pi m / 128): quarter-wave table as cos64 (xz.h); the residue twiddles of NQ = 8 are 128th roots
+BD_HD constexpr float cos128(int m) {
+    constexpr float q[33] = {
+        1.000000000e+00f, 9.987954562e-01f, 9.951847267e-01f, 9.891765100e-01f, 9.807852804e-01f, 9.700312532e-01f,
+        9.569403357e-01f, 9.415440652e-01f, 9.238795325e-01f, 9.039892931e-01f, 8.819212643e-01f, 8.577286100e-01f,
+        8.314696123e-01f, 8.032075315e-01f, 7.730104534e-01f, 7.409511254e-01f, 7.071067812e-01f, 6.715589548e-01f,
+        6.343932842e-01f, 5.956993045e-01f, 5.555702330e-01f, 5.141027442e-01f, 4.713967368e-01f, 4.275550934e-01f,
+        3.826834324e-01f, 3.368898534e-01f, 2.902846773e-01f, 2.429801799e-01f, 1.950903220e-01f, 1.467304745e-01f,
+        9.801714033e-02f, 4.906767433e-02f, 0.000000000e+00f
+    };
+    m &= 127;
+    return m <= 32 ? q[m] : (m <= 64 ? -q[64 - m] : (m <= 96 ? -q[m - 64] : q[128 - m]));
+}
+// z * exp(DIR 2 pi i m / 128), m known after unrolling
+template <int DIR>
+BD_HD float2 pk_mul_w128(float2 z, int m) {
+    m &= 127;
+    if ((m & 1) == 0) return pk_mul_w64<DIR>(z, m >> 1);
+    const float c = cos128(m), s = (float)DIR * cos128(m - 32);
+    return pk_fma(pk_swap(z), bd_f2(-s, s), pk_mul(z, pk_bc(c)));
+}
+// z * exp(DIR 2 pi i m / 8)
+template <int DIR>
+BD_HD float2 pk_mul_w8(float2 z, int m) { return pk_mul_w64<DIR>(z, 8 * (m & 7)); }
+
 template <int LS, int NQ>
 struct YZFused {
     using Args = YZArgs;
@@ -274,13 +299,18 @@ struct YZFused {
     static BD_HD long smem_elems(const Args&) { return (long)NPEN * PITCH; }
 
     // blockIdx.x = kx NQ + o; residues q and NQ - q (which read each other's kernel-spectrum slots) are neighbours
-    static BD_HD int q_of_order(int o) { return NQ == 4 ? ((o >> 1) | ((o & 1) << 1)) : o; }     // 0, 2, 1, 3
+    static BD_HD int q_of_order(int o) {
+        if (NQ == 4) return (o >> 1) | ((o & 1) << 1);                       // 0, 2, 1, 3
+        if (NQ == 8) return o == 0 ? 0 : (o == 1 ? 4 : ((o & 1) ? 8 - (o >> 1) : (o >> 1)));   // 0, 4, 1, 7, 2, 6, 3, 5
+        return o;
+    }
 
     // constant input twiddle of the residue: z * W_(NQ R0)^(DIR r Q)
     template <int DIR, int Q>
     static BD_HD float2 in_tw(float2 z, int r) {
         if constexpr (Q == 0) return z;
-        else return pk_mul_w64<DIR>(z, r * Q * (64 / (NQ * R0)));
+        else if constexpr (NQ * R0 <= 64) return pk_mul_w64<DIR>(z, r * Q * (64 / (NQ * R0)));
+        else return pk_mul_w128<DIR>(z, r * Q * (128 / (NQ * R0)));
     }
 
     // phase 0: load, residue stage and first pass (radix R0, stride 16) of every pencil
@@ -291,6 +321,30 @@ struct YZFused {
         Tw tw[R0];
         BD_UNROLL
         for (int q0 = 0; q0 < R0; ++q0) tw[q0] = make_tw(BD_LDG(&a.tw[(Q * R0 + q0) * 16 + j]));
+        if constexpr (NQ == 8) {
+            // four non-zero quarters x[n + LS r'], r' < 4: a_q[n] = sum_r' W_8^(q r') x[n + LS r'], two quarters at a time
+            for (int pc = pg; pc < NPEN; pc += PG) {
+                const float2* xp = a.X + ((long)pc * a.nkx + kx) * a.ny + j;
+                float2 v[R0], b0[R0], b1[R0];
+                BD_UNROLL
+                for (int r = 0; r < R0; ++r) { b0[r] = BD_LDCG(xp + 16 * r); b1[r] = BD_LDCG(xp + 16 * r + LS); }
+                BD_UNROLL
+                for (int r = 0; r < R0; ++r) v[r] = pk_add(b0[r], pk_mul_w8<-1>(b1[r], Q));
+                BD_UNROLL
+                for (int r = 0; r < R0; ++r) { b0[r] = BD_LDCG(xp + 16 * r + 2 * LS); b1[r] = BD_LDCG(xp + 16 * r + 3 * LS); }
+                BD_UNROLL
+                for (int r = 0; r < R0; ++r)
+                    v[r] = in_tw<-1, Q>(pk_add(v[r], pk_add(pk_mul_w8<-1>(b0[r], 2 * Q), pk_mul_w8<-1>(b1[r], 3 * Q))), r);
+                PkDft<R0, -1>::run(v);
+                float2* po = sm + pc * PITCH + j;
+                BD_UNROLL
+                for (int q0 = 0; q0 < R0; ++q0) {
+                    if (Q == 0 && q0 == 0) po[0] = v[0];
+                    else po[17 * q0] = pk_cmul(v[q0], tw[q0]);
+                }
+            }
+            return;
+        }
         constexpr int NLD = NQ == 4 ? 2 * R0 : NIN;
         float2 nxt[NLD];
         auto issue = [&](int pc) {
@@ -448,7 +502,11 @@ struct YZFused {
             }
             if (q == 0) load_pass<0>(tid, kx, a, sm);
             if constexpr (NQ >= 2) { if (q == 1) load_pass<1>(tid, kx, a, sm); }
-            if constexpr (NQ == 4) { if (q == 2) load_pass<2>(tid, kx, a, sm); else if (q == 3) load_pass<3>(tid, kx, a, sm); }
+            if constexpr (NQ >= 4) { if (q == 2) load_pass<2>(tid, kx, a, sm); else if (q == 3) load_pass<3>(tid, kx, a, sm); }
+            if constexpr (NQ == 8) {
+                if (q == 4) load_pass<4>(tid, kx, a, sm); else if (q == 5) load_pass<5>(tid, kx, a, sm);
+                else if (q == 6) load_pass<6>(tid, kx, a, sm); else if (q == 7) load_pass<7>(tid, kx, a, sm);
+            }
         } else if constexpr (PH == 1) {
             pass16<-1>(tid, sm);
         } else if constexpr (PH == 2) {
@@ -458,7 +516,11 @@ struct YZFused {
         } else {
             if (q == 0) pass_store<0>(tid, kx, a, sm);
             if constexpr (NQ >= 2) { if (q == 1) pass_store<1>(tid, kx, a, sm); }
-            if constexpr (NQ == 4) { if (q == 2) pass_store<2>(tid, kx, a, sm); else if (q == 3) pass_store<3>(tid, kx, a, sm); }
+            if constexpr (NQ >= 4) { if (q == 2) pass_store<2>(tid, kx, a, sm); else if (q == 3) pass_store<3>(tid, kx, a, sm); }
+            if constexpr (NQ == 8) {
+                if (q == 4) pass_store<4>(tid, kx, a, sm); else if (q == 5) pass_store<5>(tid, kx, a, sm);
+                else if (q == 6) pass_store<6>(tid, kx, a, sm); else if (q == 7) pass_store<7>(tid, kx, a, sm);
+            }
         }
     }
 };
@@ -534,8 +596,20 @@ struct XInvP {
     static constexpr int NP = dec_np(LX);
     static constexpr int NPHASES = NP + 1;
     static constexpr int RB = 16;                        // rows of H per block
-    static constexpr int JB = NQ == 4 ? 8 : 16, JBS = NQ == 4 ? 3 : 4;   // points of a partial plane per block
+    static constexpr int JB = NQ == 8 ? 4 : (NQ == 4 ? 8 : 16), JBS = NQ == 8 ? 2 : (NQ == 4 ? 3 : 4);   // points of a partial plane per block
     static BD_HD long smem_elems(const Args&) { return (long)RB * SRows<LX>::PITCH; }
+
+    // h[n + LS r] = sum_q W_8^(-q r) P_q[n], r < 4: the first half of an inverse 8-point transform
+    static BD_HD void quarter8(const float2 (&p)[NQ], float2 (&y)[4]) {
+        const float2 e0 = pk_add(p[0], p[4 % NQ]), e1 = pk_sub(p[0], p[4 % NQ]), e2 = pk_add(p[2 % NQ], p[6 % NQ]), e3 = pk_sub(p[2 % NQ], p[6 % NQ]);
+        const float2 o0 = pk_add(p[1 % NQ], p[5 % NQ]), o1 = pk_sub(p[1 % NQ], p[5 % NQ]), o2 = pk_add(p[3 % NQ], p[7 % NQ]), o3 = pk_sub(p[3 % NQ], p[7 % NQ]);
+        const float2 ev[4] = {pk_add(e0, e2), pk_add_ib<+1>(e1, e3), pk_sub(e0, e2), pk_add_ib<-1>(e1, e3)};
+        const float2 od[4] = {pk_add(o0, o2), pk_add_ib<+1>(o1, o3), pk_sub(o0, o2), pk_add_ib<-1>(o1, o3)};
+        y[0] = pk_add(ev[0], od[0]);
+        y[1] = pk_add(ev[1], pk_mul_w8<+1>(od[1], 1));
+        y[2] = pk_add_ib<+1>(ev[2], od[2]);
+        y[3] = pk_add(ev[3], pk_mul_w8<+1>(od[3], 3));
+    }
 
     template <int PH>
     static BD_HD void phase(int tid, int bx, int by, const Args& a, float2* sm) {
@@ -560,6 +634,12 @@ struct XInvP {
                     const float2 Ym1 = pk_add_ib<+1>(pk_sub(am[0], am[2]), pk_sub(am[1], am[3]));
                     xinv_pre(LX, kp, Yk0, Ym0, xp, sm + jj * SRows<LX>::PITCH);
                     xinv_pre(LX, kp, Yk1, Ym1, xp, sm + (JB + jj) * SRows<LX>::PITCH);
+                } else if constexpr (NQ == 8) {
+                    float2 Yk[4], Ym[4];
+                    quarter8(ak, Yk);
+                    quarter8(am, Ym);
+                    BD_UNROLL
+                    for (int r = 0; r < 4; ++r) xinv_pre(LX, kp, Yk[r], Ym[r], xp, sm + (r * JB + jj) * SRows<LX>::PITCH);
                 } else if constexpr (NQ == 2) {
                     xinv_pre(LX, kp, pk_add(ak[0], ak[1]), pk_add(am[0], am[1]), xp, sm + jj * SRows<LX>::PITCH);
                 } else {
@@ -569,7 +649,7 @@ struct XInvP {
         } else if constexpr (PH < NP) {
             x_rows_pass<LX, NP - PH, true, NT>(tid, RB, s, s, a.ptw);
         } else {
-            // row = hi JB + lo  ->  y = j0 + lo + hi lsp   (hi = 1 only for NQ = 4, where lsp = ny / 2)
+            // row = hi JB + lo  ->  y = j0 + lo + hi lsp   (hi > 0 only for NQ = 4 and 8, where lsp = ny / 2 and ny / 4)
             float* h0 = a.H + ((long)cz * a.ny + j0) * LX;
             if (a.en.M) {
                 double acc = 0.0;

@@ -210,7 +210,7 @@ def test_float3_layout_and_accumulate_variants_match_the_oracle(shape):
 
 
 def test_kernel_path_chosen_per_mesh():
-    expect = {(1, 32, 32): 2, (1, 1024, 1024): 2, (128, 128, 128): 3, (32, 512, 512): 4, (32, 256, 16): 4, (16, 512, 512): 3, (32, 16, 1024): 0, (512, 2, 4): 0}
+    expect = {(1, 32, 32): 2, (1, 1024, 1024): 2, (128, 128, 128): 3, (32, 512, 512): 4, (32, 256, 16): 4, (32, 1024, 64): 4, (32, 64, 1024): 4, (16, 512, 512): 3, (32, 16, 1024): 0, (512, 2, 4): 0}
     for (nz, ny, nx), path in expect.items():
         plan = binding.DemagPlan(nx, ny, nz, 2e-9, 2e-9, 1e-9)
         assert plan.layout()["path"] == path
@@ -410,3 +410,54 @@ def test_periodic_tiny_mesh_against_the_copy_by_copy_sum():
     plan.close()
     with pytest.raises(binding.DemagError, match="images"):
         binding.DemagPlan(8, 4, 2, *h, images=(0, -1, 0))
+
+
+# ----------------------------------------------------------------- plane path beyond C5: ny = 1024 (eight ky residues), nx = 1024
+@pytest.mark.parametrize("shape", [(32, 1024, 64), (32, 64, 1024)])
+def test_plane_path_with_1024_cells_along_y_or_x(shape):
+    nz, ny, nx = shape
+    h, Ms = (2e-9, 2e-9, 1e-9), 1.1e6
+    M_host = W.make_texture("helix", shape, Ms, seed=121)
+    plan = binding.DemagPlan(nx, ny, nz, *h)
+    assert plan.layout()["path"] == 4
+    H, E = gpu_apply(plan, M_host, want_energy=True)
+    H_ref = demag_fft(M_host, h)
+    assert_parity(H, H_ref, Ms)
+    assert abs(E - demag_energy(M_host, H_ref, h)) <= TOL_E * abs(E)
+    plan.close()
+
+
+def test_1024x1024x32_film_sampled_against_the_written_out_sum():
+    """The next size up from C5 (33.5 M cells; plane path, eight residues, 1024-point x rows).  The oracle cannot hold its
+    padded spectra, so M is a handful of magnetized cells in an empty mesh and sampled outputs are compared with the
+    written-out sum of PAPER.md:L323 over those cells, N from oracle.newell one displacement at a time."""
+    nz, ny, nx = 32, 1024, 1024
+    h, Ms = (2e-9, 2e-9, 1e-9), 8e5
+    rng = np.random.default_rng(122)
+    src = [(int(rng.integers(nz)), int(rng.integers(ny)), int(rng.integers(nx))) for _ in range(6)] + [(0, 0, 0), (31, 1023, 1023)]
+    vec = rng.standard_normal((len(src), 3))
+    vec *= Ms / np.linalg.norm(vec, axis=1)[:, None]
+    plan = binding.DemagPlan(nx, ny, nz, *h)
+    assert plan.layout()["path"] == 4
+    M = torch.zeros(3, nz, ny, nx, device="cuda")
+    for (k, j, i), v in zip(src, vec):
+        M[:, k, j, i] = torch.tensor(v, dtype=torch.float32)
+    H = torch.full_like(M, float("nan"))
+    plan.apply(M, H)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(H).all())
+    targets = src + [(int(rng.integers(nz)), int(rng.integers(ny)), int(rng.integers(nx))) for _ in range(24)]
+    targets += [(k, min(j + 1, ny - 1), i) for (k, j, i) in src[:4]] + [(min(k + 1, nz - 1), j, i) for (k, j, i) in src[:4]]
+    Mv = np.array([M[:, k, j, i].cpu().numpy().astype(np.float64) for (k, j, i) in src])
+    sym = [[0, 3, 4], [3, 1, 5], [4, 5, 2]]
+    worst = 0.0
+    for (kt, jt, it) in targets:
+        want = np.zeros(3)
+        for (ks, js, is_), m in zip(src, Mv):
+            N = [newell.newell_point(c, (it - is_) * h[0], (jt - js) * h[1], (kt - ks) * h[2], *h) for c in range(6)]
+            for a in range(3):
+                want[a] -= sum(N[sym[a][b]] * m[b] for b in range(3))
+        got = H[:, kt, jt, it].cpu().numpy().astype(np.float64)
+        worst = max(worst, np.abs(got - want).max() / Ms)
+    assert worst <= TOL_MAX, worst
+    plan.close()

@@ -218,6 +218,8 @@ PLANE_CASES = [
     ((32, 128, 16), (2.0, 3.0, 1.0), "random", 0),        # LS = 256, one residue
     ((32, 256, 4), (2.0, 2.0, 1.0), "random", 0),         # LS = 256, two residues
     ((32, 512, 4), (2.0, 2.0, 1.0), "helix", 0),          # LS = 256, four residues: C5's y and z
+    ((32, 256, 4), (2.0, 3.0, 1.0), "random", 8),         # LS = 64, eight residues
+    ((32, 1024, 4), (2.0, 2.0, 1.0), "random", 0),        # LS = 256, eight residues (128th roots): ny = 1024
 ]
 
 
