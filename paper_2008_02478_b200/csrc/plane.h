@@ -203,7 +203,16 @@ BD_HD void pl_load_k(const float4* __restrict__ kA, const float4* __restrict__ k
     BD_UNROLL
     for (int h = 0; h < 2; ++h) {
         BD_UNROLL
-        for (int c = 0; c < 6; ++c) k.d[h][c] = BD_LDG(kA + c * kcs + h * khs);
+        for (int c = 0; c < 6; ++c) {
+#if defined(__CUDA_ARCH__) && defined(BD_YZ_VOLATILE_K)
+            // issued where it stands: the list is on its way while the forward transform runs
+            const float4* q = kA + c * kcs + h * khs;
+            asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];"
+                         : "=f"(k.d[h][c].x), "=f"(k.d[h][c].y), "=f"(k.d[h][c].z), "=f"(k.d[h][c].w) : "l"(q));
+#else
+            k.d[h][c] = BD_LDG(kA + c * kcs + h * khs);
+#endif
+        }
     }
     k.kB = kB;
 }
