@@ -626,15 +626,9 @@ struct XInvP {
         const int cz = bx / bpc, j0 = (bx - cz * bpc) * JB;
         SRows<LX> s{sm};
         if constexpr (PH == 0) {
-            constexpr int items = (LX / 2 + 1) * JB;
-            for (int w = tid; w < items; w += NT) {
-                const int kp = w >> JBS, jj = w & (JB - 1), km = LX - kp;
-                const float4 xp = BD_LDG(&a.xpost[kp]);
-                const float2* pk = a.P + ((long)cz * a.nkx + kp) * a.lsp + j0 + jj;
-                const float2* pm = a.P + ((long)cz * a.nkx + km) * a.lsp + j0 + jj;
-                float2 ak[NQ], am[NQ];
-                BD_UNROLL
-                for (int q = 0; q < NQ; ++q) { ak[q] = BD_LDCG(pk + q * a.qstride); am[q] = BD_LDCG(pm + q * a.qstride); }
+            // two neighbouring points of the partial planes per item: 16-byte loads, NQ x 2 of them in flight per thread
+            constexpr int items = (LX / 2 + 1) * (JB / 2);
+            auto emit = [&](int kp, int jj, const float4& xp, const float2 (&ak)[NQ], const float2 (&am)[NQ]) {
                 if constexpr (NQ == 4) {
                     // h[n] = P0 + P1 + P2 + P3,  h[n + LS] = P0 + i P1 - P2 - i P3
                     const float2 Yk0 = pk_add(pk_add(ak[0], ak[2]), pk_add(ak[1], ak[3]));
@@ -654,6 +648,22 @@ struct XInvP {
                 } else {
                     xinv_pre(LX, kp, ak[0], am[0], xp, sm + jj * SRows<LX>::PITCH);
                 }
+            };
+            for (int w = tid; w < items; w += NT) {
+                const int kp = w >> (JBS - 1), jj = 2 * (w & (JB / 2 - 1)), km = LX - kp;
+                const float4 xp = BD_LDG(&a.xpost[kp]);
+                const float4* pk = reinterpret_cast<const float4*>(a.P + ((long)cz * a.nkx + kp) * a.lsp + j0 + jj);
+                const float4* pm = reinterpret_cast<const float4*>(a.P + ((long)cz * a.nkx + km) * a.lsp + j0 + jj);
+                float4 bk[NQ], bm[NQ];
+                BD_UNROLL
+                for (int q = 0; q < NQ; ++q) { bk[q] = BD_LDCG(pk + q * (a.qstride / 2)); bm[q] = BD_LDCG(pm + q * (a.qstride / 2)); }
+                float2 ak[NQ], am[NQ];
+                BD_UNROLL
+                for (int q = 0; q < NQ; ++q) { ak[q] = bd_f2(bk[q].x, bk[q].y); am[q] = bd_f2(bm[q].x, bm[q].y); }
+                emit(kp, jj, xp, ak, am);
+                BD_UNROLL
+                for (int q = 0; q < NQ; ++q) { ak[q] = bd_f2(bk[q].z, bk[q].w); am[q] = bd_f2(bm[q].z, bm[q].w); }
+                emit(kp, jj + 1, xp, ak, am);
             }
         } else if constexpr (PH < NP) {
             x_rows_pass<LX, NP - PH, true, NT>(tid, RB, s, s, a.ptw);
