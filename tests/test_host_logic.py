@@ -284,3 +284,32 @@ def test_emulated_accumulate_adds_the_same_field_to_what_h_holds(emu, shape, nq)
     finally:
         emu.emu_set_accumulate(0)
     assert np.array_equal(Hacc, H0 + H)
+
+
+@pytest.fixture(scope="session")
+def asan_emu():
+    """tests/emu/asan_main.cpp: the emulation as an AddressSanitizer executable with exactly sized buffers."""
+    import subprocess
+    here = os.path.join(os.path.dirname(__file__), "emu")
+    exe = os.path.join(here, "asan_emu")
+    cuda_inc = os.path.join(os.environ.get("CUDA_HOME", "/usr/local/cuda"), "include")
+    csrc = os.path.join(os.path.dirname(os.path.dirname(__file__)), "paper_2008_02478_b200", "csrc")
+    deps = [os.path.join(here, f) for f in ("asan_main.cpp", "emulate.cpp")] + [os.path.join(csrc, f) for f in os.listdir(csrc) if f.endswith(".h")]
+    if os.path.exists(exe) and all(os.path.getmtime(d) <= os.path.getmtime(exe) for d in deps):
+        return exe
+    # -O0: the instrumented template code compiles in half a minute (3.5 minutes at -O1) and still runs in seconds
+    res = subprocess.run(["g++", "-std=c++17", "-O0", "-g", "-fsanitize=address", "-fno-omit-frame-pointer", "-I", cuda_inc,
+                          "-I", here, "-o", exe, os.path.join(here, "asan_main.cpp")], capture_output=True, text=True)
+    if res.returncode != 0:
+        pytest.skip("no AddressSanitizer toolchain: " + res.stderr[-300:])
+    return exe
+
+
+# small-ny and small-nz shapes (more row groups than rows), every kernel path: tiled 2-D, tiled 3-D, plane (1, 2, 4, 8
+# residues), chunked fallback
+@pytest.mark.parametrize("args", [(8, 512, 4), (128, 256, 2), (64, 8, 1), (4, 2, 1), (16, 4, 8), (8, 4, 64), (4, 32, 32),
+                                  (8, 64, 32, 0, 2), (4, 128, 32, 0, 4), (4, 256, 32, 0, 8), (8, 16, 8, -1), (16, 8, 4, 3)])
+def test_emulation_under_address_sanitizer(asan_emu, args):
+    import subprocess
+    res = subprocess.run([asan_emu] + [str(a) for a in args], capture_output=True, text=True, timeout=900)
+    assert res.returncode == 0, res.stdout[-500:] + res.stderr[-3000:]
