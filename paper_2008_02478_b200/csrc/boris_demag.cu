@@ -132,9 +132,13 @@ __device__ __forceinline__ double block_sum(double v, double* sh) {
     return v;
 }
 
+// sum of four products: each product m h is split exactly into its rounded fp32 value p and the residual
+// e = fma(m, h, -p); the p are added in fp64, the residuals (2^-24 of the products) in fp32 and then to the fp64 sum:
+// the result differs from the all-fp64 sum by 2^-48 of the terms, at one conversion per product instead of two
 __device__ __forceinline__ double dot4(const float4& m, const float4& h) {
-    // every product of two floats is exact in fp64; the sum is fp64
-    return (double)m.x * h.x + (double)m.y * h.y + (double)m.z * h.z + (double)m.w * h.w;
+    const float p0 = m.x * h.x, p1 = m.y * h.y, p2 = m.z * h.z, p3 = m.w * h.w;
+    const float e = (fmaf(m.x, h.x, -p0) + fmaf(m.y, h.y, -p1)) + (fmaf(m.z, h.z, -p2) + fmaf(m.w, h.w, -p3));
+    return (((double)p0 + (double)p1) + ((double)p2 + (double)p3)) + (double)e;
 }
 
 __global__ void __launch_bounds__(kEnergyThreads) k_energy_partial(const float4* __restrict__ M, const float4* __restrict__ H,
