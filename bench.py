@@ -552,6 +552,31 @@ def main():
             print(f"[bench] fp64 variant timing skipped: {e}", file=sys.stderr)
     del plan, M, H, E
     torch.cuda.empty_cache()
+    # the next size up from the headline mesh (same plane path, eight ky residues): time per cell against C5's
+    if world == 1 and not args.no_all_configs and cfg.name == "C5":
+        try:
+            big = W.Config("C5x4", 1024, 1024, 32, cfg.hx, cfg.hy, cfg.hz, cfg.Ms, 2005, "random")
+            pb = binding.DemagPlan(big.nx, big.ny, big.nz, *big.h)
+            Mb = torch.randn(3, big.nz, big.ny, big.nx, device="cuda") * (cfg.Ms / 3 ** 0.5)
+            Hb = torch.empty_like(Mb)
+            for _ in range(3):
+                pb.apply(Mb, Hb)
+            torch.cuda.synchronize()
+            ba, bb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ba.record(torch.cuda.current_stream())
+            for _ in range(5):
+                pb.apply(Mb, Hb)
+            bb.record(torch.cuda.current_stream())
+            torch.cuda.synchronize()
+            msb = ba.elapsed_time(bb) / 5
+            line["next_size"] = {"mesh": [big.nx, big.ny, big.nz], "path": pb.layout()["path"], "ms_per_apply": msb,
+                                 "ns_per_cell": msb * 1e6 / big.cells,
+                                 "per_cell_over_headline": (msb / big.cells) / (ms_step / cfg.cells)}
+            pb.close()
+            del Mb, Hb
+            torch.cuda.empty_cache()
+        except Exception as e:
+            print(f"[bench] next-size timing skipped: {e}", file=sys.stderr)
     if world == 1 and not args.no_all_configs:
         allc = {cfg.name: {k: v for k, v in res.items() if k != "kernels"}}
         for name in sorted(W.CONFIGS):
