@@ -34,10 +34,17 @@ struct MinBlocks<K, std::void_t<decltype(K::MINB)>> { static constexpr int value
 // grid has completed and its writes are visible.  Every kernel of the library waits before it touches memory,
 // so completion orders chain: nothing runs ahead of data it reads or overwrites.  Outside such a launch both
 // instructions are no-ops.
+template <class K, class = void>
+struct HasPrologue : std::false_type {};
+template <class K>
+struct HasPrologue<K, std::void_t<decltype(&K::prologue)>> : std::true_type {};
+
 template <class K>
 __global__ void __launch_bounds__(K::NT, MinBlocks<K>::value) phase_kernel(const __grid_constant__ typename K::Args a) {
     extern __shared__ __align__(16) float2 bd_smem[];
     asm volatile("griddepcontrol.launch_dependents;");
+    // what a block may do before its predecessor grid has finished: hints for data no kernel of the evaluation writes
+    if constexpr (HasPrologue<K>::value) K::prologue(threadIdx.x, blockIdx.x, a);
     asm volatile("griddepcontrol.wait;" ::: "memory");
     run_phases<K, 0>(a, bd_smem);
 }

@@ -498,17 +498,19 @@ struct YZFused {
         }
     }
 
+    // before the predecessor kernel has finished (launcher.cuh): the kernel-spectrum slots of this residue start towards
+    // L2 (the blocks of one kx run side by side: between them they fetch all of its slots)
+    static BD_HD void prologue(int tid, int bx, const Args& a) {
+        const int kx = bx / NQ, q = q_of_order(bx % NQ);
+        constexpr long KB = 6L * (ZS + 1) * 2 * NSL * 4 * (long)sizeof(float);
+        const char* kq = reinterpret_cast<const char*>(a.KP) + ((long)kx * NQ + q) * KB;
+        for (long o = (long)tid * 128; o < KB; o += NT * 128) bd_prefetch_l2(kq + o);
+    }
+
     template <int PH>
     static BD_HD void phase(int tid, int bx, int by, const Args& a, float2* sm) {
         const int kx = bx / NQ, q = q_of_order(bx % NQ);
         if constexpr (PH == 0) {
-            {
-                // the kernel-spectrum slots of this residue start towards L2 while the pencils are loaded (the
-                // blocks of one kx run side by side: between them they fetch all of its slots)
-                constexpr long KB = 6L * (ZS + 1) * 2 * NSL * 4 * (long)sizeof(float);
-                const char* kq = reinterpret_cast<const char*>(a.KP) + ((long)kx * NQ + q) * KB;
-                for (long o = (long)tid * 128; o < KB; o += NT * 128) bd_prefetch_l2(kq + o);
-            }
             if (q == 0) load_pass<0>(tid, kx, a, sm);
             if constexpr (NQ >= 2) { if (q == 1) load_pass<1>(tid, kx, a, sm); }
             if constexpr (NQ >= 4) { if (q == 2) load_pass<2>(tid, kx, a, sm); else if (q == 3) load_pass<3>(tid, kx, a, sm); }

@@ -335,15 +335,19 @@ struct YFused {
         return GTile<COLS>{a.V + ((long)b.kz * a.ntl + b.tile) * NY * COLS + col, cstride};
     }
 
+    // before the predecessor kernel has finished (launcher.cuh): the block's kernel-spectrum tile starts on its way to L2
+    static BD_HD void prologue(int tid, int bx, const Args& a) {
+        const Blk b = decode(bx, a);
+        constexpr long KB = (long)NR * COLS * NC * RL * sizeof(float);
+        const char* kt = reinterpret_cast<const char*>(a.K) + ((long)b.kzr * a.ntl + b.tile) * KB;
+        for (long o = (long)tid * 128; o < KB; o += NT * 128) bd_prefetch_l2(kt + o);
+    }
+
     template <int P, bool INV>
     static BD_HD void pass(int tid, int bx, const Args& a, float2* sm) {
         constexpr int ITEMS = (L / dec_r(L, P)) * COLS;
         const Blk b = decode(bx, a);
         if constexpr (P == 0 && !INV) {
-            // start the block's kernel-spectrum tile on its way to L2 while the pencils are transformed
-            constexpr long KB = (long)NR * COLS * NC * RL * sizeof(float);
-            const char* kt = reinterpret_cast<const char*>(a.K) + ((long)b.kzr * a.ntl + b.tile) * KB;
-            for (long o = (long)tid * 128; o < KB; o += NT * 128) bd_prefetch_l2(kt + o);
             // ... and the input tile of the block that will follow this one on the SM
             const int nb = bx + a.pf;
             if (a.pf > 0 && nb < a.ntl * a.pz) {
