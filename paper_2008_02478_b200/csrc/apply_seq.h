@@ -222,18 +222,19 @@ int enqueue_plane_x(Launcher& run, const PlanView& p, const float* M, float* H, 
         }
     });
 }
-template <class Launcher>
-int enqueue_plane_yz(Launcher& run, const PlanView& p) {
+// the fused y/z kernel of slabs of NZ cells (separate templates: one translation unit per thickness)
+template <int NZ, class Launcher>
+int enqueue_plane_yz_nz(Launcher& run, const PlanView& p) {
     const PlaneGeom& g = p.cfg.plane;
     YZArgs ya{p.X, p.P, p.KP, p.kidx, p.pl_tw, p.pl_zt, p.nx + 1, p.ny};
     const Grid gy{(unsigned)((p.nx + 1) * g.nq), 1};
     auto go = [&](auto lsc) {
         constexpr int LS = decltype(lsc)::value;
         switch (g.nq) {
-            case 1: return run.template run<YZFused<LS, 1>>(gy, ya);
-            case 2: return run.template run<YZFused<LS, 2>>(gy, ya);
-            case 4: return run.template run<YZFused<LS, 4>>(gy, ya);
-            case 8: return run.template run<YZFused<LS, 8>>(gy, ya);
+            case 1: return run.template run<YZFused<LS, 1, NZ>>(gy, ya);
+            case 2: return run.template run<YZFused<LS, 2, NZ>>(gy, ya);
+            case 4: return run.template run<YZFused<LS, 4, NZ>>(gy, ya);
+            case 8: return run.template run<YZFused<LS, 8, NZ>>(gy, ya);
             default: return -1;
         }
     };
@@ -241,6 +242,15 @@ int enqueue_plane_yz(Launcher& run, const PlanView& p) {
         case 64: return go(IC<64>{});
         case 128: return go(IC<128>{});
         case 256: return go(IC<256>{});
+        default: return -1;
+    }
+}
+template <class Launcher>
+int enqueue_plane_yz(Launcher& run, const PlanView& p) {
+    switch (p.nz) {
+        case 32: return enqueue_plane_yz_nz<32>(run, p);
+        case 16: return enqueue_plane_yz_nz<16>(run, p);
+        case 8: return enqueue_plane_yz_nz<8>(run, p);
         default: return -1;
     }
 }

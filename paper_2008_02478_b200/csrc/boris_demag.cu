@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -469,6 +470,7 @@ boris_demag_plan* boris_demag_plan_create_pbc(int ux, int uy, int uz, double hx,
     p->padmode = nx != ux || ny != uy || nz != uz;
     const int Py = 2 * ny, Pz = nz > 1 ? 2 * nz : 1;
     p->cfg = bd::make_launch_cfg(nx, ny, nz);
+    if (const char* e = getenv("BORIS_DEMAG_NO_PLANE")) { if (e[0] == '1') p->cfg.plane.on = 0; }     // A/B measurements
     {
         int sms = 148;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);

@@ -29,7 +29,7 @@ namespace bd {
 #define BD_YZ_NT 384
 #endif
 constexpr int kKindYZFused = 1;          // timing slot of the fused kernel (as YFused)
-constexpr int kPlaneNZ = 32;             // slab thickness the plane path is built for
+constexpr int kPlaneNZ = 32;             // thickest slab of the plane path; 16 and 8 take it with 2 and 1 lanes per column
 
 BD_HD constexpr int pl_pe(int e) { return e + (e >> 4); }            // shared pencil padding: 1 per 16
 // odd: the four lanes of a ky column store rows 4 apart (zstage), which then fall into different banks
@@ -49,7 +49,7 @@ struct PlaneGeom {
 // nq_force > 0: take that many residues if the geometry allows it (tests)
 inline PlaneGeom plane_geom(int nx, int ny, int nz, int nq_force = 0) {
     PlaneGeom g{0, 1, 0, 0, 0, 0};
-    if (nz != kPlaneNZ || nx < 4 || ny < 32 || ny > 1024) return g;
+    if ((nz != 32 && nz != 16 && nz != 8) || nx < 4 || ny < 32 || ny > 1024) return g;
     const int Py = 2 * ny;
     int nq = 1;
     while (Py / nq > 256) nq *= 2;
@@ -192,10 +192,11 @@ BD_HD void pl_mul3(float kxx, float kyy, float kzz, float kxy, float kxz, float 
 
 BD_HD float pl_f4(const float4& v, int i) { return i == 0 ? v.x : (i == 1 ? v.y : (i == 2 ? v.z : v.w)); }
 
-// One lane of a ky column: frequencies kz = 4 m + p, m < 16, of the 64-point z transform of the
-// 32 cells; returns its part y[c][j] of the inverse transform,
-//     out[j] = sum_p y_p[j],   out[j + 16] = sum_p i^p y_p[j]          (j < 16).
-// col: the column in shared memory (element z of component c at col[(c 32 + z) pitch]);
+// One lane of a ky column: frequencies kz = ZS m + p, m < 16, of the 2 NZ-point z transform of the NZ cells
+// (ZS = NZ / 8 lanes per column: 4, 2 or 1); returns its part y[c][j] of the inverse transform: for NZ = 32
+//     out[j] = sum_p y_p[j],   out[j + 16] = sum_p i^p y_p[j]          (j < 16),
+// for NZ = 16 out[j] = y_0[j] + y_1[j], for NZ = 8 out[j] = y[j], j < 8.
+// col: the column in shared memory (element z of component c at col[(c NZ + z) pitch]);
 // k: the lane's direct and mirror lists (pl_load_k: kA / kB point at h = 0 of component 0, kcs / khs are the float4
 // strides between components and halves); sy = -1 for a column at ky > Py/2.
 struct PlK { float4 d[2][6]; const float4* kB; };     // a lane's direct list [h][c]; its mirror list is read when needed
@@ -216,22 +217,42 @@ BD_HD void pl_load_k(const float4* __restrict__ kA, const float4* __restrict__ k
     }
     k.kB = kB;
 }
-BD_HD void pl_zlane32(int p, float sy, const float2* col, int pitch, const PlK& k, long kcs, long khs,
-                      const float2* __restrict__ zt, float2 (&v)[3][16]) {
-    // (-i)^p as the pair (c, (-s, s)) of a twiddle
-    Tw rot;
-    rot.c = p == 0 ? 1.f : (p == 2 ? -1.f : 0.f);
-    { const float s = p == 1 ? -1.f : (p == 3 ? 1.f : 0.f); rot.ns = bd_f2(-s, s); }
-    BD_UNROLL
-    for (int c = 0; c < 3; ++c) {
+template <int NZ>
+BD_HD void pl_zlane(int p, float sy, const float2* col, int pitch, const PlK& k, long kcs, long khs,
+                    const float2* __restrict__ zt, float2 (&v)[3][16]) {
+    // first stage of the 2 NZ-point transform of the NZ cells, split by the residue p of kz modulo ZS = NZ / 8 and pruned to
+    // its non-zero inputs:  a_p[j] = W_Pz^(j p) sum_{r < ZS/2} x[j + 16 r] W_ZS^(r p)
+    if constexpr (NZ == 32) {
+        // (-i)^p as the pair (c, (-s, s)) of a twiddle
+        Tw rot;
+        rot.c = p == 0 ? 1.f : (p == 2 ? -1.f : 0.f);
+        { const float s = p == 1 ? -1.f : (p == 3 ? 1.f : 0.f); rot.ns = bd_f2(-s, s); }
         BD_UNROLL
-        for (int j = 0; j < 16; ++j) {
-            const Tw t = make_tw(BD_LDG(&zt[p * 16 + j]));
-            const float2 x0 = col[(c * 32 + j) * pitch], x1 = col[(c * 32 + j + 16) * pitch];
-            const float2 a = pk_fma(pk_swap(x1), rot.ns, pk_fma(x1, pk_bc(rot.c), x0));
-            v[c][j] = pk_cmul(a, t);
+        for (int c = 0; c < 3; ++c) {
+            BD_UNROLL
+            for (int j = 0; j < 16; ++j) {
+                const Tw t = make_tw(BD_LDG(&zt[p * 16 + j]));
+                const float2 x0 = col[(c * 32 + j) * pitch], x1 = col[(c * 32 + j + 16) * pitch];
+                const float2 a = pk_fma(pk_swap(x1), rot.ns, pk_fma(x1, pk_bc(rot.c), x0));
+                v[c][j] = pk_cmul(a, t);
+            }
+            PkDft<16, -1>::run(v[c]);
         }
-        PkDft<16, -1>::run(v[c]);
+    } else if constexpr (NZ == 16) {
+        BD_UNROLL
+        for (int c = 0; c < 3; ++c) {
+            BD_UNROLL
+            for (int j = 0; j < 16; ++j) v[c][j] = pk_cmul(col[(c * 16 + j) * pitch], make_tw(BD_LDG(&zt[p * 16 + j])));
+            PkDft<16, -1>::run(v[c]);
+        }
+    } else {
+        // one lane, 16 frequencies, 8 cells: the zero padding prunes the transform itself
+        BD_UNROLL
+        for (int c = 0; c < 3; ++c) {
+            BD_UNROLL
+            for (int j = 0; j < 8; ++j) v[c][j] = col[(c * 8 + j) * pitch];
+            PkDftPruned<16, -1>::run(v[c]);
+        }
     }
     // direct frequencies m = 0..7, then the mirrored ones m = 15 - i
     BD_UNROLL
@@ -256,13 +277,18 @@ BD_HD void pl_zlane32(int p, float sy, const float2* col, int pitch, const PlK& 
                     -sy * pl_f4(km[5], i), v[0][m], v[1][m], v[2][m]);
         }
     }
-    BD_UNROLL
-    for (int c = 0; c < 3; ++c) PkDft<16, +1>::run(v[c]);
-    BD_UNROLL
-    for (int j = 0; j < 16; ++j) {
-        const Tw t = make_tw(BD_LDG(&zt[p * 16 + j]));
+    if constexpr (NZ == 8) {
         BD_UNROLL
-        for (int c = 0; c < 3; ++c) v[c][j] = pk_cmulc(v[c][j], t);
+        for (int c = 0; c < 3; ++c) PkDftTrunc<16, +1>::run(v[c]);       // the 8 cells: v[c][0..8)
+    } else {
+        BD_UNROLL
+        for (int c = 0; c < 3; ++c) PkDft<16, +1>::run(v[c]);
+        BD_UNROLL
+        for (int j = 0; j < 16; ++j) {
+            const Tw t = make_tw(BD_LDG(&zt[p * 16 + j]));
+            BD_UNROLL
+            for (int c = 0; c < 3; ++c) v[c][j] = pk_cmulc(v[c][j], t);
+        }
     }
 }
 
@@ -291,13 +317,13 @@ BD_HD float2 pk_mul_w128(float2 z, int m) {
 template <int DIR>
 BD_HD float2 pk_mul_w8(float2 z, int m) { return pk_mul_w64<DIR>(z, 8 * (m & 7)); }
 
-template <int LS, int NQ>
+template <int LS, int NQ, int NZ_ = kPlaneNZ>
 struct YZFused {
     using Args = YZArgs;
     static constexpr int KIND = kKindYZFused;
-    static constexpr int NZ = kPlaneNZ, NPEN = 3 * NZ, ZS = 2 * NZ / 16;
-    static constexpr int NT = BD_YZ_NT;
-    static constexpr int MINB = 1;
+    static constexpr int NZ = NZ_, NPEN = 3 * NZ, ZS = 2 * NZ / 16;
+    static constexpr int NT = BD_YZ_NT * NZ / kPlaneNZ;       // thinner slabs: smaller blocks, 32 / NZ of them per SM
+    static constexpr int MINB = kPlaneNZ / NZ;
     static constexpr int NPHASES = 5;
     static constexpr int R0 = LS / 16;                   // first-pass radix; the second pass is radix 16
     static constexpr int PITCH = pl_pitch(LS);
@@ -444,38 +470,60 @@ struct YZFused {
             PlK kc;
             const float sy = lists(w, kc);
             float2 y[3][16];
-            pl_zlane32(p, sy, col, PITCH, kc, KCS, KHS, a.zt, y);
-            // out[j] = sum_p y_p[j], out[j + 16] = sum_p i^p y_p[j]: two exchange rounds among the 4 lanes
-            const bool hi = (p & 2) != 0, lo = (p & 1) != 0;
-            const float sg = hi ? -1.f : 1.f;
-            float2 S[3][8], D[3][8];
-            BD_UNROLL
-            for (int c = 0; c < 3; ++c) {
+            pl_zlane<NZ>(p, sy, col, PITCH, kc, KCS, KHS, a.zt, y);
+            if constexpr (ZS == 4) {
+                // out[j] = sum_p y_p[j], out[j + 16] = sum_p i^p y_p[j]: two exchange rounds among the 4 lanes
+                const bool hi = (p & 2) != 0, lo = (p & 1) != 0;
+                const float sg = hi ? -1.f : 1.f;
+                float2 S[3][8], D[3][8];
                 BD_UNROLL
-                for (int i = 0; i < 8; ++i) {
-                    const float2 send = hi ? y[c][i] : y[c][8 + i], mine = hi ? y[c][8 + i] : y[c][i];
-                    float2 oth;
-                    oth.x = __shfl_xor_sync(0xffffffffu, send.x, 2);
-                    oth.y = __shfl_xor_sync(0xffffffffu, send.y, 2);
-                    S[c][i] = pk_add(mine, oth);
-                    D[c][i] = pk_mul(pk_sub(mine, oth), pk_bc(sg));
+                for (int c = 0; c < 3; ++c) {
+                    BD_UNROLL
+                    for (int i = 0; i < 8; ++i) {
+                        const float2 send = hi ? y[c][i] : y[c][8 + i], mine = hi ? y[c][8 + i] : y[c][i];
+                        float2 oth;
+                        oth.x = __shfl_xor_sync(0xffffffffu, send.x, 2);
+                        oth.y = __shfl_xor_sync(0xffffffffu, send.y, 2);
+                        S[c][i] = pk_add(mine, oth);
+                        D[c][i] = pk_mul(pk_sub(mine, oth), pk_bc(sg));
+                    }
                 }
-            }
-            const int jb = (hi ? 8 : 0) + (lo ? 4 : 0);
-            BD_UNROLL
-            for (int c = 0; c < 3; ++c) {
+                const int jb = (hi ? 8 : 0) + (lo ? 4 : 0);
                 BD_UNROLL
-                for (int i = 0; i < 4; ++i) {
-                    const float2 sS = lo ? S[c][i] : S[c][4 + i], sD = lo ? D[c][i] : D[c][4 + i];
-                    const float2 kS = lo ? S[c][4 + i] : S[c][i], kD = lo ? D[c][4 + i] : D[c][i];
-                    float2 rS, rD;
-                    rS.x = __shfl_xor_sync(0xffffffffu, sS.x, 1);
-                    rS.y = __shfl_xor_sync(0xffffffffu, sS.y, 1);
-                    rD.x = __shfl_xor_sync(0xffffffffu, sD.x, 1);
-                    rD.y = __shfl_xor_sync(0xffffffffu, sD.y, 1);
-                    const float2 ev = lo ? rD : kD, od = lo ? kD : rD;
-                    col[(c * 32 + jb + i) * PITCH] = pk_add(kS, rS);
-                    col[(c * 32 + 16 + jb + i) * PITCH] = pk_add_ib<+1>(ev, od);
+                for (int c = 0; c < 3; ++c) {
+                    BD_UNROLL
+                    for (int i = 0; i < 4; ++i) {
+                        const float2 sS = lo ? S[c][i] : S[c][4 + i], sD = lo ? D[c][i] : D[c][4 + i];
+                        const float2 kS = lo ? S[c][4 + i] : S[c][i], kD = lo ? D[c][4 + i] : D[c][i];
+                        float2 rS, rD;
+                        rS.x = __shfl_xor_sync(0xffffffffu, sS.x, 1);
+                        rS.y = __shfl_xor_sync(0xffffffffu, sS.y, 1);
+                        rD.x = __shfl_xor_sync(0xffffffffu, sD.x, 1);
+                        rD.y = __shfl_xor_sync(0xffffffffu, sD.y, 1);
+                        const float2 ev = lo ? rD : kD, od = lo ? kD : rD;
+                        col[(c * NZ + jb + i) * PITCH] = pk_add(kS, rS);
+                        col[(c * NZ + 16 + jb + i) * PITCH] = pk_add_ib<+1>(ev, od);
+                    }
+                }
+            } else if constexpr (ZS == 2) {
+                // out[j] = y_0[j] + y_1[j]: each lane keeps eight cells and sends the other eight
+                const bool lo = (p & 1) != 0;
+                BD_UNROLL
+                for (int c = 0; c < 3; ++c) {
+                    BD_UNROLL
+                    for (int i = 0; i < 8; ++i) {
+                        const float2 send = lo ? y[c][i] : y[c][8 + i], mine = lo ? y[c][8 + i] : y[c][i];
+                        float2 oth;
+                        oth.x = __shfl_xor_sync(0xffffffffu, send.x, 1);
+                        oth.y = __shfl_xor_sync(0xffffffffu, send.y, 1);
+                        col[(c * NZ + (lo ? 8 : 0) + i) * PITCH] = pk_add(mine, oth);
+                    }
+                }
+            } else {
+                BD_UNROLL
+                for (int c = 0; c < 3; ++c) {
+                    BD_UNROLL
+                    for (int j = 0; j < 8; ++j) col[(c * NZ + j) * PITCH] = y[c][j];
                 }
             }
 #else
@@ -485,14 +533,20 @@ struct YZFused {
             for (int pp = 0; pp < ZS; ++pp) {
                 PlK k;
                 const float sy = lists(w + pp, k);
-                pl_zlane32(pp, sy, col, PITCH, k, KCS, KHS, a.zt, y[pp]);
+                pl_zlane<NZ>(pp, sy, col, PITCH, k, KCS, KHS, a.zt, y[pp]);
             }
             for (int c = 0; c < 3; ++c)
                 for (int j = 0; j < 16; ++j) {
-                    const float2 Se = pk_add(y[0][c][j], y[2][c][j]), So = pk_add(y[1][c][j], y[3][c][j]);
-                    const float2 De = pk_sub(y[0][c][j], y[2][c][j]), Do = pk_sub(y[1][c][j], y[3][c][j]);
-                    col[(c * 32 + j) * PITCH] = pk_add(Se, So);
-                    col[(c * 32 + 16 + j) * PITCH] = pk_add_ib<+1>(De, Do);
+                    if constexpr (ZS == 4) {
+                        const float2 Se = pk_add(y[0][c][j], y[2][c][j]), So = pk_add(y[1][c][j], y[3][c][j]);
+                        const float2 De = pk_sub(y[0][c][j], y[2][c][j]), Do = pk_sub(y[1][c][j], y[3][c][j]);
+                        col[(c * NZ + j) * PITCH] = pk_add(Se, So);
+                        col[(c * NZ + 16 + j) * PITCH] = pk_add_ib<+1>(De, Do);
+                    } else if constexpr (ZS == 2) {
+                        col[(c * NZ + j) * PITCH] = pk_add(y[0][c][j], y[1][c][j]);
+                    } else {
+                        if (j < 8) col[(c * NZ + j) * PITCH] = y[0][c][j];
+                    }
                 }
 #endif
         }

@@ -210,7 +210,7 @@ def test_float3_layout_and_accumulate_variants_match_the_oracle(shape):
 
 
 def test_kernel_path_chosen_per_mesh():
-    expect = {(1, 32, 32): 2, (1, 1024, 1024): 2, (128, 128, 128): 3, (32, 512, 512): 4, (32, 256, 16): 4, (32, 1024, 64): 4, (32, 64, 1024): 4, (16, 512, 512): 3, (32, 16, 1024): 0, (512, 2, 4): 0}
+    expect = {(1, 32, 32): 2, (1, 1024, 1024): 2, (128, 128, 128): 3, (32, 512, 512): 4, (32, 256, 16): 4, (32, 1024, 64): 4, (32, 64, 1024): 4, (16, 512, 512): 4, (8, 64, 64): 4, (16, 16, 64): 3, (4, 64, 64): 3, (32, 16, 1024): 0, (512, 2, 4): 0}
     for (nz, ny, nx), path in expect.items():
         plan = binding.DemagPlan(nx, ny, nz, 2e-9, 2e-9, 1e-9)
         assert plan.layout()["path"] == path
@@ -460,4 +460,40 @@ def test_1024x1024x32_film_sampled_against_the_written_out_sum():
         got = H[:, kt, jt, it].cpu().numpy().astype(np.float64)
         worst = max(worst, np.abs(got - want).max() / Ms)
     assert worst <= TOL_MAX, worst
+    plan.close()
+
+
+# ----------------------------------------------------------------- plane path on 16- and 8-cell slabs (the paper's pipelined regime, L283)
+@pytest.mark.parametrize("shape,texture", [((16, 64, 128), "helix"), ((8, 256, 64), "random"), ((16, 1024, 16), "random"),
+                                           ((8, 32, 32), "vortex"), ((8, 40, 100), "random"), ((16, 512, 512), "helix")])
+def test_plane_path_on_thin_slabs(shape, texture):
+    nz, ny, nx = shape
+    h, Ms = (2e-9, 3e-9, 1e-9), 8e5
+    M_host = W.make_texture(texture, shape, Ms, seed=131)
+    plan = binding.DemagPlan(nx, ny, nz, *h)
+    assert plan.layout()["path"] == 4
+    H, E = gpu_apply(plan, M_host, want_energy=True)
+    H_ref = demag_fft(M_host, h)
+    assert_parity(H, H_ref, Ms)
+    assert abs(E - demag_energy(M_host, H_ref, h)) <= TOL_E * abs(E)
+    M = torch.from_numpy(M_host).cuda()
+    H0 = torch.from_numpy(H).cuda()
+    if (nx & (nx - 1)) == 0 and (ny & (ny - 1)) == 0:           # fused accumulate on the plane path
+        Hacc = H0.clone()
+        plan.apply_ex(M, Hacc, plan.ACCUMULATE)
+        assert torch.equal(Hacc, H0 + H0)
+    plan.close()
+
+
+@pytest.mark.parametrize("shape", [(16, 64, 128), (8, 256, 64), (32, 64, 32)])
+def test_tiled_3d_kernels_stay_reachable_on_slabs_the_plane_path_takes(shape, monkeypatch):
+    """BORIS_DEMAG_NO_PLANE=1 at plan creation selects XZFwd / YFused / ZXInv (the A/B switch of profiles/r02_plane.md)."""
+    nz, ny, nx = shape
+    h, Ms = (2e-9, 3e-9, 1e-9), 8e5
+    M_host = W.make_texture("random", shape, Ms, seed=132)
+    monkeypatch.setenv("BORIS_DEMAG_NO_PLANE", "1")
+    plan = binding.DemagPlan(nx, ny, nz, *h)
+    monkeypatch.delenv("BORIS_DEMAG_NO_PLANE")
+    assert plan.layout()["path"] == 3
+    assert_parity(gpu_apply(plan, M_host), demag_fft(M_host, h), Ms)
     plan.close()

@@ -220,6 +220,12 @@ PLANE_CASES = [
     ((32, 512, 4), (2.0, 2.0, 1.0), "helix", 0),          # LS = 256, four residues: C5's y and z
     ((32, 256, 4), (2.0, 3.0, 1.0), "random", 8),         # LS = 64, eight residues
     ((32, 1024, 4), (2.0, 2.0, 1.0), "random", 0),        # LS = 256, eight residues (128th roots): ny = 1024
+    ((16, 32, 8), (3.0, 2.0, 1.0), "random", 0),          # 16 cells: two lanes per column; LS = 64, one residue
+    ((16, 128, 4), (2.0, 2.0, 1.0), "helix", 0),          # 16 cells, LS = 256
+    ((16, 256, 4), (2.0, 2.0, 2.0), "random", 0),         # 16 cells, two residues
+    ((8, 64, 8), (2.0, 3.0, 1.0), "random", 0),           # 8 cells: one lane, the transform itself pruned; LS = 128
+    ((8, 512, 4), (2.0, 2.0, 1.0), "random", 0),          # 8 cells, four residues
+    ((8, 128, 4), (4.0, 4.0, 1.0), "random", 4),          # 8 cells, LS = 64, four residues
 ]
 
 
@@ -308,8 +314,23 @@ def asan_emu():
 # small-ny and small-nz shapes (more row groups than rows), every kernel path: tiled 2-D, tiled 3-D, plane (1, 2, 4, 8
 # residues), chunked fallback
 @pytest.mark.parametrize("args", [(8, 512, 4), (128, 256, 2), (64, 8, 1), (4, 2, 1), (16, 4, 8), (8, 4, 64), (4, 32, 32),
-                                  (8, 64, 32, 0, 2), (4, 128, 32, 0, 4), (4, 256, 32, 0, 8), (8, 16, 8, -1), (16, 8, 4, 3)])
+                                  (8, 64, 32, 0, 2), (4, 128, 32, 0, 4), (4, 256, 32, 0, 8), (8, 16, 8, -1), (16, 8, 4, 3),
+                                  (8, 32, 16), (4, 64, 8), (8, 128, 16, 0, 2), (4, 32, 8, 0, -1)])
 def test_emulation_under_address_sanitizer(asan_emu, args):
     import subprocess
     res = subprocess.run([asan_emu] + [str(a) for a in args], capture_output=True, text=True, timeout=900)
     assert res.returncode == 0, res.stdout[-500:] + res.stderr[-3000:]
+
+
+@pytest.mark.parametrize("shape", [(16, 32, 32), (8, 32, 16), (32, 32, 8)])
+def test_emulated_tiled_3d_kernels_on_slabs_the_plane_path_would_take(emu, shape):
+    """XZFwd / YFused / ZXInv stay reachable (BORIS-internal choice: the plane path takes these slabs by default)."""
+    nz, ny, nx = shape
+    h, Ms = (2.0, 2.0, 1.0), 8e5
+    M = W.make_texture("random", shape, Ms, seed=19)
+    K = binding.spectrum_host(nx, ny, nz, *h)
+    H = np.full(M.shape, np.nan, np.float32)
+    assert emu.emu_apply_ex(nx, ny, nz, vp(K), vp(M), vp(H), 0, -1) == 0
+    H_ref = demag_fft(M, h)
+    err = np.abs(H - H_ref)
+    assert err.max() <= 1e-5 * Ms and np.sqrt((err ** 2).sum() / (H_ref ** 2).sum()) <= 2e-6
