@@ -29,7 +29,7 @@ namespace bd {
 #define BD_YZ_NT 384
 #endif
 constexpr int kKindYZFused = 1;          // timing slot of the fused kernel (as YFused)
-constexpr int kPlaneNZ = 32;             // thickest slab of the plane path; 16 and 8 take it with 2 and 1 lanes per column
+constexpr int kPlaneNZ = 32;             // the slab the plane path was built for (4 lanes per ky column); 64, 16 and 8 cells: 8, 2, 1 lanes
 
 BD_HD constexpr int pl_pe(int e) { return e + (e >> 4); }            // shared pencil padding: 1 per 16
 // odd: the four lanes of a ky column store rows 4 apart (zstage), which then fall into different banks
@@ -49,14 +49,15 @@ struct PlaneGeom {
 // nq_force > 0: take that many residues if the geometry allows it (tests)
 inline PlaneGeom plane_geom(int nx, int ny, int nz, int nq_force = 0) {
     PlaneGeom g{0, 1, 0, 0, 0, 0};
-    if ((nz != 32 && nz != 16 && nz != 8) || nx < 4 || ny < 32 || ny > 1024) return g;
+    if ((nz != 64 && nz != 32 && nz != 16 && nz != 8) || nx < 4 || ny < 32 || ny > 1024) return g;
     const int Py = 2 * ny;
+    const int lsmax = nz > 32 ? 128 : 256;           // 3 nz pencils of LS points in 227 KB
     int nq = 1;
-    while (Py / nq > 256) nq *= 2;
+    while (Py / nq > lsmax) nq *= 2;
     if (nq_force > 0) nq = nq_force;
     if (nq != 1 && nq != 2 && nq != 4 && nq != 8) return g;
     const int ls = Py / nq;
-    if (ls < 64 || ls > 256) return g;
+    if (ls < 64 || ls > lsmax) return g;
     g.on = 1; g.nq = nq; g.ls = ls; g.lsp = ls < ny ? ls : ny; g.zs = 2 * nz / 16; g.nsl = ls / 2 + 1;
     return g;
 }
@@ -217,12 +218,47 @@ BD_HD void pl_load_k(const float4* __restrict__ kA, const float4* __restrict__ k
     }
     k.kB = kB;
 }
+// exp(-2 pi i m / 8), m at run time (a lane's constant)
+BD_HD float2 pl_w8(int m) {
+    constexpr float C = 0.70710678118654752440f;
+    switch (m & 7) {
+        case 0: return bd_f2(1.f, 0.f);
+        case 1: return bd_f2(C, -C);
+        case 2: return bd_f2(0.f, -1.f);
+        case 3: return bd_f2(-C, -C);
+        case 4: return bd_f2(-1.f, 0.f);
+        case 5: return bd_f2(-C, C);
+        case 6: return bd_f2(0.f, 1.f);
+        default: return bd_f2(C, C);
+    }
+}
+
 template <int NZ>
 BD_HD void pl_zlane(int p, float sy, const float2* col, int pitch, const PlK& k, long kcs, long khs,
                     const float2* __restrict__ zt, float2 (&v)[3][16]) {
     // first stage of the 2 NZ-point transform of the NZ cells, split by the residue p of kz modulo ZS = NZ / 8 and pruned to
     // its non-zero inputs:  a_p[j] = W_Pz^(j p) sum_{r < ZS/2} x[j + 16 r] W_ZS^(r p)
-    if constexpr (NZ == 32) {
+    if constexpr (NZ == 64) {
+        // eight lanes: x[j] + W_8^p x[j + 16] + (-i)^p x[j + 32] + W_8^(3p) x[j + 48]
+        const int p4 = p & 3;
+        Tw rot;
+        rot.c = p4 == 0 ? 1.f : (p4 == 2 ? -1.f : 0.f);
+        { const float s = p4 == 1 ? -1.f : (p4 == 3 ? 1.f : 0.f); rot.ns = bd_f2(-s, s); }
+        const Tw w1 = make_tw(pl_w8(p)), w3 = make_tw(pl_w8(3 * p));
+        BD_UNROLL
+        for (int c = 0; c < 3; ++c) {
+            BD_UNROLL
+            for (int j = 0; j < 16; ++j) {
+                const Tw t = make_tw(BD_LDG(&zt[p * 16 + j]));
+                const float2 x0 = col[(c * 64 + j) * pitch], x1 = col[(c * 64 + j + 16) * pitch];
+                const float2 x2 = col[(c * 64 + j + 32) * pitch], x3 = col[(c * 64 + j + 48) * pitch];
+                float2 a = pk_fma(pk_swap(x2), rot.ns, pk_fma(x2, pk_bc(rot.c), x0));
+                a = pk_add(a, pk_add(pk_cmul(x1, w1), pk_cmul(x3, w3)));
+                v[c][j] = pk_cmul(a, t);
+            }
+            PkDft<16, -1>::run(v[c]);
+        }
+    } else if constexpr (NZ == 32) {
         // (-i)^p as the pair (c, (-s, s)) of a twiddle
         Tw rot;
         rot.c = p == 0 ? 1.f : (p == 2 ? -1.f : 0.f);
@@ -292,6 +328,45 @@ BD_HD void pl_zlane(int p, float sy, const float2* col, int pitch, const PlK& k,
     }
 }
 
+#if defined(__CUDA_ARCH__)
+// Four lanes q = 2 hi + lo (xor distances 2 and 1) each hold C_q[c][0..NJ); afterwards the lane holds, for the NJ / 4
+// values j = jb + i (jb = hi NJ/2 + lo NJ/4),  o0[c][i] = sum_q C_q[c][j]  and  o1[c][i] = sum_q i^q C_q[c][j]
+// (the two exchange rounds of the 4-lane z stage, for any NJ).
+template <int NJ>
+__device__ __forceinline__ void pl_exchange4(const float2 (&C)[3][NJ], bool hi, bool lo, float2 (&o0)[3][NJ / 4], float2 (&o1)[3][NJ / 4]) {
+    const float sg = hi ? -1.f : 1.f;
+    float2 S[3][NJ / 2], D[3][NJ / 2];
+    BD_UNROLL
+    for (int c = 0; c < 3; ++c) {
+        BD_UNROLL
+        for (int i = 0; i < NJ / 2; ++i) {
+            const float2 send = hi ? C[c][i] : C[c][NJ / 2 + i], mine = hi ? C[c][NJ / 2 + i] : C[c][i];
+            float2 oth;
+            oth.x = __shfl_xor_sync(0xffffffffu, send.x, 2);
+            oth.y = __shfl_xor_sync(0xffffffffu, send.y, 2);
+            S[c][i] = pk_add(mine, oth);
+            D[c][i] = pk_mul(pk_sub(mine, oth), pk_bc(sg));
+        }
+    }
+    BD_UNROLL
+    for (int c = 0; c < 3; ++c) {
+        BD_UNROLL
+        for (int i = 0; i < NJ / 4; ++i) {
+            const float2 sS = lo ? S[c][i] : S[c][NJ / 4 + i], sD = lo ? D[c][i] : D[c][NJ / 4 + i];
+            const float2 kS = lo ? S[c][NJ / 4 + i] : S[c][i], kD = lo ? D[c][NJ / 4 + i] : D[c][i];
+            float2 rS, rD;
+            rS.x = __shfl_xor_sync(0xffffffffu, sS.x, 1);
+            rS.y = __shfl_xor_sync(0xffffffffu, sS.y, 1);
+            rD.x = __shfl_xor_sync(0xffffffffu, sD.x, 1);
+            rD.y = __shfl_xor_sync(0xffffffffu, sD.y, 1);
+            const float2 ev = lo ? rD : kD, od = lo ? kD : rD;
+            o0[c][i] = pk_add(kS, rS);
+            o1[c][i] = pk_add_ib<+1>(ev, od);
+        }
+    }
+}
+#endif
+
 // cos(2 pi m / 128): quarter-wave table as cos64 (xz.h); the residue twiddles of NQ = 8 are 128th roots
 BD_HD constexpr float cos128(int m) {
     constexpr float q[33] = {
@@ -322,8 +397,8 @@ struct YZFused {
     using Args = YZArgs;
     static constexpr int KIND = kKindYZFused;
     static constexpr int NZ = NZ_, NPEN = 3 * NZ, ZS = 2 * NZ / 16;
-    static constexpr int NT = BD_YZ_NT * NZ / kPlaneNZ;       // thinner slabs: smaller blocks, 32 / NZ of them per SM
-    static constexpr int MINB = kPlaneNZ / NZ;
+    static constexpr int NT = NZ >= kPlaneNZ ? BD_YZ_NT : BD_YZ_NT * NZ / kPlaneNZ;   // thinner slabs: smaller blocks, 32 / NZ of them per SM
+    static constexpr int MINB = NZ >= kPlaneNZ ? 1 : kPlaneNZ / NZ;
     static constexpr int NPHASES = 5;
     static constexpr int R0 = LS / 16;                   // first-pass radix; the second pass is radix 16
     static constexpr int PITCH = pl_pitch(LS);
@@ -505,6 +580,39 @@ struct YZFused {
                         col[(c * NZ + 16 + jb + i) * PITCH] = pk_add_ib<+1>(ev, od);
                     }
                 }
+            } else if constexpr (ZS == 8) {
+                // out[j + 16 r] = sum_p W_8^(-r p) y_p[j], r < 4.  Lanes p and p + 4 first: A = y_q + y_(q+4) feeds r = 0, 2,
+                // B = y_q - y_(q+4) feeds r = 1, 3; then the four lanes q of a half combine A and W_8^(-q) B as the 4-lane stage does
+                const bool top = (p & 4) != 0, hi = (p & 2) != 0, lo = (p & 1) != 0;
+                const float st = top ? -1.f : 1.f;
+                const Tw wq = make_tw(pl_w8(p & 3));            // W_8^(-q) = conj(W_8^q)
+                float2 A[3][8], B[3][8];
+                BD_UNROLL
+                for (int c = 0; c < 3; ++c) {
+                    BD_UNROLL
+                    for (int i = 0; i < 8; ++i) {
+                        const float2 send = top ? y[c][i] : y[c][8 + i], mine = top ? y[c][8 + i] : y[c][i];
+                        float2 oth;
+                        oth.x = __shfl_xor_sync(0xffffffffu, send.x, 4);
+                        oth.y = __shfl_xor_sync(0xffffffffu, send.y, 4);
+                        A[c][i] = pk_add(mine, oth);
+                        B[c][i] = pk_cmulc(pk_mul(pk_sub(mine, oth), pk_bc(st)), wq);
+                    }
+                }
+                float2 r0[3][2], r2[3][2], r1[3][2], r3[3][2];
+                pl_exchange4<8>(A, hi, lo, r0, r2);
+                pl_exchange4<8>(B, hi, lo, r1, r3);
+                const int jb = (top ? 8 : 0) + (hi ? 4 : 0) + (lo ? 2 : 0);
+                BD_UNROLL
+                for (int c = 0; c < 3; ++c) {
+                    BD_UNROLL
+                    for (int i = 0; i < 2; ++i) {
+                        col[(c * NZ + jb + i) * PITCH] = r0[c][i];
+                        col[(c * NZ + 16 + jb + i) * PITCH] = r1[c][i];
+                        col[(c * NZ + 32 + jb + i) * PITCH] = r2[c][i];
+                        col[(c * NZ + 48 + jb + i) * PITCH] = r3[c][i];
+                    }
+                }
             } else if constexpr (ZS == 2) {
                 // out[j] = y_0[j] + y_1[j]: each lane keeps eight cells and sends the other eight
                 const bool lo = (p & 1) != 0;
@@ -529,7 +637,7 @@ struct YZFused {
 #else
             // host emulation (tests/emu): lane 0 of a column runs the four lanes in turn, same arithmetic
             if (p != 0) continue;
-            float2 y[4][3][16];
+            float2 y[ZS][3][16];
             for (int pp = 0; pp < ZS; ++pp) {
                 PlK k;
                 const float sy = lists(w + pp, k);
@@ -537,7 +645,13 @@ struct YZFused {
             }
             for (int c = 0; c < 3; ++c)
                 for (int j = 0; j < 16; ++j) {
-                    if constexpr (ZS == 4) {
+                    if constexpr (ZS == 8) {
+                        for (int r = 0; r < 4; ++r) {
+                            float2 acc = bd_f2(0.f, 0.f);
+                            for (int pp = 0; pp < 8; ++pp) acc = pk_add(acc, pk_cmulc(y[pp][c][j], make_tw(pl_w8(r * pp))));
+                            col[(c * NZ + 16 * r + j) * PITCH] = acc;
+                        }
+                    } else if constexpr (ZS == 4) {
                         const float2 Se = pk_add(y[0][c][j], y[2][c][j]), So = pk_add(y[1][c][j], y[3][c][j]);
                         const float2 De = pk_sub(y[0][c][j], y[2][c][j]), Do = pk_sub(y[1][c][j], y[3][c][j]);
                         col[(c * NZ + j) * PITCH] = pk_add(Se, So);
