@@ -1,5 +1,5 @@
-// plane.h — the plane path of thin slabs (nz = 32, the paper's pipelined regime
-// of few cells along z): the x spectrum stays y- and z-UNPADDED in HBM and the whole padded
+// plane.h — the plane path of slabs (nz = 8, 16, 32 and, on wide meshes, 64, the paper's
+// pipelined regime of few cells along z): the x spectrum stays y- and z-UNPADDED in HBM and the whole padded
 // (y, z) plane of one kx is transformed, multiplied by the kernel spectrum and transformed back
 // on chip (S2..S6 of SURVEY.md §8(a) in one launch, all 3 components).
 //
@@ -8,17 +8,17 @@
 //   XInvP         S7 (+S8)    P -> H, summing the NQ partial planes            (this file)
 //
 // The padded plane of one kx (3 x nz x Py complex) does not fit one SM, so the y transform is
-// split by the residue q of ky modulo NQ (decimation in frequency, first stage done on load):
-//     X^[q + NQ k] = sum_{n < LS} W_LS^(n k) a_q[n],   LS = Py / NQ,
+// split by the residue q of ky modulo NQ = 1, 2, 4 or 8 (decimation in frequency, first stage done on load):
+//     X^[q + NQ k] = sum_{n < LS} W_LS^(n k) a_q[n],   LS = Py / NQ <= 256 (128 at nz = 64),
 //     a_q[n] = W_Py^(n q) sum_r x[n + LS r] W_NQ^(q r)            (x = 0 beyond ny: r < NQ/2)
 // Block (kx, q) holds its 3 x nz pencils of LS points in shared memory (3 x 32 x 256 complex =
-// 204 KB with padding), runs the z transform, the multiply and the inverse z transform in
-// registers per ky column (4 lanes per column, 16 frequencies kz = 4 m + p each), transforms
-// back along y and writes its PARTIAL result
+// 204 KB with padding at nz = 32; slabs of 16 / 8 cells take half / a quarter of that and of the threads, 2 / 4 blocks per
+// SM), runs the z transform, the multiply and the inverse z transform in registers per ky column — ZS = nz / 8 lanes per
+// column, lane p taking the 16 frequencies kz = ZS m + p — transforms back along y and writes its PARTIAL result
 //     P_q[n] = W_Py^(-n q) sum_k H^[q + NQ k] W_LS^(-n k),        n < LS,
 // of which the inverse x kernel forms  h[n + LS r] = sum_q W_NQ^(-q r) P_q[n]  (r < NQ/2 kept).
 // HBM per evaluation at 512x512x32: 0.10 + 0.20 | 0.20 + 0.25 + 0.40 | 0.40 + 0.10 GB = 1.66 GB
-// (the tiled path: 2.04 GB), all of it in pieces of at least 64 contiguous bytes.
+// (the tiled path: 2.04 GB), all of it in pieces of at least 64 contiguous bytes (32 at NQ = 8).
 #pragma once
 #include "xt.h"
 #include "xz.h"
@@ -206,14 +206,7 @@ BD_HD void pl_load_k(const float4* __restrict__ kA, const float4* __restrict__ k
     for (int h = 0; h < 2; ++h) {
         BD_UNROLL
         for (int c = 0; c < 6; ++c) {
-#if defined(__CUDA_ARCH__) && defined(BD_YZ_VOLATILE_K)
-            // issued where it stands: the list is on its way while the forward transform runs
-            const float4* q = kA + c * kcs + h * khs;
-            asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];"
-                         : "=f"(k.d[h][c].x), "=f"(k.d[h][c].y), "=f"(k.d[h][c].z), "=f"(k.d[h][c].w) : "l"(q));
-#else
             k.d[h][c] = BD_LDG(kA + c * kcs + h * khs);
-#endif
         }
     }
     k.kB = kB;
