@@ -255,6 +255,8 @@ int enqueue_plane_yz(Launcher& run, const PlanView& p) {
         case 32: return enqueue_plane_yz_nz<32>(run, p);
         case 16: return enqueue_plane_yz_nz<16>(run, p);
         case 8: return enqueue_plane_yz_nz<8>(run, p);
+        case 4: return enqueue_plane_yz_nz<4>(run, p);
+        case 2: return enqueue_plane_yz_nz<2>(run, p);
         default: return -1;
     }
 }

@@ -1,4 +1,4 @@
-// plane.h — the plane path of slabs (nz = 8, 16, 32 and, on wide meshes, 64, the paper's
+// plane.h — the plane path of slabs (nz = 2, 4, 8, 16, 32 and, on wide meshes, 64, the paper's
 // pipelined regime of few cells along z): the x spectrum stays y- and z-UNPADDED in HBM and the whole padded
 // (y, z) plane of one kx is transformed, multiplied by the kernel spectrum and transformed back
 // on chip (S2..S6 of SURVEY.md §8(a) in one launch, all 3 components).
@@ -14,7 +14,7 @@
 // Block (kx, q) holds its 3 x nz pencils of LS points in shared memory (3 x 32 x 256 complex =
 // 204 KB with padding at nz = 32; slabs of 16 / 8 cells take half / a quarter of that and of the threads, 2 / 4 blocks per
 // SM), runs the z transform, the multiply and the inverse z transform in registers per ky column — ZS = nz / 8 lanes per
-// column, lane p taking the 16 frequencies kz = ZS m + p — transforms back along y and writes its PARTIAL result
+// column, lane p taking the 16 frequencies kz = ZS m + p (one lane with all 2 nz frequencies below 8 cells) — transforms back along y and writes its PARTIAL result
 //     P_q[n] = W_Py^(-n q) sum_k H^[q + NQ k] W_LS^(-n k),        n < LS,
 // of which the inverse x kernel forms  h[n + LS r] = sum_q W_NQ^(-q r) P_q[n]  (r < NQ/2 kept).
 // HBM per evaluation at 512x512x32: 0.10 + 0.20 | 0.20 + 0.25 + 0.40 | 0.40 + 0.10 GB = 1.66 GB
@@ -43,13 +43,13 @@ struct PlaneGeom {
     int nq;        // residues of ky (1, 2, 4 or 8)
     int ls;        // points of the sub-transform, Py / nq  (64, 128 or 256)
     int lsp;       // stored points of a partial plane: min(ls, ny)
-    int zs;        // lanes per ky column, Pz / 16
+    int zs;        // lanes per ky column, Pz / 16 (1 for slabs of fewer than 8 cells)
     int nsl;       // kernel-spectrum slots per residue, ls / 2 + 1
 };
 // nq_force > 0: take that many residues if the geometry allows it (tests)
 inline PlaneGeom plane_geom(int nx, int ny, int nz, int nq_force = 0) {
     PlaneGeom g{0, 1, 0, 0, 0, 0};
-    if ((nz != 64 && nz != 32 && nz != 16 && nz != 8) || nx < 4 || ny < 32 || ny > 1024) return g;
+    if ((nz != 64 && nz != 32 && nz != 16 && nz != 8 && nz != 4 && nz != 2) || nx < 4 || ny < 32 || ny > 1024) return g;
     const int Py = 2 * ny;
     const int lsmax = nz > 32 ? 128 : 256;           // 3 nz pencils of LS points in 227 KB
     int nq = 1;
@@ -58,7 +58,7 @@ inline PlaneGeom plane_geom(int nx, int ny, int nz, int nq_force = 0) {
     if (nq != 1 && nq != 2 && nq != 4 && nq != 8) return g;
     const int ls = Py / nq;
     if (ls < 64 || ls > lsmax) return g;
-    g.on = 1; g.nq = nq; g.ls = ls; g.lsp = ls < ny ? ls : ny; g.zs = 2 * nz / 16; g.nsl = ls / 2 + 1;
+    g.on = 1; g.nq = nq; g.ls = ls; g.lsp = ls < ny ? ls : ny; g.zs = nz >= 8 ? 2 * nz / 16 : 1; g.nsl = ls / 2 + 1;
     return g;
 }
 
@@ -73,10 +73,14 @@ inline PlaneGeom plane_geom(int nx, int ny, int nz, int nq_force = 0) {
 // kidx[q LS + e] = slot | qs << 12 | (ky > Py/2) << 15
 struct PlaneK {
     int nx, ny, nz, nq, ls, zs, nsl;
-    BD_HD long per_kx() const { return (long)nq * 6 * (zs + 1) * 2 * nsl * 4; }
+    // a lane's lists hold hb = min(8, nz) frequencies each (8: a lane has 16 frequencies; slabs of 4 / 2 cells have 8 / 4
+    // frequencies in all), stored as nh = 2 or 1 groups of four
+    BD_HD int hb() const { return nz >= 8 ? 8 : nz; }
+    BD_HD int nh() const { return nz >= 8 ? 2 : 1; }
+    BD_HD long per_kx() const { return (long)nq * 6 * (zs + 1) * nh() * nsl * 4; }
     BD_HD long storage_elems() const { return (long)(nx + 1) * per_kx(); }
     BD_HD long index(int kx, int qs, int c, int pr, int h, int slot, int i) const {
-        return ((((((long)kx * nq + qs) * 6 + c) * (zs + 1) + pr) * 2 + h) * nsl + slot) * 4 + i;
+        return ((((((long)kx * nq + qs) * 6 + c) * (zs + 1) + pr) * nh() + h) * nsl + slot) * 4 + i;
     }
 };
 inline PlaneK make_plane_k(int nx, int ny, int nz, const PlaneGeom& g) {
@@ -105,12 +109,12 @@ inline void plane_fill_tables(int ny, const PlaneGeom& g, int* kidx, int* slot_k
 BD_HD double plane_storage_value(const PlaneK& k, long idx, const int* slot_ky, const double* Kred) {
     const int i = (int)(idx % 4); idx /= 4;
     const int slot = (int)(idx % k.nsl); idx /= k.nsl;
-    const int h = (int)(idx % 2); idx /= 2;
+    const int h = (int)(idx % k.nh()); idx /= k.nh();
     const int pr = (int)(idx % (k.zs + 1)); idx /= (k.zs + 1);
     const int c = (int)(idx % 6); idx /= 6;
     const int qs = (int)(idx % k.nq); const int kx = (int)(idx / k.nq);
     const int ky = slot_ky[qs * k.nsl + slot];
-    if (ky < 0) return 0.0;
+    if (ky < 0 || 4 * h + i >= k.hb()) return 0.0;
     const int kz = pr < k.zs ? k.zs * (4 * h + i) + pr : k.zs * (4 * h + i + 1);
     return Kred[(((long)c * (k.nz + 1) + kz) * (k.ny + 1) + ky) * (k.nx + 1) + kx];
 }
@@ -119,7 +123,7 @@ BD_HD long plane_storage_index_of(const PlaneK& k, const int* kidx, int c, int k
     const int qs = ky % k.nq, e = pl_pos_of_freq(k.ls, ky / k.nq);
     const int slot = kidx[qs * k.ls + e] & 0xfff;
     int pr = kz % k.zs, m = kz / k.zs;
-    if (m >= 8) { pr = k.zs; m = 7; }          // the Nyquist plane kz = Pz/2 = ZS 8
+    if (m >= k.hb()) { pr = k.zs; m = k.hb() - 1; }          // the Nyquist plane kz = Pz/2 = ZS hb
     return k.index(kx, qs, c, pr, m / 4, slot, m % 4);
 }
 
@@ -200,10 +204,11 @@ BD_HD float pl_f4(const float4& v, int i) { return i == 0 ? v.x : (i == 1 ? v.y 
 // col: the column in shared memory (element z of component c at col[(c NZ + z) pitch]);
 // k: the lane's direct and mirror lists (pl_load_k: kA / kB point at h = 0 of component 0, kcs / khs are the float4
 // strides between components and halves); sy = -1 for a column at ky > Py/2.
-struct PlK { float4 d[2][6]; const float4* kB; };     // a lane's direct list [h][c]; its mirror list is read when needed
-BD_HD void pl_load_k(const float4* __restrict__ kA, const float4* __restrict__ kB, long kcs, long khs, PlK& k) {
+template <int NH> struct PlK { float4 d[NH][6]; const float4* kB; };     // a lane's direct list [h][c]; its mirror list is read when needed
+template <int NH>
+BD_HD void pl_load_k(const float4* __restrict__ kA, const float4* __restrict__ kB, long kcs, long khs, PlK<NH>& k) {
     BD_UNROLL
-    for (int h = 0; h < 2; ++h) {
+    for (int h = 0; h < NH; ++h) {
         BD_UNROLL
         for (int c = 0; c < 6; ++c) {
             k.d[h][c] = BD_LDG(kA + c * kcs + h * khs);
@@ -227,7 +232,7 @@ BD_HD float2 pl_w8(int m) {
 }
 
 template <int NZ>
-BD_HD void pl_zlane(int p, float sy, const float2* col, int pitch, const PlK& k, long kcs, long khs,
+BD_HD void pl_zlane(int p, float sy, const float2* col, int pitch, const PlK<(NZ >= 8 ? 2 : 1)>& k, long kcs, long khs,
                     const float2* __restrict__ zt, float2 (&v)[3][16]) {
     // first stage of the 2 NZ-point transform of the NZ cells, split by the residue p of kz modulo ZS = NZ / 8 and pruned to
     // its non-zero inputs:  a_p[j] = W_Pz^(j p) sum_{r < ZS/2} x[j + 16 r] W_ZS^(r p)
@@ -275,19 +280,20 @@ BD_HD void pl_zlane(int p, float sy, const float2* col, int pitch, const PlK& k,
             PkDft<16, -1>::run(v[c]);
         }
     } else {
-        // one lane, 16 frequencies, 8 cells: the zero padding prunes the transform itself
+        // one lane, all 2 NZ frequencies, NZ <= 8 cells: the zero padding prunes the transform itself
         BD_UNROLL
         for (int c = 0; c < 3; ++c) {
             BD_UNROLL
-            for (int j = 0; j < 8; ++j) v[c][j] = col[(c * 8 + j) * pitch];
-            PkDftPruned<16, -1>::run(v[c]);
+            for (int j = 0; j < NZ; ++j) v[c][j] = col[(c * NZ + j) * pitch];
+            PkDftPruned<2 * NZ, -1>::run(v[c]);
         }
     }
-    // direct frequencies m = 0..7, then the mirrored ones m = 15 - i
+    constexpr int NH = NZ >= 8 ? 2 : 1, HB = NZ >= 8 ? 8 : NZ, FPL = 2 * HB;     // list groups, list entries, the lane's frequencies
+    // direct frequencies m = 0..HB-1, then the mirrored ones m = FPL - 1 - i
     BD_UNROLL
-    for (int h = 0; h < 2; ++h) {
+    for (int h = 0; h < NH; ++h) {
         BD_UNROLL
-        for (int i = 0; i < 4; ++i) {
+        for (int i = 0; i < (HB < 4 ? HB : 4); ++i) {
             const int m = 4 * h + i;
             pl_mul3(pl_f4(k.d[h][0], i), pl_f4(k.d[h][1], i), pl_f4(k.d[h][2], i), sy * pl_f4(k.d[h][3], i), pl_f4(k.d[h][4], i),
                     sy * pl_f4(k.d[h][5], i), v[0][m], v[1][m], v[2][m]);
@@ -295,20 +301,20 @@ BD_HD void pl_zlane(int p, float sy, const float2* col, int pitch, const PlK& k,
     }
     // the mirror list is the direct list of the partner lane (same warp, same iteration): mostly still in L1
     BD_UNROLL
-    for (int h = 0; h < 2; ++h) {
+    for (int h = 0; h < NH; ++h) {
         float4 km[6];
         BD_UNROLL
         for (int c = 0; c < 6; ++c) km[c] = BD_LDG(k.kB + c * kcs + h * khs);
         BD_UNROLL
-        for (int i = 0; i < 4; ++i) {
-            const int m = 15 - (4 * h + i);
+        for (int i = 0; i < (HB < 4 ? HB : 4); ++i) {
+            const int m = FPL - 1 - (4 * h + i);
             pl_mul3(pl_f4(km[0], i), pl_f4(km[1], i), pl_f4(km[2], i), sy * pl_f4(km[3], i), -pl_f4(km[4], i),
                     -sy * pl_f4(km[5], i), v[0][m], v[1][m], v[2][m]);
         }
     }
-    if constexpr (NZ == 8) {
+    if constexpr (NZ <= 8) {
         BD_UNROLL
-        for (int c = 0; c < 3; ++c) PkDftTrunc<16, +1>::run(v[c]);       // the 8 cells: v[c][0..8)
+        for (int c = 0; c < 3; ++c) PkDftTrunc<2 * NZ, +1>::run(v[c]);   // the NZ cells: v[c][0..NZ)
     } else {
         BD_UNROLL
         for (int c = 0; c < 3; ++c) PkDft<16, +1>::run(v[c]);
@@ -389,9 +395,10 @@ template <int LS, int NQ, int NZ_ = kPlaneNZ>
 struct YZFused {
     using Args = YZArgs;
     static constexpr int KIND = kKindYZFused;
-    static constexpr int NZ = NZ_, NPEN = 3 * NZ, ZS = 2 * NZ / 16;
-    static constexpr int NT = NZ >= kPlaneNZ ? BD_YZ_NT : BD_YZ_NT * NZ / kPlaneNZ;   // thinner slabs: smaller blocks, 32 / NZ of them per SM
-    static constexpr int MINB = NZ >= kPlaneNZ ? 1 : kPlaneNZ / NZ;
+    static constexpr int NZ = NZ_, NPEN = 3 * NZ, ZS = NZ >= 8 ? 2 * NZ / 16 : 1, NH = NZ >= 8 ? 2 : 1;
+    // thinner slabs: smaller blocks (at least 96 threads), 32 / NZ (at most 4) of them per SM
+    static constexpr int NT = NZ >= kPlaneNZ ? BD_YZ_NT : (NZ >= 8 ? BD_YZ_NT * NZ / kPlaneNZ : BD_YZ_NT / 4);
+    static constexpr int MINB = NZ >= kPlaneNZ ? 1 : (NZ >= 8 ? kPlaneNZ / NZ : 4);
     static constexpr int NPHASES = 5;
     static constexpr int R0 = LS / 16;                   // first-pass radix; the second pass is radix 16
     static constexpr int PITCH = pl_pitch(LS);
@@ -521,21 +528,21 @@ struct YZFused {
 
     // phase 2: z transform, multiply, inverse z transform of every ky column; 4 lanes per column
     static BD_HD void zstage(int tid, int kx, int q, const Args& a, float2* sm) {
-        const float4* kbase = reinterpret_cast<const float4*>(a.KP) + (long)kx * (NQ * 6L * (ZS + 1) * 2 * NSL);
-        constexpr long KCS = (long)(ZS + 1) * 2 * NSL, KHS = NSL;
+        const float4* kbase = reinterpret_cast<const float4*>(a.KP) + (long)kx * (NQ * 6L * (ZS + 1) * NH * NSL);
+        constexpr long KCS = (long)(ZS + 1) * NH * NSL, KHS = NSL;
         // item w = (column e, lane p): its kernel-spectrum lists and the sign of the y-odd components
-        auto lists = [&](int w, PlK& k) {
+        auto lists = [&](int w, PlK<NH>& k) {
             const int p = w & (ZS - 1), e = w / ZS;
             const int ki = BD_LDG(&a.kidx[q * LS + e]);
             const float4* kq = kbase + (long)((ki >> 12) & 7) * 6 * KCS + (ki & 0xfff);
-            pl_load_k(kq + (long)p * 2 * NSL, kq + (long)(p ? ZS - p : ZS) * 2 * NSL, KCS, KHS, k);
+            pl_load_k<NH>(kq + (long)p * NH * NSL, kq + (long)(p ? ZS - p : ZS) * NH * NSL, KCS, KHS, k);
             return (ki >> 15) ? -1.f : 1.f;
         };
         for (int w = tid; w < LS * ZS; w += NT) {
             const int p = w & (ZS - 1), e = w / ZS;
             float2* col = sm + pl_pe(e);
 #if defined(__CUDA_ARCH__)
-            PlK kc;
+            PlK<NH> kc;
             const float sy = lists(w, kc);
             float2 y[3][16];
             pl_zlane<NZ>(p, sy, col, PITCH, kc, KCS, KHS, a.zt, y);
@@ -624,7 +631,7 @@ struct YZFused {
                 BD_UNROLL
                 for (int c = 0; c < 3; ++c) {
                     BD_UNROLL
-                    for (int j = 0; j < 8; ++j) col[(c * NZ + j) * PITCH] = y[c][j];
+                    for (int j = 0; j < NZ; ++j) col[(c * NZ + j) * PITCH] = y[c][j];
                 }
             }
 #else
@@ -632,7 +639,7 @@ struct YZFused {
             if (p != 0) continue;
             float2 y[ZS][3][16];
             for (int pp = 0; pp < ZS; ++pp) {
-                PlK k;
+                PlK<NH> k;
                 const float sy = lists(w + pp, k);
                 pl_zlane<NZ>(pp, sy, col, PITCH, k, KCS, KHS, a.zt, y[pp]);
             }
@@ -652,7 +659,7 @@ struct YZFused {
                     } else if constexpr (ZS == 2) {
                         col[(c * NZ + j) * PITCH] = pk_add(y[0][c][j], y[1][c][j]);
                     } else {
-                        if (j < 8) col[(c * NZ + j) * PITCH] = y[0][c][j];
+                        if (j < NZ) col[(c * NZ + j) * PITCH] = y[0][c][j];
                     }
                 }
 #endif
@@ -663,7 +670,7 @@ struct YZFused {
     // L2 (the blocks of one kx run side by side: between them they fetch all of its slots)
     static BD_HD void prologue(int tid, int bx, const Args& a) {
         const int kx = bx / NQ, q = q_of_order(bx % NQ);
-        constexpr long KB = 6L * (ZS + 1) * 2 * NSL * 4 * (long)sizeof(float);
+        constexpr long KB = 6L * (ZS + 1) * NH * NSL * 4 * (long)sizeof(float);
         const char* kq = reinterpret_cast<const char*>(a.KP) + ((long)kx * NQ + q) * KB;
         for (long o = (long)tid * 128; o < KB; o += NT * 128) bd_prefetch_l2(kq + o);
     }

@@ -210,7 +210,7 @@ def test_float3_layout_and_accumulate_variants_match_the_oracle(shape):
 
 
 def test_kernel_path_chosen_per_mesh():
-    expect = {(1, 32, 32): 2, (1, 1024, 1024): 2, (128, 128, 128): 3, (32, 512, 512): 4, (32, 256, 16): 4, (32, 1024, 64): 4, (32, 64, 1024): 4, (16, 512, 512): 4, (8, 64, 64): 4, (16, 16, 64): 3, (4, 64, 64): 3, (64, 64, 512): 4, (64, 64, 256): 3, (32, 16, 1024): 0, (512, 2, 4): 0}
+    expect = {(1, 32, 32): 2, (1, 1024, 1024): 2, (128, 128, 128): 3, (32, 512, 512): 4, (32, 256, 16): 4, (32, 1024, 64): 4, (32, 64, 1024): 4, (16, 512, 512): 4, (8, 64, 64): 4, (16, 16, 64): 3, (4, 64, 64): 4, (2, 32, 32): 4, (4, 16, 64): 3, (64, 64, 512): 4, (64, 64, 256): 3, (32, 16, 1024): 0, (512, 2, 4): 0}
     for (nz, ny, nx), path in expect.items():
         plan = binding.DemagPlan(nx, ny, nz, 2e-9, 2e-9, 1e-9)
         assert plan.layout()["path"] == path
@@ -466,7 +466,9 @@ def test_1024x1024x32_film_sampled_against_the_written_out_sum():
 # ----------------------------------------------------------------- plane path on 16- and 8-cell slabs (the paper's pipelined regime, L283)
 @pytest.mark.parametrize("shape,texture", [((16, 64, 128), "helix"), ((8, 256, 64), "random"), ((16, 1024, 16), "random"),
                                            ((8, 32, 32), "vortex"), ((8, 40, 100), "random"), ((16, 512, 512), "helix"),
-                                           ((64, 32, 512), "random"), ((64, 256, 512), "helix"), ((64, 48, 1000), "random")])
+                                           ((64, 32, 512), "random"), ((64, 256, 512), "helix"), ((64, 48, 1000), "random"),
+                                           ((4, 256, 64), "random"), ((2, 512, 128), "helix"), ((4, 40, 20), "random"),
+                                           ((2, 1024, 16), "random"), ((4, 1024, 1024), "helix")])
 def test_plane_path_on_thin_slabs(shape, texture):
     nz, ny, nx = shape
     h, Ms = (2e-9, 3e-9, 1e-9), 8e5
@@ -486,7 +488,7 @@ def test_plane_path_on_thin_slabs(shape, texture):
     plan.close()
 
 
-@pytest.mark.parametrize("shape", [(16, 64, 128), (8, 256, 64), (32, 64, 32)])
+@pytest.mark.parametrize("shape", [(16, 64, 128), (8, 256, 64), (32, 64, 32), (4, 128, 64), (2, 64, 256)])
 def test_tiled_3d_kernels_stay_reachable_on_slabs_the_plane_path_takes(shape, monkeypatch):
     """BORIS_DEMAG_NO_PLANE=1 at plan creation selects XZFwd / YFused / ZXInv (the A/B switch of profiles/r02_plane.md)."""
     nz, ny, nx = shape

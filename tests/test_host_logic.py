@@ -226,6 +226,10 @@ PLANE_CASES = [
     ((8, 64, 8), (2.0, 3.0, 1.0), "random", 0),           # 8 cells: one lane, the transform itself pruned; LS = 128
     ((8, 512, 4), (2.0, 2.0, 1.0), "random", 0),          # 8 cells, four residues
     ((8, 128, 4), (4.0, 4.0, 1.0), "random", 4),          # 8 cells, LS = 64, four residues
+    ((4, 64, 8), (2.0, 3.0, 1.0), "random", 0),           # 4 cells: one lane, 8 frequencies
+    ((4, 512, 4), (2.0, 2.0, 1.0), "helix", 0),           # 4 cells, four residues
+    ((2, 32, 16), (3.0, 2.0, 1.0), "random", 0),          # 2 cells: one lane, 4 frequencies
+    ((2, 256, 4), (2.0, 2.0, 2.0), "random", 0),          # 2 cells, two residues
     ((64, 32, 4), (2.0, 2.0, 1.0), "random", 1),          # 64 cells: eight lanes per column; LS = 64
     ((64, 128, 4), (2.0, 3.0, 2.0), "helix", 2),          # 64 cells, LS = 128, two residues
 ]
@@ -317,14 +321,14 @@ def asan_emu():
 # residues), chunked fallback
 @pytest.mark.parametrize("args", [(8, 512, 4), (128, 256, 2), (64, 8, 1), (4, 2, 1), (16, 4, 8), (8, 4, 64), (4, 32, 32),
                                   (8, 64, 32, 0, 2), (4, 128, 32, 0, 4), (4, 256, 32, 0, 8), (8, 16, 8, -1), (16, 8, 4, 3),
-                                  (8, 32, 16), (4, 64, 8), (8, 128, 16, 0, 2), (4, 32, 8, 0, -1), (4, 64, 64, 0, 1), (4, 128, 64, 0, 2)])
+                                  (8, 32, 16), (4, 64, 8), (8, 128, 16, 0, 2), (4, 32, 8, 0, -1), (4, 64, 64, 0, 1), (4, 128, 64, 0, 2), (8, 64, 4), (4, 32, 2), (8, 128, 2, 0, 2)])
 def test_emulation_under_address_sanitizer(asan_emu, args):
     import subprocess
     res = subprocess.run([asan_emu] + [str(a) for a in args], capture_output=True, text=True, timeout=900)
     assert res.returncode == 0, res.stdout[-500:] + res.stderr[-3000:]
 
 
-@pytest.mark.parametrize("shape", [(16, 32, 32), (8, 32, 16), (32, 32, 8)])
+@pytest.mark.parametrize("shape", [(16, 32, 32), (8, 32, 16), (32, 32, 8), (4, 32, 16), (2, 64, 8)])
 def test_emulated_tiled_3d_kernels_on_slabs_the_plane_path_would_take(emu, shape):
     """XZFwd / YFused / ZXInv stay reachable (BORIS-internal choice: the plane path takes these slabs by default)."""
     nz, ny, nx = shape
