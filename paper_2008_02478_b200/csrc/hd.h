@@ -19,6 +19,11 @@
 #define BD_LDG(p) __ldg(p)
 #define BD_LDCG(p) __ldcg(p)
 #define BD_STCG(p, v) __stcg((p), (v))
+#if defined(BD_PLAIN_STS)
+#define BD_STS(p, v) (*(p) = (v))
+#else
+#define BD_STS(p, v) bd_sts_pair((p), (v))
+#endif
 #define BD_UNROLL _Pragma("unroll")
 #define BD_PRAGMA_(x) _Pragma(#x)
 #define BD_UNROLL_N(n) BD_PRAGMA_(unroll n)
@@ -28,6 +33,7 @@
 #define BD_STCG(p, v) (*(p) = (v))
 #define BD_UNROLL
 #define BD_UNROLL_N(n)
+#define BD_STS(p, v) (*(p) = (v))
 #endif
 
 #include <vector_types.h>   // float2, float4, double2 (plain structs on the host)
@@ -42,3 +48,13 @@ BD_HD void bd_prefetch_l2(const void* p) {
     (void)p;
 #endif
 }
+
+// Store of a complex pair to SHARED memory (p must point into shared memory).  Written as st.shared.v2.f32: for the
+// plain C++ store of a float2 that came out of a packed f32x2 operation nvcc emits st.shared.u64, and ptxas (12.9)
+// then copies every such register pair into one fixed pair first (two MOVs per STS.64: 15 - 25 % of the
+// instructions of a register-DFT pass, profiles/r02_plane.md).
+#if defined(__CUDA_ARCH__)
+__device__ __forceinline__ void bd_sts_pair(float2* p, float2 v) {
+    asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"((unsigned)__cvta_generic_to_shared(p)), "f"(v.x), "f"(v.y) : "memory");
+}
+#endif

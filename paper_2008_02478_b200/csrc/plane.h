@@ -147,13 +147,20 @@ inline void plane_fill_tw(float2* h, int ny, const PlaneGeom& g) {
                 h[(q * R0 + q0) * 16 + j] = w;
             }
 }
-// zt[p 16 + j] = W_Pz^(j p), p < ZS, j < 16
+// Slot j of lane p of a 4- or 2-lane z stage holds cell (and inverse-transform output) pl_zrot(ZS, p, j): the lane's 16
+// values rotated by its own block of 16 / ZS, which puts the block the lane keeps in slots [0, 16 / ZS) and the block
+// lane p + r needs in slots [16 - r 16 / ZS, ...) for EVERY lane: the exchange of the partial inverse transforms needs
+// no per-lane selection of registers.  (Rotating the inputs of the 16-point transform by s modulates its outputs by
+// W_16^(-s m); the multiplication by the real K^ keeps that factor, and the inverse transform turns it back into the
+// same rotation of the outputs.)  The 8-lane stage of nz = 64 is not rotated.
+BD_HD constexpr int pl_zrot(int zs, int p, int j) { return (zs == 4 || zs == 2) ? ((j + (16 / zs) * p) & 15) : j; }
+// zt[p 16 + j] = W_Pz^(j' p), j' = pl_zrot(ZS, p, j), p < ZS, j < 16
 inline void plane_fill_zt(float2* h, int nz, const PlaneGeom& g) {
     const double pi = 3.14159265358979323846264338327950288;
     const int Pz = 2 * nz;
     for (int p = 0; p < g.zs; ++p)
         for (int j = 0; j < 16; ++j) {
-            const int m = (j * p) % Pz;
+            const int m = (pl_zrot(g.zs, p, j) * p) % Pz;
             float2 w;
             if ((4 * m) % Pz == 0) {
                 const float cx[4] = {1.f, 0.f, -1.f, 0.f}, sy[4] = {0.f, -1.f, 0.f, 1.f};
@@ -198,9 +205,10 @@ BD_HD void pl_mul3(float kxx, float kyy, float kzz, float kxy, float kxz, float 
 BD_HD float pl_f4(const float4& v, int i) { return i == 0 ? v.x : (i == 1 ? v.y : (i == 2 ? v.z : v.w)); }
 
 // One lane of a ky column: frequencies kz = ZS m + p, m < 16, of the 2 NZ-point z transform of the NZ cells
-// (ZS = NZ / 8 lanes per column: 4, 2 or 1); returns its part y[c][j] of the inverse transform: for NZ = 32
+// (ZS = NZ / 8 lanes per column: 4, 2 or 1); returns its part y_p[c][j] of the inverse transform: for NZ = 32
 //     out[j] = sum_p y_p[j],   out[j + 16] = sum_p i^p y_p[j]          (j < 16),
-// for NZ = 16 out[j] = y_0[j] + y_1[j], for NZ = 8 out[j] = y[j], j < 8.
+// for NZ = 16 out[j] = y_0[j] + y_1[j], for NZ = 8 out[j] = y[j], j < 8.  For NZ = 32 and 16 the lane works on rotated
+// slots (pl_zrot): v[c][j] = y_p[c][pl_zrot(ZS, p, j)].
 // col: the column in shared memory (element z of component c at col[(c NZ + z) pitch]);
 // k: the lane's direct and mirror lists (pl_load_k: kA / kB point at h = 0 of component 0, kcs / khs are the float4
 // strides between components and halves); sy = -1 for a column at ky > Py/2.
@@ -261,22 +269,29 @@ BD_HD void pl_zlane(int p, float sy, const float2* col, int pitch, const PlK<(NZ
         Tw rot;
         rot.c = p == 0 ? 1.f : (p == 2 ? -1.f : 0.f);
         { const float s = p == 1 ? -1.f : (p == 3 ? 1.f : 0.f); rot.ns = bd_f2(-s, s); }
+        // slot j = 4 a + b reads cell pl_zrot(4, p, j) = 4 ((a + p) & 3) + b
+        const float2* cr[4];
+        BD_UNROLL
+        for (int a = 0; a < 4; ++a) cr[a] = col + 4 * ((a + p) & 3) * pitch;
         BD_UNROLL
         for (int c = 0; c < 3; ++c) {
             BD_UNROLL
             for (int j = 0; j < 16; ++j) {
                 const Tw t = make_tw(BD_LDG(&zt[p * 16 + j]));
-                const float2 x0 = col[(c * 32 + j) * pitch], x1 = col[(c * 32 + j + 16) * pitch];
+                const float2 x0 = cr[j >> 2][(c * 32 + (j & 3)) * pitch], x1 = cr[j >> 2][(c * 32 + (j & 3) + 16) * pitch];
                 const float2 a = pk_fma(pk_swap(x1), rot.ns, pk_fma(x1, pk_bc(rot.c), x0));
                 v[c][j] = pk_cmul(a, t);
             }
             PkDft<16, -1>::run(v[c]);
         }
     } else if constexpr (NZ == 16) {
+        // slot j = 8 a + b reads cell pl_zrot(2, p, j) = 8 ((a + p) & 1) + b
+        const float2* cr[2] = {col + 8 * (p & 1) * pitch, col + 8 * ((p + 1) & 1) * pitch};
         BD_UNROLL
         for (int c = 0; c < 3; ++c) {
             BD_UNROLL
-            for (int j = 0; j < 16; ++j) v[c][j] = pk_cmul(col[(c * 16 + j) * pitch], make_tw(BD_LDG(&zt[p * 16 + j])));
+            for (int j = 0; j < 16; ++j)
+                v[c][j] = pk_cmul(cr[j >> 3][(c * 16 + (j & 7)) * pitch], make_tw(BD_LDG(&zt[p * 16 + j])));
             PkDft<16, -1>::run(v[c]);
         }
     } else {
@@ -449,8 +464,8 @@ struct YZFused {
                 float2* po = sm + pc * PITCH + j;
                 BD_UNROLL
                 for (int q0 = 0; q0 < R0; ++q0) {
-                    if (Q == 0 && q0 == 0) po[0] = v[0];
-                    else po[17 * q0] = pk_cmul(v[q0], tw[q0]);
+                    if (Q == 0 && q0 == 0) BD_STS(po + 0, v[0]);
+                    else BD_STS(po + 17 * q0, pk_cmul(v[q0], tw[q0]));
                 }
             }
             return;
@@ -480,8 +495,8 @@ struct YZFused {
             float2* po = sm + pc * PITCH + j;
             BD_UNROLL
             for (int q0 = 0; q0 < R0; ++q0) {
-                if (Q == 0 && q0 == 0) po[0] = v[0];
-                else po[17 * q0] = pk_cmul(v[q0], tw[q0]);
+                if (Q == 0 && q0 == 0) BD_STS(po + 0, v[0]);
+                else BD_STS(po + 17 * q0, pk_cmul(v[q0], tw[q0]));
             }
         }
     }
@@ -491,14 +506,24 @@ struct YZFused {
     static BD_HD void pass16(int tid, float2* sm) {
         constexpr int PG = NT / R0;
         const int q0 = tid % R0, pg = tid / R0;
+        // the next pencil's points are read before this one's transform: their latency runs under the arithmetic
+        float2 nxt[16];
+        if (pg < NPEN) {
+            BD_UNROLL
+            for (int i = 0; i < 16; ++i) nxt[i] = sm[pg * PITCH + 17 * q0 + i];
+        }
         for (int pc = pg; pc < NPEN; pc += PG) {
             float2* ps = sm + pc * PITCH + 17 * q0;
             float2 v[16];
             BD_UNROLL
-            for (int i = 0; i < 16; ++i) v[i] = ps[i];
+            for (int i = 0; i < 16; ++i) v[i] = nxt[i];
+            if (pc + PG < NPEN) {
+                BD_UNROLL
+                for (int i = 0; i < 16; ++i) nxt[i] = ps[PG * PITCH + i];
+            }
             PkDft<16, DIR>::run(v);
             BD_UNROLL
-            for (int i = 0; i < 16; ++i) ps[i] = v[i];
+            for (int i = 0; i < 16; ++i) BD_STS(ps + i, v[i]);
         }
     }
 
@@ -547,37 +572,26 @@ struct YZFused {
             float2 y[3][16];
             pl_zlane<NZ>(p, sy, col, PITCH, kc, KCS, KHS, a.zt, y);
             if constexpr (ZS == 4) {
-                // out[j] = sum_p y_p[j], out[j + 16] = sum_p i^p y_p[j]: two exchange rounds among the 4 lanes
-                const bool hi = (p & 2) != 0, lo = (p & 1) != 0;
-                const float sg = hi ? -1.f : 1.f;
-                float2 S[3][8], D[3][8];
-                BD_UNROLL
-                for (int c = 0; c < 3; ++c) {
-                    BD_UNROLL
-                    for (int i = 0; i < 8; ++i) {
-                        const float2 send = hi ? y[c][i] : y[c][8 + i], mine = hi ? y[c][8 + i] : y[c][i];
-                        float2 oth;
-                        oth.x = __shfl_xor_sync(0xffffffffu, send.x, 2);
-                        oth.y = __shfl_xor_sync(0xffffffffu, send.y, 2);
-                        S[c][i] = pk_add(mine, oth);
-                        D[c][i] = pk_mul(pk_sub(mine, oth), pk_bc(sg));
-                    }
-                }
-                const int jb = (hi ? 8 : 0) + (lo ? 4 : 0);
+                // out[j] = sum_p y_p[j], out[j + 16] = sum_p i^p y_p[j].  The lane keeps j = 4 p + i, i < 4: its own values
+                // sit in slots i, those of lane p + r (mod 4) in that lane's slots 16 - 4 r + i (pl_zrot): three rounds, the
+                // same registers sent by every lane.  sum_s i^s y_s = i^p (t_0 + i t_1 - t_2 - i t_3), t_r from lane p + r
+                Tw ip;
+                ip.c = p == 0 ? 1.f : (p == 2 ? -1.f : 0.f);
+                { const float sn = p == 1 ? 1.f : (p == 3 ? -1.f : 0.f); ip.ns = bd_f2(-sn, sn); }
                 BD_UNROLL
                 for (int c = 0; c < 3; ++c) {
                     BD_UNROLL
                     for (int i = 0; i < 4; ++i) {
-                        const float2 sS = lo ? S[c][i] : S[c][4 + i], sD = lo ? D[c][i] : D[c][4 + i];
-                        const float2 kS = lo ? S[c][4 + i] : S[c][i], kD = lo ? D[c][4 + i] : D[c][i];
-                        float2 rS, rD;
-                        rS.x = __shfl_xor_sync(0xffffffffu, sS.x, 1);
-                        rS.y = __shfl_xor_sync(0xffffffffu, sS.y, 1);
-                        rD.x = __shfl_xor_sync(0xffffffffu, sD.x, 1);
-                        rD.y = __shfl_xor_sync(0xffffffffu, sD.y, 1);
-                        const float2 ev = lo ? rD : kD, od = lo ? kD : rD;
-                        col[(c * NZ + jb + i) * PITCH] = pk_add(kS, rS);
-                        col[(c * NZ + 16 + jb + i) * PITCH] = pk_add_ib<+1>(ev, od);
+                        float2 t[4];
+                        t[0] = y[c][i];
+                        BD_UNROLL
+                        for (int r = 1; r < 4; ++r) {
+                            t[r].x = __shfl_sync(0xffffffffu, y[c][16 - 4 * r + i].x, (p + r) & 3, 4);
+                            t[r].y = __shfl_sync(0xffffffffu, y[c][16 - 4 * r + i].y, (p + r) & 3, 4);
+                        }
+                        BD_STS(col + (c * NZ + 4 * p + i) * PITCH, pk_add(pk_add(t[0], t[2]), pk_add(t[1], t[3])));
+                        BD_STS(col + (c * NZ + 16 + 4 * p + i) * PITCH,
+                               pk_cmul(pk_add_ib<+1>(pk_sub(t[0], t[2]), pk_sub(t[1], t[3])), ip));
                     }
                 }
             } else if constexpr (ZS == 8) {
@@ -607,31 +621,29 @@ struct YZFused {
                 for (int c = 0; c < 3; ++c) {
                     BD_UNROLL
                     for (int i = 0; i < 2; ++i) {
-                        col[(c * NZ + jb + i) * PITCH] = r0[c][i];
-                        col[(c * NZ + 16 + jb + i) * PITCH] = r1[c][i];
-                        col[(c * NZ + 32 + jb + i) * PITCH] = r2[c][i];
-                        col[(c * NZ + 48 + jb + i) * PITCH] = r3[c][i];
+                        BD_STS(col + (c * NZ + jb + i) * PITCH, r0[c][i]);
+                        BD_STS(col + (c * NZ + 16 + jb + i) * PITCH, r1[c][i]);
+                        BD_STS(col + (c * NZ + 32 + jb + i) * PITCH, r2[c][i]);
+                        BD_STS(col + (c * NZ + 48 + jb + i) * PITCH, r3[c][i]);
                     }
                 }
             } else if constexpr (ZS == 2) {
-                // out[j] = y_0[j] + y_1[j]: each lane keeps eight cells and sends the other eight
-                const bool lo = (p & 1) != 0;
+                // out[j] = y_0[j] + y_1[j]: the lane keeps j = 8 p + i (its slots i) and sends its slots 8 + i (pl_zrot)
                 BD_UNROLL
                 for (int c = 0; c < 3; ++c) {
                     BD_UNROLL
                     for (int i = 0; i < 8; ++i) {
-                        const float2 send = lo ? y[c][i] : y[c][8 + i], mine = lo ? y[c][8 + i] : y[c][i];
                         float2 oth;
-                        oth.x = __shfl_xor_sync(0xffffffffu, send.x, 1);
-                        oth.y = __shfl_xor_sync(0xffffffffu, send.y, 1);
-                        col[(c * NZ + (lo ? 8 : 0) + i) * PITCH] = pk_add(mine, oth);
+                        oth.x = __shfl_xor_sync(0xffffffffu, y[c][8 + i].x, 1);
+                        oth.y = __shfl_xor_sync(0xffffffffu, y[c][8 + i].y, 1);
+                        BD_STS(col + (c * NZ + 8 * p + i) * PITCH, pk_add(y[c][i], oth));
                     }
                 }
             } else {
                 BD_UNROLL
                 for (int c = 0; c < 3; ++c) {
                     BD_UNROLL
-                    for (int j = 0; j < NZ; ++j) col[(c * NZ + j) * PITCH] = y[c][j];
+                    for (int j = 0; j < NZ; ++j) BD_STS(col + (c * NZ + j) * PITCH, y[c][j]);
                 }
             }
 #else
@@ -652,12 +664,18 @@ struct YZFused {
                             col[(c * NZ + 16 * r + j) * PITCH] = acc;
                         }
                     } else if constexpr (ZS == 4) {
-                        const float2 Se = pk_add(y[0][c][j], y[2][c][j]), So = pk_add(y[1][c][j], y[3][c][j]);
-                        const float2 De = pk_sub(y[0][c][j], y[2][c][j]), Do = pk_sub(y[1][c][j], y[3][c][j]);
-                        col[(c * NZ + j) * PITCH] = pk_add(Se, So);
-                        col[(c * NZ + 16 + j) * PITCH] = pk_add_ib<+1>(De, Do);
+                        // y_p[j] sits in lane p's slot (j - 4 p) & 15 (pl_zrot); lane pk = j / 4 combines, starting with its own
+                        const int pk = j >> 2;
+                        float2 t[4];
+                        for (int r = 0; r < 4; ++r) t[r] = y[(pk + r) & 3][c][(j - 4 * ((pk + r) & 3)) & 15];
+                        Tw ip;
+                        ip.c = pk == 0 ? 1.f : (pk == 2 ? -1.f : 0.f);
+                        { const float sn = pk == 1 ? 1.f : (pk == 3 ? -1.f : 0.f); ip.ns = bd_f2(-sn, sn); }
+                        col[(c * NZ + j) * PITCH] = pk_add(pk_add(t[0], t[2]), pk_add(t[1], t[3]));
+                        col[(c * NZ + 16 + j) * PITCH] = pk_cmul(pk_add_ib<+1>(pk_sub(t[0], t[2]), pk_sub(t[1], t[3])), ip);
                     } else if constexpr (ZS == 2) {
-                        col[(c * NZ + j) * PITCH] = pk_add(y[0][c][j], y[1][c][j]);
+                        const int pk = j >> 3;
+                        col[(c * NZ + j) * PITCH] = pk_add(y[pk][c][j & 7], y[pk ^ 1][c][8 + (j & 7)]);
                     } else {
                         if (j < NZ) col[(c * NZ + j) * PITCH] = y[0][c][j];
                     }

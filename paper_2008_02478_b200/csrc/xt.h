@@ -33,9 +33,9 @@ struct SRows {
     static BD_HD constexpr int off(int S, int r) { return prow(L, r * S); }
     BD_HD float2* ptr(int row, int e) const { return p + row * PITCH + prow(L, e); }
     static BD_HD float2 ld(const float2* q) { return *q; }
-    BD_HD void st(float2* q, float2 v) const { *q = v; }
+    BD_HD void st(float2* q, float2 v) const { BD_STS(q, v); }
     BD_HD void pre(const float2*, int) const {}
-    BD_HD void stq(float2* q, float2 v, int) const { *q = v; }
+    BD_HD void stq(float2* q, float2 v, int) const { BD_STS(q, v); }
 };
 struct GRowsIn {               // rows of a real array read as (x[2m], x[2m+1]) pairs
     const float* p; long pitch;
@@ -283,8 +283,8 @@ struct XInvT {
                         const float2 D = bd_f2(Yk[u].x - Ym[u].x, Yk[u].y + Ym[u].y);
                         const float2 O = pk_cmulc(D, make_tw(bd_f2(xp[u].x, xp[u].y)));
                         float2* zr = sm + row * SRows<LX>::PITCH;
-                        zr[bd_float_as_int(xp[u].z)] = bd_f2(E.x - O.y, E.y + O.x);
-                        if (kp != 0 && 2 * kp != LX) zr[bd_float_as_int(xp[u].w)] = bd_f2(E.x + O.y, O.x - E.y);
+                        BD_STS(zr + bd_float_as_int(xp[u].z), bd_f2(E.x - O.y, E.y + O.x));
+                        if (kp != 0 && 2 * kp != LX) BD_STS(zr + bd_float_as_int(xp[u].w), bd_f2(E.x + O.y, O.x - E.y));
                     }
                 }
             }

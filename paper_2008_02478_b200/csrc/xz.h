@@ -271,7 +271,7 @@ struct ZXInv {
             if (p == 0) {
                 for (int m = 0; m < SP / 2; ++m) {
                     BD_UNROLL
-                    for (int z = 0; z < SUB; ++z) col[(z + SUB * m) * PITCH] = v[z];
+                    for (int z = 0; z < SUB; ++z) BD_STS(col + (z + SUB * m) * PITCH, v[z]);
                 }
             } else {
                 for (int m = 0; m < SP / 2; ++m) {
@@ -279,7 +279,7 @@ struct ZXInv {
                     BD_UNROLL
                     for (int z = 0; z < SUB; ++z) {
                         float2* q = col + (z + SUB * m) * PITCH;
-                        *q = pk_add(*q, pk_cmulc(v[z], w));
+                        BD_STS(q, pk_add(*q, pk_cmulc(v[z], w)));
                     }
                 }
             }
@@ -324,10 +324,10 @@ struct ZXInv {
         ZCol<PZ>::template inv_half<PAR>(v);
         if constexpr (PAR == 0) {
             BD_UNROLL
-            for (int z = 0; z < NZ; ++z) col[z * PITCH] = v[z];
+            for (int z = 0; z < NZ; ++z) BD_STS(col + z * PITCH, v[z]);
         } else {
             BD_UNROLL
-            for (int z = 0; z < NZ; ++z) col[z * PITCH] = pk_add(col[z * PITCH], v[z]);
+            for (int z = 0; z < NZ; ++z) BD_STS(col + z * PITCH, pk_add(col[z * PITCH], v[z]));
         }
     }
 

@@ -75,9 +75,9 @@ struct STile {                 // shared: S[c][p(e)][col]
     static BD_HD constexpr int off(int S, int r) { return r * pstep(S) * COLS; }
     BD_HD float2* ptr(int c, int e) const { return p + c * CP + pidx(e) * COLS; }
     static BD_HD float2 ld(const float2* q) { return *q; }
-    BD_HD void st(float2* q, float2 v) const { *q = v; }
+    BD_HD void st(float2* q, float2 v) const { BD_STS(q, v); }
     BD_HD void pre(const float2*, int) const {}
-    BD_HD void stq(float2* q, float2 v, int) const { *q = v; }
+    BD_HD void stq(float2* q, float2 v, int) const { BD_STS(q, v); }
 };
 template <int COLS>
 struct GTile {                 // global: V tile [y][col], component stride cstride
