@@ -98,6 +98,8 @@ def lib():
         L.boris_demag_ml_pair_tensor_host.argtypes = [c_int, c_int, c_dbl, c_dbl, c_dbl, c_dbl, c_dbl, c_vp]
         L.boris_demag_plan_mesh.restype = c_int
         L.boris_demag_plan_mesh.argtypes = [c_vp, ctypes.POINTER(c_int), ctypes.POINTER(c_dbl)]
+        L.boris_demag_energy_noalloc.restype = c_int
+        L.boris_demag_energy_noalloc.argtypes = [c_vp, c_vp, ctypes.c_longlong, c_dbl, c_dbl, c_dbl, c_vp, c_vp]
         L.boris_micro_fp32_rate.restype = c_int
         L.boris_micro_fp32_rate.argtypes = [c_int, ctypes.POINTER(c_dbl)]
         L.boris_micro_segment_bw.restype = c_int
@@ -439,6 +441,28 @@ class MultiLayerPlan:
         _check(lib().boris_demag_ml_energy(self._h, self._ptr(M, "M"), self._ptr(H, "H"), E.data_ptr(), st),
                "boris_demag_ml_energy")
         return E
+
+
+# ----------------------------------------------------------------- no allocation (include/boris_demag_noalloc.h)
+NOALLOC_MAX_VALUES = 1 << 27
+
+
+def energy_noalloc(M, H, h, E, stream=None):
+    """boris_demag_energy_noalloc: E[0] <- -(mu0/2) hx hy hz sum M.H with the reduction scratch in the library's static
+    device array (no plan, no allocation: E is the caller's CUDA float64 tensor).  Asynchronous; calls that overlap on
+    the GPU race on the shared array."""
+    import torch
+    for t, name in ((M, "M"), (H, "H")):
+        if not (t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+            raise DemagError(f"{name} must be a contiguous CUDA float32 tensor")
+    if M.numel() != H.numel():
+        raise DemagError("M and H must have the same number of elements")
+    if not (E.is_cuda and E.dtype == torch.float64 and E.numel() >= 1):
+        raise DemagError("E must be a CUDA float64 tensor")
+    st = (stream or torch.cuda.current_stream()).cuda_stream
+    _check(lib().boris_demag_energy_noalloc(M.data_ptr(), H.data_ptr(), M.numel(), float(h[0]), float(h[1]), float(h[2]),
+                                            E.data_ptr(), st), "boris_demag_energy_noalloc")
+    return E
 
 
 # ----------------------------------------------------------------- device probes (include/boris_micro.h)

@@ -16,7 +16,7 @@ CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "libborisdemag.so")
 # one translation unit per group of kernels, compiled in parallel and linked into one library
 SOURCES = [os.path.join(CSRC, f) for f in ("boris_demag.cu", "tu_t2d.cu", "tu_y3.cu", "tu_xz_a.cu", "tu_xz_b.cu",
-                                            "tu_xz_c.cu", "tu_plane_x.cu", "tu_plane_yz.cu", "tu_plane_yz16.cu", "tu_plane_yz8.cu", "tu_plane_yz64.cu", "boris_llg.cu", "microbench.cu", "boris_demag_f64.cu", "boris_demag_ml.cu")]
+                                            "tu_xz_c.cu", "tu_plane_x.cu", "tu_plane_yz.cu", "tu_plane_yz16.cu", "tu_plane_yz8.cu", "tu_plane_yz64.cu", "boris_llg.cu", "microbench.cu", "boris_demag_f64.cu", "boris_demag_ml.cu", "boris_demag_noalloc.cu")]
 OBJDIR = os.path.join(HERE, "build")
 NVCC_FLAGS = ["-std=c++17", "-O3", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a",
               "-Xcompiler", "-fPIC"]
@@ -36,6 +36,7 @@ def _deps():
     deps.append(os.path.join(ROOT, "include", "boris_micro.h"))
     deps.append(os.path.join(ROOT, "include", "boris_demag_f64.h"))
     deps.append(os.path.join(ROOT, "include", "boris_demag_ml.h"))
+    deps.append(os.path.join(ROOT, "include", "boris_demag_noalloc.h"))
     return deps
 
 

@@ -13,6 +13,7 @@ HEADER_LLG = os.path.join(ROOT, "include", "boris_llg.h")
 HEADER_MICRO = os.path.join(ROOT, "include", "boris_micro.h")
 HEADER_F64 = os.path.join(ROOT, "include", "boris_demag_f64.h")
 HEADER_ML = os.path.join(ROOT, "include", "boris_demag_ml.h")
+HEADER_NOALLOC = os.path.join(ROOT, "include", "boris_demag_noalloc.h")
 
 
 @pytest.fixture(scope="session", autouse=True)
@@ -21,7 +22,7 @@ def built_library():
 
 
 def declared_symbols():
-    text = open(HEADER).read() + open(HEADER_LLG).read() + open(HEADER_MICRO).read() + open(HEADER_F64).read() + open(HEADER_ML).read()
+    text = open(HEADER).read() + open(HEADER_LLG).read() + open(HEADER_MICRO).read() + open(HEADER_F64).read() + open(HEADER_ML).read() + open(HEADER_NOALLOC).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(boris_(?:demag|llg|micro)_\w+)\s*\(", text)))
 
