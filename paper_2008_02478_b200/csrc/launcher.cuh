@@ -14,11 +14,19 @@
 
 namespace bd {
 
+// K::warp_local_after(PH) (optional): what phase PH + 1 reads of phase PH's shared-memory writes was written by threads of the
+// same warp, and what it overwrites no other warp reads in either phase: the block barrier between them becomes a warp barrier
+template <class K, class = void>
+struct WarpLocal { static BD_HD constexpr bool after(int) { return false; } };
+template <class K>
+struct WarpLocal<K, std::void_t<decltype(K::warp_local_after(0))>> { static BD_HD constexpr bool after(int ph) { return K::warp_local_after(ph); } };
+
 template <class K, int PH>
 __device__ __forceinline__ void run_phases(const typename K::Args& a, float2* sm) {
     K::template phase<PH>(threadIdx.x, blockIdx.x, blockIdx.y, a, sm);
     if constexpr (PH + 1 < K::NPHASES) {
-        __syncthreads();
+        if constexpr (WarpLocal<K>::after(PH)) __syncwarp();
+        else __syncthreads();
         run_phases<K, PH + 1>(a, sm);
     }
 }

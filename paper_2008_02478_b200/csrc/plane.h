@@ -422,6 +422,10 @@ struct YZFused {
     static constexpr int NIN = NQ == 1 ? R0 / 2 : R0;    // first-pass inputs that are not zero padding
     static_assert(NT % 16 == 0 && NT % R0 == 0 && NT % 4 == 0, "thread mapping");
     static BD_HD long smem_elems(const Args&) { return (long)NPEN * PITCH; }
+    // With R0 = 16 the 16 threads that run a pencil's first pass (phase 0) also run its radix-16 pass (phase 1), and
+    // likewise phases 3 and 4: those phases meet at a warp barrier, so the warps of a block drift apart and the global
+    // loads and stores of phases 0 and 4 overlap the arithmetic of phases 1 and 3 of other warps
+    static BD_HD constexpr bool warp_local_after(int ph) { return R0 == 16 && NT % 32 == 0 && (ph == 0 || ph == 3); }
 
     // blockIdx.x = kx NQ + o; residues q and NQ - q (which read each other's kernel-spectrum slots) are neighbours
     static BD_HD int q_of_order(int o) {

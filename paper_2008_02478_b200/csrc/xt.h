@@ -169,6 +169,22 @@ constexpr int XB = 4;     // independent items per trip of the post / pre loops
 template <int LX, int P, bool INV, int NT, class In, class Out>
 BD_HD void x_rows_pass(int tid, int nrows, const In& in, const Out& out, const float2* ptw) {
     constexpr int IPR = LX / dec_r(LX, P);                 // butterflies per row
+    constexpr int S = dec_sublen(LX, P) / dec_r(LX, P);    // stride of the pass
+    if constexpr (P >= 1 && S == 8 && 2 * IPR <= NT && NT % 16 == 0) {
+        // The middle pass of a three-pass length works on runs of 8 consecutive points (16 banks): the two runs of a
+        // half-warp are 64 points = 68 padded slots apart and overlap in 8 banks.  Rows 8 apart are 16 banks apart (the
+        // pitch is odd), so lanes 8..15 take the same run eight rows further down: no conflicts.
+        if ((nrows & 15) == 0) {
+            constexpr int G2 = NT / (2 * IPR);             // threads per butterfly and half of 8 rows
+            const int j = tid & 7, rh = (tid >> 3) & 1, rest = tid >> 4;
+            const int it = (rest % (IPR / 8)) * 8 + j, rl = rest / (IPR / 8);
+            for (int r16 = 0; r16 < nrows; r16 += 16) {
+                if constexpr (!INV) fwd_passM<LX, P>(it, r16 + 8 * rh + rl, G2, r16 + 8 * rh + 8, in, out, ptw);
+                else inv_passM<LX, P>(it, r16 + 8 * rh + rl, G2, r16 + 8 * rh + 8, in, out, ptw);
+            }
+            return;
+        }
+    }
     if constexpr (IPR <= NT) {
         constexpr int G = NT / IPR;
         const int it = tid % IPR, rg = tid / IPR;

@@ -160,6 +160,8 @@ CASES = [
     ((1, 128, 4), (2.0, 2.0, 1.0), "domains", 0),
     ((1, 4, 1024), (2.0, 2.0, 1.0), "random", 0),         # LX = 1024
     ((1, 8, 256), (4.0, 4.0, 4.0), "helix", 0),
+    ((1, 16, 256), (3.0, 4.0, 2.0), "random", 0),         # 16 rows per block: middle x pass with rows 8 apart in a half-warp
+    ((16, 4, 256), (2.0, 3.0, 1.0), "random", 0),         # tiled 3-D, nz = 16 rows of 256: the same mapping with 512 threads
     ((2, 2, 4), (2.0, 2.0, 1.0), "random", 0),            # smallest 3-D mesh
     ((4, 8, 16), (5.0, 4.0, 3.0), "random", 0),
     ((8, 16, 8), (2.0, 2.0, 1.0), "random", 3),           # chunked kx slots with a ragged last chunk
@@ -230,6 +232,7 @@ PLANE_CASES = [
     ((4, 512, 4), (2.0, 2.0, 1.0), "helix", 0),           # 4 cells, four residues
     ((2, 32, 16), (3.0, 2.0, 1.0), "random", 0),          # 2 cells: one lane, 4 frequencies
     ((2, 256, 4), (2.0, 2.0, 2.0), "random", 0),          # 2 cells, two residues
+    ((4, 32, 256), (2.0, 2.0, 1.0), "random", 0),         # plane-path x kernels at LX = 256: 16-row blocks, three x passes
     ((64, 32, 4), (2.0, 2.0, 1.0), "random", 1),          # 64 cells: eight lanes per column; LS = 64
     ((64, 128, 4), (2.0, 3.0, 2.0), "helix", 2),          # 64 cells, LS = 128, two residues
 ]
