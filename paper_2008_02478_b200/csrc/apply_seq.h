@@ -57,8 +57,19 @@ inline LaunchCfg make_launch_cfg(int nx, int ny, int nz) {
     c.cs = (int)(cs < 1 ? 1 : (cs > nx + 1 ? nx + 1 : cs));
     c.tiled = tiled_supported(nx, ny, nz) ? 1 : 0;
     c.cols = nz == 1 ? cols_for(Py) : cols_for3d(Py);
-    c.rbt = nx >= 512 ? 8 : 4096 / nx;
-    while (c.rbt > ny) c.rbt >>= 1;
+    // narrow 2-D meshes: narrower tiles, so that YFused's (nx + 1) / cols blocks reach at least half of the SMs
+    if (nz == 1) while (c.cols > 2 && (nx + c.cols) / c.cols < 74) c.cols >>= 1;
+    // rows per block of the tiled 2-D x kernels: about 384 blocks (one wave at 3 blocks per SM) where the mesh has the rows for
+    // it, at most 32 KB of rows, at least 8 rows up to nx = 256 and 2 from nx = 512 (measured: profiles/r02_plane.md)
+    {
+        int hi = nx >= 512 ? 8 : 4096 / nx;
+        while (hi > ny) hi >>= 1;
+        int lo = nx >= 512 ? 2 : (nx <= 32 ? 32 : 8);
+        if (lo > hi) lo = hi;
+        int r = 1;
+        while (2 * r <= 3 * ny / 384) r <<= 1;
+        c.rbt = r < lo ? lo : (r > hi ? hi : r);
+    }
     c.pf_y = 0; c.pf_xz = 0;       // set by the plan from the SM count
     c.plane = plane_geom(nx, ny, nz);
     // 64-cell slabs: where the nz rows of a (c, y) slab fit one SM the tiled kernels are as fast (measured: 256 x 256 x 64
@@ -139,7 +150,7 @@ int enqueue_tiled_2d(Launcher& run, const PlanView& p, const float* M, float* H)
     const Grid gy{(unsigned)ntl, 1};
     rc = dispatch_len(Py, [&](auto ic) {
         constexpr int L = decltype(ic)::value;
-        if constexpr (cols_for(L) == COLS) return run.template run<YFused<L, 4, COLS>>(gy, ya);
+        if constexpr (COLS <= cols_for(L)) return run.template run<YFused<L, 4, COLS>>(gy, ya);
         else return -1;
     });
     if (rc) return rc;

@@ -160,7 +160,7 @@ CASES = [
     ((1, 128, 4), (2.0, 2.0, 1.0), "domains", 0),
     ((1, 4, 1024), (2.0, 2.0, 1.0), "random", 0),         # LX = 1024
     ((1, 8, 256), (4.0, 4.0, 4.0), "helix", 0),
-    ((1, 16, 256), (3.0, 4.0, 2.0), "random", 0),         # 16 rows per block: middle x pass with rows 8 apart in a half-warp
+    ((1, 16, 256), (3.0, 4.0, 2.0), "random", 0),         # 2-D mesh of 16 rows of 256: 8 rows per block
     ((16, 4, 256), (2.0, 3.0, 1.0), "random", 0),         # tiled 3-D, nz = 16 rows of 256: the same mapping with 512 threads
     ((2, 2, 4), (2.0, 2.0, 1.0), "random", 0),            # smallest 3-D mesh
     ((4, 8, 16), (5.0, 4.0, 3.0), "random", 0),
