@@ -54,6 +54,10 @@ inline PlaneGeom plane_geom(int nx, int ny, int nz, int nq_force = 0) {
     const int lsmax = nz > 32 ? 128 : 256;           // 3 nz pencils of LS points in 227 KB
     int nq = 1;
     while (Py / nq > lsmax) nq *= 2;
+    // narrow meshes: more residues while the (nx + 1) nq blocks of YZFused still fit the SMs at once (measured on 148 SMs:
+    // 64 x 64 x 32 31.6 -> 25.6 us, 128 x 128 x 8 31.7 -> 23.5 us, 32 x 128 x 32 48 -> 30 us; profiles/r02_plane.md)
+    const int per_sm = nz >= 32 ? 1 : (nz >= 8 ? 32 / nz : 4);
+    while (nq < 8 && Py / (2 * nq) >= 64 && (long)(nx + 1) * nq * 2 <= 148L * per_sm) nq *= 2;
     if (nq_force > 0) nq = nq_force;
     if (nq != 1 && nq != 2 && nq != 4 && nq != 8) return g;
     const int ls = Py / nq;
