@@ -500,3 +500,27 @@ def test_tiled_3d_kernels_stay_reachable_on_slabs_the_plane_path_takes(shape, mo
     assert plan.layout()["path"] == 3
     assert_parity(gpu_apply(plan, M_host), demag_fft(M_host, h), Ms)
     plan.close()
+
+
+# ----------------------------------------------------------------- narrow meshes: launch geometry chosen for the SM count
+@pytest.mark.parametrize("shape,path", [((1, 64, 64), 2), ((1, 128, 512), 2), ((1, 256, 1024), 2), ((1, 1024, 128), 2), ((1, 512, 512), 2),
+                                        ((32, 64, 64), 4), ((32, 128, 32), 4), ((8, 128, 128), 4), ((16, 64, 64), 4)])
+def test_narrow_meshes_with_their_own_launch_geometry(shape, path):
+    """2-D: rows per block of the x kernels and columns per YFused tile follow the block count (make_launch_cfg);
+    slabs: extra ky residues while the blocks still fit the SMs at once (plane_geom).  Same parity bar."""
+    nz, ny, nx = shape
+    h, Ms = (3e-9, 2e-9, 1e-9), 8e5
+    M_host = W.make_texture("random", shape, Ms, seed=151)
+    plan = binding.DemagPlan(nx, ny, nz, *h)
+    assert plan.layout()["path"] == path
+    H, E = gpu_apply(plan, M_host, want_energy=True)
+    H_ref = demag_fft(M_host, h)
+    assert_parity(H, H_ref, Ms)
+    assert abs(E - demag_energy(M_host, H_ref, h)) <= TOL_E * abs(E)
+    M = torch.from_numpy(M_host).cuda()
+    H2 = torch.full_like(M, float("nan"))
+    E2 = plan.apply_energy(M, H2)
+    torch.cuda.synchronize()
+    assert np.array_equal(H2.cpu().numpy(), H)
+    assert abs(E2.item() - E) <= 1e-12 * abs(E)
+    plan.close()
