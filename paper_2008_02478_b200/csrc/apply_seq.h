@@ -73,8 +73,10 @@ inline LaunchCfg make_launch_cfg(int nx, int ny, int nz) {
     c.pf_y = 0; c.pf_xz = 0;       // set by the plan from the SM count
     c.plane = plane_geom(nx, ny, nz);
     // 64-cell slabs: where the nz rows of a (c, y) slab fit one SM the tiled kernels are as fast (measured: 256 x 256 x 64
-    // 0.478 against 0.497 ms); the plane path takes the slabs they cannot hold (nx >= 512), instead of the chunked kernels
-    if (nz == 64 && c.tiled) c.plane.on = 0;
+    // 0.493 against 0.515 ms, 128 x 128 x 64 0.134 against 0.138 ms) unless the mesh is narrow (64 x 64 x 64 60 against 46 us,
+    // 256 x 64 x 64 155 against 128 us, 64 x 256 x 64 173 against 153 us); the plane path also takes the slabs they cannot
+    // hold (nx >= 512), instead of the chunked kernels
+    if (nz == 64 && c.tiled && nx > 64 && ny > 64) c.plane.on = 0;
     return c;
 }
 

@@ -210,7 +210,8 @@ def test_float3_layout_and_accumulate_variants_match_the_oracle(shape):
 
 
 def test_kernel_path_chosen_per_mesh():
-    expect = {(1, 32, 32): 2, (1, 1024, 1024): 2, (128, 128, 128): 3, (32, 512, 512): 4, (32, 256, 16): 4, (32, 1024, 64): 4, (32, 64, 1024): 4, (16, 512, 512): 4, (8, 64, 64): 4, (16, 16, 64): 3, (4, 64, 64): 4, (2, 32, 32): 4, (4, 16, 64): 3, (64, 64, 512): 4, (64, 64, 256): 3, (32, 16, 1024): 0, (512, 2, 4): 0}
+    expect = {(1, 32, 32): 2, (1, 1024, 1024): 2, (128, 128, 128): 3, (32, 512, 512): 4, (32, 256, 16): 4, (32, 1024, 64): 4, (32, 64, 1024): 4, (16, 512, 512): 4, (8, 64, 64): 4, (16, 16, 64): 3, (4, 64, 64): 4, (2, 32, 32): 4, (4, 16, 64): 3, (64, 64, 512): 4, (64, 64, 256): 4, (64, 128, 128): 3, (64, 256, 256): 3,
+              (32, 16, 1024): 0, (512, 2, 4): 0}
     for (nz, ny, nx), path in expect.items():
         plan = binding.DemagPlan(nx, ny, nz, 2e-9, 2e-9, 1e-9)
         assert plan.layout()["path"] == path
@@ -504,7 +505,8 @@ def test_tiled_3d_kernels_stay_reachable_on_slabs_the_plane_path_takes(shape, mo
 
 # ----------------------------------------------------------------- narrow meshes: launch geometry chosen for the SM count
 @pytest.mark.parametrize("shape,path", [((1, 64, 64), 2), ((1, 128, 512), 2), ((1, 256, 1024), 2), ((1, 1024, 128), 2), ((1, 512, 512), 2),
-                                        ((32, 64, 64), 4), ((32, 128, 32), 4), ((8, 128, 128), 4), ((16, 64, 64), 4)])
+                                        ((32, 64, 64), 4), ((32, 128, 32), 4), ((8, 128, 128), 4), ((16, 64, 64), 4),
+                                        ((64, 64, 64), 4), ((64, 32, 128), 4), ((64, 128, 128), 3)])
 def test_narrow_meshes_with_their_own_launch_geometry(shape, path):
     """2-D: rows per block of the x kernels and columns per YFused tile follow the block count (make_launch_cfg);
     slabs: extra ky residues while the blocks still fit the SMs at once (plane_geom).  Same parity bar."""
