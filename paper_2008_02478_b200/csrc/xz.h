@@ -286,6 +286,74 @@ struct ZXInv {
         }
     }
 
+#if defined(__CUDA_ARCH__)
+    // The same column by SP lanes of one warp, lane p = its pass: u_p[z] = W_PZ^(-p z) (32-point inverse transform of the
+    // inputs p + SP k), then x[z + 32 m] = sum_p u_p[z] w^(p m), w = exp(2 pi i / SP), m < SP / 2, across the lanes: a
+    // radix-2 inverse transform over p truncated to its first half, one stage per lane distance D = T / 2 (T = SP, SP / 2, ..):
+    //   even m = 2 m':  sum_(p < D) (u_p + u_(p+D)) w_D^(p m'),      odd m = 2 m' + 1:  sum_(p < D) (u_p - u_(p+D)) w_T^p w_D^(p m')
+    // - two problems of half the size.  Lane p < D keeps the lower half of the z range of both, lane p + D the upper half: a lane
+    // always holds 32 values (2^s vectors of 32 / 2^s points) and ends with the SP / 2 outputs m of the 32 / SP points z from
+    // z = p 32 / SP on.  (The last stage, T = 2, has only m' = 0.)  Every lane of the warp must call (full-mask shuffles).
+    template <int T, int NV>
+    static __device__ __forceinline__ void lanes_stage(float2 (&a)[32], int p, const float2* __restrict__ ztw) {
+        constexpr int D = T / 2, LEN = 32 / NV, HL = LEN / 2;
+        const bool hi = (p & D) != 0;
+        const float sg = hi ? -1.f : 1.f;
+        float2 b[32];
+        Tw w;
+        if constexpr (T > 2) w = make_tw(BD_LDG(&ztw[(p & (D - 1)) * (PZ / T)]));
+        BD_UNROLL
+        for (int v = 0; v < NV; ++v) {
+            BD_UNROLL
+            for (int z = 0; z < HL; ++z) {
+                const float2 lo = a[v * LEN + z], up = a[v * LEN + HL + z];
+                const float2 mine = hi ? up : lo, send = hi ? lo : up;
+                float2 oth;
+                oth.x = __shfl_xor_sync(0xffffffffu, send.x, D);
+                oth.y = __shfl_xor_sync(0xffffffffu, send.y, D);
+                if constexpr (T > 2) {
+                    b[(2 * v) * HL + z] = pk_add(mine, oth);
+                    b[(2 * v + 1) * HL + z] = pk_cmulc(pk_mul(pk_sub(mine, oth), pk_bc(sg)), w);
+                } else {
+                    b[v * HL + z] = pk_add(mine, oth);
+                }
+            }
+        }
+        BD_UNROLL
+        for (int i = 0; i < (T > 2 ? 32 : 16); ++i) a[i] = b[i];
+        if constexpr (T > 2) lanes_stage<T / 2, 2 * NV>(a, p, ztw);
+    }
+    static __device__ __forceinline__ void zcolumn_lanes(const float2* in, float2* col, long kzs, int p, bool active,
+                                                         const float2* __restrict__ ztw) {
+        constexpr int SUB = ZSplit<NZ>::SUB, SP = ZSplit<NZ>::SP;
+        static_assert(SUB == 32 && (SP == 4 || SP == 8 || SP == 16), "32-point passes on 4, 8 or 16 lanes");
+        float2 v[32];
+        if (active) {
+            const float2* ip = in + p * kzs;
+            BD_UNROLL
+            for (int k = 0; k < SUB; ++k) { v[k] = BD_LDCG(ip); ip += SP * kzs; }
+        } else {
+            BD_UNROLL
+            for (int k = 0; k < SUB; ++k) v[k] = bd_f2(0.f, 0.f);
+        }
+        PkDft<SUB, +1>::run(v);
+        BD_UNROLL
+        for (int z = 1; z < SUB; ++z) v[z] = pk_cmulc2(v[z], BD_LDG(&ztw[p * z]));
+        lanes_stage<SP, 1>(v, p, ztw);
+        if (!active) return;
+        // vector i of the result is output m = bit-reversed i (the first stage's parity is the top bit of i)
+        constexpr int NVF = SP / 2, ZL = 32 / SP, LB = SP == 4 ? 1 : (SP == 8 ? 2 : 3);
+        BD_UNROLL
+        for (int i = 0; i < NVF; ++i) {
+            int m = 0;
+            BD_UNROLL
+            for (int bit = 0; bit < LB; ++bit) m |= ((i >> bit) & 1) << (LB - 1 - bit);
+            BD_UNROLL
+            for (int z = 0; z < ZL; ++z) BD_STS(col + (p * ZL + z + SUB * m) * PITCH, v[i * ZL + z]);
+        }
+    }
+#endif
+
     // frequencies kz = 2k + PAR of one column -> their part of x[z]; the odd half adds to
     // what the even half left in shared memory.  Column 0 carries P^ = Y0^ + i YN^.
     // nq: the Nyquist column, spread over the lanes of warp 0 (lane l holds kz = l and l + 32); only
@@ -340,11 +408,23 @@ struct ZXInv {
             const long kzs = (long)a.ntl * a.ny * cols;
             const float2* vc = a.V + (long)c * PZ * kzs;
             if constexpr (ZSplit<NZ>::ON) {
+#if defined(__CUDA_ARCH__)
+                // one (column, pass) per lane, the SP passes of a column on neighbouring lanes (whole warps make the trips)
+                constexpr int SP = ZSplit<NZ>::SP;
+                for (int w = tid; (w & ~31) < (LX + 1) * SP; w += NT) {
+                    const bool active = w < (LX + 1) * SP;
+                    const int kx = active ? w / SP : 0, p = w % SP;
+                    const float2* in = vc + ((long)((kx >> a.cs) * a.ny + y) << a.cs) + (kx & (cols - 1));
+                    float2* col = sm + (kx == LX ? prow(LX, LX) : xz_pos(a.xpost, LX, kx));
+                    zcolumn_lanes(in, col, kzs, p, active, a.ztw);
+                }
+#else
                 for (int kx = tid; kx <= LX; kx += NT) {
                     const float2* in = vc + ((long)((kx >> a.cs) * a.ny + y) << a.cs) + (kx & (cols - 1));
                     float2* col = sm + (kx == LX ? prow(LX, LX) : xz_pos(a.xpost, LX, kx));
                     zcolumn(in, col, kzs, a.ztw);
                 }
+#endif
             } else {
                 const float2* inn = vc + ((long)((LX >> a.cs) * a.ny + y) << a.cs) + (LX & (cols - 1));
                 float2 nq[NQ];

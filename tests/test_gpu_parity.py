@@ -506,7 +506,8 @@ def test_tiled_3d_kernels_stay_reachable_on_slabs_the_plane_path_takes(shape, mo
 # ----------------------------------------------------------------- narrow meshes: launch geometry chosen for the SM count
 @pytest.mark.parametrize("shape,path", [((1, 64, 64), 2), ((1, 128, 512), 2), ((1, 256, 1024), 2), ((1, 1024, 128), 2), ((1, 512, 512), 2),
                                         ((32, 64, 64), 4), ((32, 128, 32), 4), ((8, 128, 128), 4), ((16, 64, 64), 4),
-                                        ((64, 64, 64), 4), ((64, 32, 128), 4), ((64, 128, 128), 3)])
+                                        ((64, 64, 64), 4), ((64, 32, 128), 4), ((64, 128, 128), 3),
+                                        ((256, 4, 32), 3), ((128, 8, 64), 3), ((64, 16, 4), 3)])      # z columns on 16, 8, 4 lanes (ZXInv)
 def test_narrow_meshes_with_their_own_launch_geometry(shape, path):
     """2-D: rows per block of the x kernels and columns per YFused tile follow the block count (make_launch_cfg);
     slabs: extra ky residues while the blocks still fit the SMs at once (plane_geom).  Same parity bar."""
