@@ -323,8 +323,11 @@ struct ZXInv {
         for (int i = 0; i < (T > 2 ? 32 : 16); ++i) a[i] = b[i];
         if constexpr (T > 2) lanes_stage<T / 2, 2 * NV>(a, p, ztw);
     }
-    static __device__ __forceinline__ void zcolumn_lanes(const float2* in, float2* col, long kzs, int p, bool active,
-                                                         const float2* __restrict__ ztw) {
+    // inn / coln (column 0 only, else null): the Nyquist column kx = LX rides along as the imaginary part, P^ = Y0^ + i YN^ —
+    // both are spectra of real columns, so the transform of P^ has x0 in its real and xN in its imaginary part; column 0
+    // keeps the pair (the x pre-pass reads its real part only), the Nyquist slot gets (xN, 0)
+    static __device__ __forceinline__ void zcolumn_lanes(const float2* in, const float2* inn, float2* col, float2* coln, long kzs, int p,
+                                                         bool active, const float2* __restrict__ ztw) {
         constexpr int SUB = ZSplit<NZ>::SUB, SP = ZSplit<NZ>::SP;
         static_assert(SUB == 32 && (SP == 4 || SP == 8 || SP == 16), "32-point passes on 4, 8 or 16 lanes");
         float2 v[32];
@@ -332,6 +335,11 @@ struct ZXInv {
             const float2* ip = in + p * kzs;
             BD_UNROLL
             for (int k = 0; k < SUB; ++k) { v[k] = BD_LDCG(ip); ip += SP * kzs; }
+            if (inn) {
+                const float2* np = inn + p * kzs;
+                BD_UNROLL
+                for (int k = 0; k < SUB; ++k) { const float2 n = BD_LDCG(np); np += SP * kzs; v[k] = bd_f2(v[k].x - n.y, v[k].y + n.x); }
+            }
         } else {
             BD_UNROLL
             for (int k = 0; k < SUB; ++k) v[k] = bd_f2(0.f, 0.f);
@@ -349,7 +357,10 @@ struct ZXInv {
             BD_UNROLL
             for (int bit = 0; bit < LB; ++bit) m |= ((i >> bit) & 1) << (LB - 1 - bit);
             BD_UNROLL
-            for (int z = 0; z < ZL; ++z) BD_STS(col + (p * ZL + z + SUB * m) * PITCH, v[i * ZL + z]);
+            for (int z = 0; z < ZL; ++z) {
+                BD_STS(col + (p * ZL + z + SUB * m) * PITCH, v[i * ZL + z]);
+                if (coln) BD_STS(coln + (p * ZL + z + SUB * m) * PITCH, bd_f2(v[i * ZL + z].y, 0.f));
+            }
         }
     }
 #endif
@@ -411,12 +422,13 @@ struct ZXInv {
 #if defined(__CUDA_ARCH__)
                 // one (column, pass) per lane, the SP passes of a column on neighbouring lanes (whole warps make the trips)
                 constexpr int SP = ZSplit<NZ>::SP;
-                for (int w = tid; (w & ~31) < (LX + 1) * SP; w += NT) {
-                    const bool active = w < (LX + 1) * SP;
-                    const int kx = active ? w / SP : 0, p = w % SP;
+                const float2* inn = vc + ((long)((LX >> a.cs) * a.ny + y) << a.cs) + (LX & (cols - 1));
+                for (int w = tid; (w & ~31) < LX * SP; w += NT) {
+                    const bool active = w < LX * SP;
+                    const int kx = active ? w / SP : 1, p = w % SP;
                     const float2* in = vc + ((long)((kx >> a.cs) * a.ny + y) << a.cs) + (kx & (cols - 1));
-                    float2* col = sm + (kx == LX ? prow(LX, LX) : xz_pos(a.xpost, LX, kx));
-                    zcolumn_lanes(in, col, kzs, p, active, a.ztw);
+                    float2* col = sm + xz_pos(a.xpost, LX, kx);
+                    zcolumn_lanes(in, kx == 0 ? inn : nullptr, col, kx == 0 ? sm + prow(LX, LX) : nullptr, kzs, p, active, a.ztw);
                 }
 #else
                 for (int kx = tid; kx <= LX; kx += NT) {
