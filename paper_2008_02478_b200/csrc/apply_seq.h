@@ -38,7 +38,7 @@ constexpr long kMaxDynSmem = 227L * 1024;
 // z column (2 nz points) in registers
 inline bool tiled_supported(int nx, int ny, int nz) {
     if (nz == 1) return true;
-    return nz <= 256 && (long)nz * ((prow(nx, nx) + 1) | 1) * (long)sizeof(float2) <= kMaxDynSmem;
+    return nz <= 256 && ((long)nz * ((prow(nx, nx) + 1) | 1) + (nz > 32 ? 2 * nz : 0)) * (long)sizeof(float2) <= kMaxDynSmem;
 }
 
 inline LaunchCfg make_launch_cfg(int nx, int ny, int nz) {

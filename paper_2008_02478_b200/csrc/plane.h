@@ -243,9 +243,12 @@ BD_HD float2 pl_w8(int m) {
     }
 }
 
+// zt: the block's copy of the z twiddles in shared memory, zt[j ZS + p] = (plane_fill_zt)[p 16 + j] (the lanes of a column are
+// neighbours: one wavefront per load)
 template <int NZ>
 BD_HD void pl_zlane(int p, float sy, const float2* col, int pitch, const PlK<(NZ >= 8 ? 2 : 1)>& k, long kcs, long khs,
-                    const float2* __restrict__ zt, float2 (&v)[3][16]) {
+                    const float2* zt, float2 (&v)[3][16]) {
+    constexpr int ZSL = NZ >= 8 ? 2 * NZ / 16 : 1;
     // first stage of the 2 NZ-point transform of the NZ cells, split by the residue p of kz modulo ZS = NZ / 8 and pruned to
     // its non-zero inputs:  a_p[j] = W_Pz^(j p) sum_{r < ZS/2} x[j + 16 r] W_ZS^(r p)
     if constexpr (NZ == 64) {
@@ -259,7 +262,7 @@ BD_HD void pl_zlane(int p, float sy, const float2* col, int pitch, const PlK<(NZ
         for (int c = 0; c < 3; ++c) {
             BD_UNROLL
             for (int j = 0; j < 16; ++j) {
-                const Tw t = make_tw(BD_LDG(&zt[p * 16 + j]));
+                const Tw t = make_tw(zt[j * ZSL + p]);
                 const float2 x0 = col[(c * 64 + j) * pitch], x1 = col[(c * 64 + j + 16) * pitch];
                 const float2 x2 = col[(c * 64 + j + 32) * pitch], x3 = col[(c * 64 + j + 48) * pitch];
                 float2 a = pk_fma(pk_swap(x2), rot.ns, pk_fma(x2, pk_bc(rot.c), x0));
@@ -281,7 +284,7 @@ BD_HD void pl_zlane(int p, float sy, const float2* col, int pitch, const PlK<(NZ
         for (int c = 0; c < 3; ++c) {
             BD_UNROLL
             for (int j = 0; j < 16; ++j) {
-                const Tw t = make_tw(BD_LDG(&zt[p * 16 + j]));
+                const Tw t = make_tw(zt[j * ZSL + p]);
                 const float2 x0 = cr[j >> 2][(c * 32 + (j & 3)) * pitch], x1 = cr[j >> 2][(c * 32 + (j & 3) + 16) * pitch];
                 const float2 a = pk_fma(pk_swap(x1), rot.ns, pk_fma(x1, pk_bc(rot.c), x0));
                 v[c][j] = pk_cmul(a, t);
@@ -295,7 +298,7 @@ BD_HD void pl_zlane(int p, float sy, const float2* col, int pitch, const PlK<(NZ
         for (int c = 0; c < 3; ++c) {
             BD_UNROLL
             for (int j = 0; j < 16; ++j)
-                v[c][j] = pk_cmul(cr[j >> 3][(c * 16 + (j & 7)) * pitch], make_tw(BD_LDG(&zt[p * 16 + j])));
+                v[c][j] = pk_cmul(cr[j >> 3][(c * 16 + (j & 7)) * pitch], make_tw(zt[j * ZSL + p]));
             PkDft<16, -1>::run(v[c]);
         }
     } else {
@@ -339,7 +342,7 @@ BD_HD void pl_zlane(int p, float sy, const float2* col, int pitch, const PlK<(NZ
         for (int c = 0; c < 3; ++c) PkDft<16, +1>::run(v[c]);
         BD_UNROLL
         for (int j = 0; j < 16; ++j) {
-            const Tw t = make_tw(BD_LDG(&zt[p * 16 + j]));
+            const Tw t = make_tw(zt[j * ZSL + p]);
             BD_UNROLL
             for (int c = 0; c < 3; ++c) v[c][j] = pk_cmulc(v[c][j], t);
         }
@@ -425,7 +428,7 @@ struct YZFused {
     static constexpr int LSP = NQ == 1 ? LS / 2 : LS;    // stored points of a partial plane
     static constexpr int NIN = NQ == 1 ? R0 / 2 : R0;    // first-pass inputs that are not zero padding
     static_assert(NT % 16 == 0 && NT % R0 == 0 && NT % 4 == 0, "thread mapping");
-    static BD_HD long smem_elems(const Args&) { return (long)NPEN * PITCH; }
+    static BD_HD long smem_elems(const Args&) { return (long)NPEN * PITCH + ZS * 16; }      // pencils, then the z twiddles
     // With R0 = 16 the 16 threads that run a pencil's first pass (phase 0) also run its radix-16 pass (phase 1), and
     // likewise phases 3 and 4: those phases meet at a warp barrier, so the warps of a block drift apart and the global
     // loads and stores of phases 0 and 4 overlap the arithmetic of phases 1 and 3 of other warps
@@ -578,7 +581,7 @@ struct YZFused {
             PlK<NH> kc;
             const float sy = lists(w, kc);
             float2 y[3][16];
-            pl_zlane<NZ>(p, sy, col, PITCH, kc, KCS, KHS, a.zt, y);
+            pl_zlane<NZ>(p, sy, col, PITCH, kc, KCS, KHS, sm + NPEN * PITCH, y);
             if constexpr (ZS == 4) {
                 // out[j] = sum_p y_p[j], out[j + 16] = sum_p i^p y_p[j].  The lane keeps j = 4 p + i, i < 4: its own values
                 // sit in slots i, those of lane p + r (mod 4) in that lane's slots 16 - 4 r + i (pl_zrot): three rounds, the
@@ -661,7 +664,7 @@ struct YZFused {
             for (int pp = 0; pp < ZS; ++pp) {
                 PlK<NH> k;
                 const float sy = lists(w + pp, k);
-                pl_zlane<NZ>(pp, sy, col, PITCH, k, KCS, KHS, a.zt, y[pp]);
+                pl_zlane<NZ>(pp, sy, col, PITCH, k, KCS, KHS, sm + NPEN * PITCH, y[pp]);
             }
             for (int c = 0; c < 3; ++c)
                 for (int j = 0; j < 16; ++j) {
@@ -705,6 +708,7 @@ struct YZFused {
     static BD_HD void phase(int tid, int bx, int by, const Args& a, float2* sm) {
         const int kx = bx / NQ, q = q_of_order(bx % NQ);
         if constexpr (PH == 0) {
+            for (int i = tid; i < ZS * 16; i += NT) sm[NPEN * PITCH + i] = BD_LDG(&a.zt[(i % ZS) * 16 + i / ZS]);
             if (q == 0) load_pass<0>(tid, kx, a, sm);
             if constexpr (NQ >= 2) { if (q == 1) load_pass<1>(tid, kx, a, sm); }
             if constexpr (NQ >= 4) { if (q == 2) load_pass<2>(tid, kx, a, sm); else if (q == 3) load_pass<3>(tid, kx, a, sm); }

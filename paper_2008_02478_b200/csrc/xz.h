@@ -133,10 +133,12 @@ struct XZFwd {
     static constexpr int NPHASES = NP + 2;
     static constexpr int PZ = 2 * NZ;
     static constexpr int PITCH = SRows<LX>::PITCH;
-    static BD_HD long smem_elems(const Args&) { return (long)NZ * PITCH; }
+    // nz > 32: behind the rows, the twiddles of the z passes in the order the lanes read them, stw[z SP + p] = W_PZ^(p z)
+    // (neighbouring lanes = neighbouring passes of a column: one wavefront per load, and no global load in the z stage)
+    static BD_HD long smem_elems(const Args&) { return (long)NZ * PITCH + (ZSplit<NZ>::ON ? PZ : 0); }
 
     // pass p of one column (nz > 32, ZSplit): frequencies kz = SP k + p
-    static BD_HD void zpass(const float2* col, float2* out, long kzs, int p, const float2* __restrict__ ztw) {
+    static BD_HD void zpass(const float2* col, float2* out, long kzs, int p, const float2* __restrict__ ztw, const float2* stw) {
         constexpr int SUB = ZSplit<NZ>::SUB, SP = ZSplit<NZ>::SP;
         float2 v[SUB];
         BD_UNROLL
@@ -148,7 +150,7 @@ struct XZFwd {
         }
         if (p != 0) {
             BD_UNROLL
-            for (int z = 1; z < SUB; ++z) v[z] = pk_cmul2(v[z], BD_LDG(&ztw[p * z]));
+            for (int z = 1; z < SUB; ++z) v[z] = pk_cmul2(v[z], stw[z * SP + p]);
         }
         PkDft<SUB, -1>::run(v);
         out += p * kzs;
@@ -194,6 +196,10 @@ struct XZFwd {
                 for (int o = tid; o < NZ * LPR; o += NT)
                     bd_prefetch_l2(mn + (long)(o / LPR) * a.ny * LX * 4 + (o % LPR) * 128);
             }
+            if constexpr (ZSplit<NZ>::ON) {
+                constexpr int SP = ZSplit<NZ>::SP;
+                for (int i = tid; i < PZ; i += NT) sm[NZ * PITCH + i] = BD_LDG(&a.ztw[((i % SP) * (i / SP)) & (PZ - 1)]);
+            }
             x_rows_pass<LX, 0, false, NT>(tid, NZ, in, s, a.ptw);
         } else if constexpr (PH < NP) {
             x_rows_pass<LX, PH, false, NT>(tid, NZ, s, s, a.ptw);
@@ -229,7 +235,7 @@ struct XZFwd {
                     const int kx = w / SP, p = w - kx * SP;
                     const float2* col = sm + (kx == LX ? prow(LX, LX) : xz_pos(a.xpost, LX, kx));
                     float2* out = vc + ((long)((kx >> a.cs) * a.ny + y) << a.cs) + (kx & (cols - 1));
-                    zpass(col, out, kzs, p, a.ztw);
+                    zpass(col, out, kzs, p, a.ztw, sm + NZ * PITCH);
                 }
             } else {
                 for (int kx = tid; kx < LX; kx += NT) {
@@ -254,7 +260,7 @@ struct ZXInv {
     static constexpr int NPHASES = NP + 2;
     static constexpr int PZ = 2 * NZ;
     static constexpr int PITCH = SRows<LX>::PITCH;
-    static BD_HD long smem_elems(const Args&) { return (long)NZ * PITCH; }
+    static BD_HD long smem_elems(const Args&) { return (long)NZ * PITCH + (ZSplit<NZ>::ON ? PZ : 0); }     // + the twiddle table of XZFwd
 
     // all passes of one column (nz > 32, ZSplit)
     static BD_HD void zcolumn(const float2* in, float2* col, long kzs, const float2* __restrict__ ztw) {
@@ -327,7 +333,7 @@ struct ZXInv {
     // both are spectra of real columns, so the transform of P^ has x0 in its real and xN in its imaginary part; column 0
     // keeps the pair (the x pre-pass reads its real part only), the Nyquist slot gets (xN, 0)
     static __device__ __forceinline__ void zcolumn_lanes(const float2* in, const float2* inn, float2* col, float2* coln, long kzs, int p,
-                                                         bool active, const float2* __restrict__ ztw) {
+                                                         bool active, const float2* __restrict__ ztw, const float2* stw) {
         constexpr int SUB = ZSplit<NZ>::SUB, SP = ZSplit<NZ>::SP;
         static_assert(SUB == 32 && (SP == 4 || SP == 8 || SP == 16), "32-point passes on 4, 8 or 16 lanes");
         float2 v[32];
@@ -346,7 +352,7 @@ struct ZXInv {
         }
         PkDft<SUB, +1>::run(v);
         BD_UNROLL
-        for (int z = 1; z < SUB; ++z) v[z] = pk_cmulc2(v[z], BD_LDG(&ztw[p * z]));
+        for (int z = 1; z < SUB; ++z) v[z] = pk_cmulc2(v[z], stw[z * SP + p]);
         lanes_stage<SP, 1>(v, p, ztw);
         if (!active) return;
         // vector i of the result is output m = bit-reversed i (the first stage's parity is the top bit of i)
@@ -423,12 +429,14 @@ struct ZXInv {
                 // one (column, pass) per lane, the SP passes of a column on neighbouring lanes (whole warps make the trips)
                 constexpr int SP = ZSplit<NZ>::SP;
                 const float2* inn = vc + ((long)((LX >> a.cs) * a.ny + y) << a.cs) + (LX & (cols - 1));
+                for (int i = tid; i < PZ; i += NT) sm[NZ * PITCH + i] = BD_LDG(&a.ztw[((i % SP) * (i / SP)) & (PZ - 1)]);
+                __syncthreads();
                 for (int w = tid; (w & ~31) < LX * SP; w += NT) {
                     const bool active = w < LX * SP;
                     const int kx = active ? w / SP : 1, p = w % SP;
                     const float2* in = vc + ((long)((kx >> a.cs) * a.ny + y) << a.cs) + (kx & (cols - 1));
                     float2* col = sm + xz_pos(a.xpost, LX, kx);
-                    zcolumn_lanes(in, kx == 0 ? inn : nullptr, col, kx == 0 ? sm + prow(LX, LX) : nullptr, kzs, p, active, a.ztw);
+                    zcolumn_lanes(in, kx == 0 ? inn : nullptr, col, kx == 0 ? sm + prow(LX, LX) : nullptr, kzs, p, active, a.ztw, sm + NZ * PITCH);
                 }
 #else
                 for (int kx = tid; kx <= LX; kx += NT) {
